@@ -1,0 +1,143 @@
+/*
+ * strata_na3d.h -- C ABI of libstrata_na3d.so: StereoRoPE + 3D neighbourhood attention for sm_100a.
+ *
+ * The one data-parallel hot path of STRATA's transformer (arxiv/paper_2606_31248):
+ *   PAPER.md:79     "3D Neighborhood Attention (NATTEN), with stereographic rotary position
+ *                    embeddings inside local (x,y,lev) windows"
+ *   PAPER.md:93-99  StereoRoPE: tile-centred stereographic coordinates (eq. (1)) "replace
+ *                    row/column indices as inputs to axial 2D RoPE"
+ * For every query token i = (l, y, x) of a (L x Y x X) token grid and every head:
+ *   phi[t][j]   = sum_a coords[t][a] * freqs[a][j]                      rotary angle, j < d/2
+ *   qrot, krot  = each channel pair of q, k rotated by phi (V is not rotated)
+ *   window(i)   = box of k_L x k_Y x k_X keys starting at clamp(i_a - floor(k_a/2), 0, n_a - k_a)
+ *                 on every axis (inward-clamped NATTEN window, reading R1)
+ *   s_ij        = scale * qrot_i . krot_j,  j in window(i)
+ *   lse_i       = ln sum_j exp(s_ij)                                      (natural log)
+ *   o_i         = sum_j exp(s_ij - lse_i) v_j
+ * and, for the backward, dq, dk, dv of  sum_i dO_i . o_i  including the transpose rotation R(-phi)
+ * (no gradient flows to coords, freqs or through lse).
+ *
+ * Conventions common to every entry point
+ *   - Tensors are contiguous in the fixed layouts below; base pointers must be 16-byte aligned.
+ *       q, k, v, o, d_o, dq, dk, dv : [B, L, Y, X, H, d]   element type desc->dtype
+ *       lse                         : [B, H, L, Y, X]      float32
+ *       coords                      : [B, L, Y, X, A]      float32  (A = desc->rope_axes)
+ *       freqs                       : [A, d/2]             float32
+ *   - Device entry points take DEVICE pointers owned by the caller; the library allocates no
+ *     device memory (scratch comes from `workspace`), never frees caller memory, never
+ *     synchronises, and enqueues all work on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  They are safe to capture in a CUDA graph.
+ *   - `_host` entry points take HOST pointers (pinned memory recommended) plus a DEVICE workspace;
+ *     they enqueue H2D copies, the same kernels, and D2H copies on `stream` and return without
+ *     synchronising: the caller synchronises the stream before reading the outputs.
+ *   - Outputs are fully overwritten (gradients are not accumulated into).
+ *   - Errors are return codes only: no exceptions, no abort, no printing.
+ *       INVALID_ARG  null required pointer, misaligned pointer, odd or non-positive head_dim,
+ *                    window[a] < 1 or > grid[a], non-positive sizes, bad enum value
+ *       UNSUPPORTED  legal but not implemented (head_dim not in {32, 64, 128}; rope_axes > 3;
+ *                    impl = TCGEN05 for a shape the tensor-core path does not cover)
+ *       WORKSPACE    workspace null or smaller than the *_workspace_bytes query says
+ *       CUDA         a CUDA runtime / driver call failed (cudaGetLastError is consumed)
+ */
+#ifndef STRATA_NA3D_H_
+#define STRATA_NA3D_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  STRATA_OK = 0,
+  STRATA_ERR_INVALID_ARG = 1,
+  STRATA_ERR_UNSUPPORTED = 2,
+  STRATA_ERR_WORKSPACE = 3,
+  STRATA_ERR_CUDA = 4
+} strata_status_t;
+
+typedef enum { STRATA_DTYPE_F32 = 0, STRATA_DTYPE_BF16 = 1 } strata_dtype_t;
+
+/* Which channels form a rotary pair: (2j, 2j+1) [complex form of RoFormer] or (j, j + d/2). */
+typedef enum { STRATA_ROPE_INTERLEAVED = 0, STRATA_ROPE_HALF = 1 } strata_rope_pairing_t;
+
+/* Kernel family.  AUTO picks the tcgen05 tensor-core kernels when they cover the problem
+ * (bf16, see strata_na3d_impl_selected) and the fp32 CUDA-core kernels otherwise. */
+typedef enum { STRATA_IMPL_AUTO = 0, STRATA_IMPL_SIMT = 1, STRATA_IMPL_TCGEN05 = 2 } strata_impl_t;
+
+typedef struct {
+  int32_t batch, heads, head_dim; /* B, H, d; d in {32, 64, 128}                               */
+  int32_t grid[3];                /* L, Y, X (levels, y, x), each >= 1                          */
+  int32_t window[3];              /* k_L, k_Y, k_X with 1 <= k_a <= grid[a]; even sizes allowed */
+  int32_t rope_axes;              /* A: 0 = no RoPE, 2 = (x, y) [paper], 3 = (x, y, level)      */
+  int32_t rope_pairing;           /* strata_rope_pairing_t                                      */
+  int32_t dtype;                  /* strata_dtype_t of q, k, v, o, d_o, dq, dk, dv              */
+  int32_t impl;                   /* strata_impl_t                                              */
+  float scale;                    /* softmax scale; <= 0 means 1/sqrt(head_dim)                 */
+} strata_na3d_desc_t;
+
+/* Bytes of DEVICE scratch the device entry points need for this problem (backward != 0: for
+ * strata_na3d_bwd).  0 on an invalid descriptor.  PAPER.md has no counterpart; the scratch holds
+ * the rotary tables / rotated operands (A1, A2) and the backward's row statistics (B1). */
+size_t strata_na3d_workspace_bytes(const strata_na3d_desc_t* desc, int backward);
+
+/* Bytes of DEVICE scratch the _host entry points need (staging for every tensor + the above). */
+size_t strata_na3d_host_workspace_bytes(const strata_na3d_desc_t* desc, int backward);
+
+/* Kernel family AUTO resolves to for this descriptor (a strata_impl_t), or -1 if invalid. */
+int strata_na3d_impl_selected(const strata_na3d_desc_t* desc, int backward);
+
+/* Forward: A1-A6 of DESIGN.md.  Reads q, k, v, coords, freqs; writes o and
+ * lse.  coords / freqs may be NULL iff rope_axes == 0. */
+strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc,
+                                const void* q, const void* k, const void* v,
+                                const float* coords, const float* freqs,
+                                void* o, float* lse,
+                                void* workspace, size_t workspace_bytes, void* stream);
+
+/* Backward: B1-B4 of DESIGN.md.  o and lse are the forward's outputs for the same inputs.
+ * Writes dq, dk, dv (same layout and dtype as q). */
+strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc,
+                                const void* q, const void* k, const void* v,
+                                const void* o, const void* d_o, const float* lse,
+                                const float* coords, const float* freqs,
+                                void* dq, void* dk, void* dv,
+                                void* workspace, size_t workspace_bytes, void* stream);
+
+/* Same operations on HOST buffers; `workspace` is DEVICE memory of at least
+ * strata_na3d_host_workspace_bytes().  Asynchronous on `stream`. */
+strata_status_t strata_na3d_fwd_host(const strata_na3d_desc_t* desc,
+                                     const void* q, const void* k, const void* v,
+                                     const float* coords, const float* freqs,
+                                     void* o, float* lse,
+                                     void* workspace, size_t workspace_bytes, void* stream);
+
+strata_status_t strata_na3d_bwd_host(const strata_na3d_desc_t* desc,
+                                     const void* q, const void* k, const void* v,
+                                     const void* o, const void* d_o, const float* lse,
+                                     const float* coords, const float* freqs,
+                                     void* dq, void* dk, void* dv,
+                                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* Number of kernel launches the last successful call on this thread enqueued (for bench.py's
+ * `gpu_launches`; memcpy nodes are not counted). */
+int strata_na3d_last_launch_count(void);
+
+/* Per-kernel device timing for bench.py's roofline line.  While profiling is enabled (per host
+ * thread), every kernel a device entry point launches is bracketed by CUDA events recorded on
+ * `stream` (up to 4096 kernels; later ones are not recorded).  After the caller has synchronised
+ * the stream, strata_na3d_profile_read copies the durations (milliseconds, launch order) of all
+ * kernels recorded since profiling was enabled into ms[0..capacity) and returns their number (-1 if
+ * an event query failed); names[i], if names != NULL, receives a static string naming kernel i.
+ * strata_na3d_set_profiling(1) also clears the record.  Do not enable it while capturing a graph. */
+void strata_na3d_set_profiling(int enable);
+int strata_na3d_profile_read(float* ms, const char** names, int capacity);
+
+const char* strata_status_string(strata_status_t status);
+int strata_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STRATA_NA3D_H_ */

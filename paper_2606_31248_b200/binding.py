@@ -1,0 +1,249 @@
+"""Thin ctypes binding of libstrata_na3d.so (include/strata_na3d.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; nothing here computes.  PyTorch
+supplies device memory and streams.  There is no CPU fallback: if the library is missing or a call
+fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence, Tuple
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libstrata_na3d.so")
+
+STRATA_OK = 0
+DTYPE_F32, DTYPE_BF16 = 0, 1
+ROPE_INTERLEAVED, ROPE_HALF = 0, 1
+IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05 = 0, 1, 2
+
+EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
+           "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",
+           "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
+           "strata_status_string", "strata_version")
+
+
+class StrataError(RuntimeError):
+    pass
+
+
+class _CDesc(ctypes.Structure):
+    _fields_ = [("batch", ctypes.c_int32), ("heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("grid", ctypes.c_int32 * 3), ("window", ctypes.c_int32 * 3),
+                ("rope_axes", ctypes.c_int32), ("rope_pairing", ctypes.c_int32),
+                ("dtype", ctypes.c_int32), ("impl", ctypes.c_int32), ("scale", ctypes.c_float)]
+
+
+@dataclass(frozen=True)
+class NA3DDesc:
+    """Mirror of strata_na3d_desc_t."""
+    batch: int
+    heads: int
+    head_dim: int
+    grid: Tuple[int, int, int]
+    window: Tuple[int, int, int]
+    rope_axes: int = 2
+    rope_pairing: int = ROPE_INTERLEAVED
+    dtype: int = DTYPE_BF16
+    impl: int = IMPL_AUTO
+    scale: float = 0.0
+
+    def c(self) -> _CDesc:
+        return _CDesc(self.batch, self.heads, self.head_dim, (ctypes.c_int32 * 3)(*self.grid),
+                      (ctypes.c_int32 * 3)(*self.window), self.rope_axes, self.rope_pairing,
+                      self.dtype, self.impl, self.scale)
+
+    @property
+    def tensor_shape(self):
+        return (self.batch,) + tuple(self.grid) + (self.heads, self.head_dim)
+
+    @property
+    def lse_shape(self):
+        return (self.batch, self.heads) + tuple(self.grid)
+
+    @property
+    def torch_dtype(self):
+        return torch.float32 if self.dtype == DTYPE_F32 else torch.bfloat16
+
+
+_LIB = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load the C-ABI library; fail loudly if it has not been built."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise StrataError(f"{LIB_PATH} is missing: run `python -m paper_2606_31248_b200.build` "
+                              "(there is no fallback path)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, sz, i32 = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
+        dp = ctypes.POINTER(_CDesc)
+        L.strata_na3d_workspace_bytes.restype = sz
+        L.strata_na3d_workspace_bytes.argtypes = [dp, i32]
+        L.strata_na3d_host_workspace_bytes.restype = sz
+        L.strata_na3d_host_workspace_bytes.argtypes = [dp, i32]
+        L.strata_na3d_impl_selected.restype = i32
+        L.strata_na3d_impl_selected.argtypes = [dp, i32]
+        for name in ("strata_na3d_fwd", "strata_na3d_fwd_host"):
+            f = getattr(L, name)
+            f.restype = i32
+            f.argtypes = [dp] + [vp] * 8 + [sz, vp]
+        for name in ("strata_na3d_bwd", "strata_na3d_bwd_host"):
+            f = getattr(L, name)
+            f.restype = i32
+            f.argtypes = [dp] + [vp] * 12 + [sz, vp]
+        L.strata_na3d_last_launch_count.restype = i32
+        L.strata_na3d_set_profiling.restype = None
+        L.strata_na3d_set_profiling.argtypes = [i32]
+        L.strata_na3d_profile_read.restype = i32
+        L.strata_na3d_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_char_p), i32]
+        L.strata_status_string.restype = ctypes.c_char_p
+        L.strata_status_string.argtypes = [i32]
+        L.strata_version.restype = i32
+        _LIB = L
+    return _LIB
+
+
+def _check(status: int, what: str):
+    if status != STRATA_OK:
+        raise StrataError(f"{what}: {lib().strata_status_string(status).decode()} (status {status})")
+
+
+def _ptr(t) -> Optional[int]:
+    """Raw address of a torch tensor (device or host) or None."""
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor):
+        raise TypeError("expected a torch.Tensor")
+    if not t.is_contiguous():
+        raise ValueError("tensors must be contiguous")
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream or None
+    return int(stream) or None
+
+
+# ------------------------------------------------------------------ 1:1 wrappers of the C entry points
+def strata_version() -> int:
+    return int(lib().strata_version())
+
+
+def strata_na3d_workspace_bytes(desc: NA3DDesc, backward: bool = False) -> int:
+    return int(lib().strata_na3d_workspace_bytes(ctypes.byref(desc.c()), int(backward)))
+
+
+def strata_na3d_host_workspace_bytes(desc: NA3DDesc, backward: bool = False) -> int:
+    return int(lib().strata_na3d_host_workspace_bytes(ctypes.byref(desc.c()), int(backward)))
+
+
+def strata_na3d_impl_selected(desc: NA3DDesc, backward: bool = False) -> int:
+    return int(lib().strata_na3d_impl_selected(ctypes.byref(desc.c()), int(backward)))
+
+
+def strata_na3d_last_launch_count() -> int:
+    return int(lib().strata_na3d_last_launch_count())
+
+
+def strata_na3d_set_profiling(enable: bool) -> None:
+    lib().strata_na3d_set_profiling(int(bool(enable)))
+
+
+def strata_na3d_profile_read(capacity: int = 4096):
+    """[(kernel name, milliseconds)] of every kernel since profiling was enabled; sync the stream first."""
+    ms = (ctypes.c_float * capacity)()
+    names = (ctypes.c_char_p * capacity)()
+    n = int(lib().strata_na3d_profile_read(ms, names, capacity))
+    if n < 0:
+        raise StrataError("strata_na3d_profile_read: event query failed")
+    return [(names[i].decode(), float(ms[i])) for i in range(min(n, capacity))]
+
+
+def strata_na3d_fwd_status(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None, host=False) -> int:
+    """Raw status code (tests of the error paths use this)."""
+    fn = lib().strata_na3d_fwd_host if host else lib().strata_na3d_fwd
+    ws_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    return int(fn(ctypes.byref(desc.c()), _ptr(q), _ptr(k), _ptr(v), _ptr(coords), _ptr(freqs), _ptr(o),
+                  _ptr(lse), _ptr(workspace), ws_bytes, _stream_handle(stream)))
+
+
+def strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None,
+                           host=False) -> int:
+    fn = lib().strata_na3d_bwd_host if host else lib().strata_na3d_bwd
+    ws_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    return int(fn(ctypes.byref(desc.c()), _ptr(q), _ptr(k), _ptr(v), _ptr(o), _ptr(d_o), _ptr(lse),
+                  _ptr(coords), _ptr(freqs), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(workspace), ws_bytes,
+                  _stream_handle(stream)))
+
+
+def strata_na3d_fwd(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None):
+    _check(strata_na3d_fwd_status(desc, q, k, v, coords, freqs, o, lse, workspace, stream), "strata_na3d_fwd")
+
+
+def strata_na3d_bwd(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None):
+    _check(strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream),
+           "strata_na3d_bwd")
+
+
+def strata_na3d_fwd_host(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None):
+    _check(strata_na3d_fwd_status(desc, q, k, v, coords, freqs, o, lse, workspace, stream, host=True),
+           "strata_na3d_fwd_host")
+
+
+def strata_na3d_bwd_host(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None):
+    _check(strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream,
+                                  host=True), "strata_na3d_bwd_host")
+
+
+# ------------------------------------------------------------------ convenience: allocate + call
+def desc_for(q: torch.Tensor, window: Sequence[int], rope_axes: int, rope_pairing: int = ROPE_INTERLEAVED,
+             scale: float = 0.0, impl: int = IMPL_AUTO) -> NA3DDesc:
+    if q.dim() != 6:
+        raise ValueError("q must be [B, L, Y, X, H, d]")
+    if q.dtype not in (torch.float32, torch.bfloat16):
+        raise TypeError("dtype must be float32 or bfloat16")
+    B, L, Y, X, H, D = q.shape
+    return NA3DDesc(B, H, D, (L, Y, X), tuple(int(w) for w in window), rope_axes, rope_pairing,
+                    DTYPE_F32 if q.dtype == torch.float32 else DTYPE_BF16, impl, float(scale))
+
+
+def alloc_workspace(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 16), dtype=torch.uint8, device=device)
+
+
+def na3d_forward(q, k, v, coords, freqs, window, rope_pairing=ROPE_INTERLEAVED, scale=0.0, impl=IMPL_AUTO,
+                 workspace=None, stream=None):
+    """StereoRoPE + NA3D forward on device tensors.  Returns (o, lse)."""
+    if not q.is_cuda:
+        raise StrataError("na3d_forward needs CUDA tensors (there is no CPU path)")
+    rope_axes = 0 if coords is None else coords.shape[-1]
+    desc = desc_for(q, window, rope_axes, rope_pairing, scale, impl)
+    o = torch.empty_like(q)
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32, device=q.device)
+    if workspace is None:
+        workspace = alloc_workspace(strata_na3d_workspace_bytes(desc, False), q.device)
+    strata_na3d_fwd(desc, q, k, v, coords, freqs, o, lse, workspace, stream)
+    return o, lse
+
+
+def na3d_backward(q, k, v, o, d_o, lse, coords, freqs, window, rope_pairing=ROPE_INTERLEAVED, scale=0.0,
+                  impl=IMPL_AUTO, workspace=None, stream=None):
+    """StereoRoPE + NA3D backward on device tensors.  Returns (dq, dk, dv)."""
+    if not q.is_cuda:
+        raise StrataError("na3d_backward needs CUDA tensors (there is no CPU path)")
+    rope_axes = 0 if coords is None else coords.shape[-1]
+    desc = desc_for(q, window, rope_axes, rope_pairing, scale, impl)
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(q), torch.empty_like(q)
+    if workspace is None:
+        workspace = alloc_workspace(strata_na3d_workspace_bytes(desc, True), q.device)
+    strata_na3d_bwd(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream)
+    return dq, dk, dv

@@ -1,0 +1,66 @@
+// common.cuh -- shared declarations of the CUDA path (never included by oracle/).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace strata {
+
+// Problem description in the paper's notation: B samples, H heads, head_dim D,
+// token grid (L, Y, X), window (kL, kY, kX), A rotary axes.
+struct Problem {
+  int B, H, D;
+  int L, Y, X;
+  int kL, kY, kX;
+  int A;        // rotary axes (0 = no RoPE)
+  int pairing;  // 0: (2j, 2j+1)   1: (j, j + D/2)
+  int dtype;    // 0 f32, 1 bf16
+  float scale;  // resolved softmax scale (> 0)
+  long long N;  // L * Y * X
+  __host__ __device__ long long rows() const { return (long long)B * N * H; }    // (b, token, h) rows
+  __host__ __device__ long long elems() const { return rows() * D; }
+};
+
+// A3 (inward clamp): first key of query i's window on an axis.
+__host__ __device__ inline int window_start(int i, int k, int n) {
+  int s = i - k / 2;
+  s = s < 0 ? 0 : s;
+  return s > n - k ? n - k : s;
+}
+
+// B3: queries whose window holds key j on one axis form the interval [lo, hi] (any k >= 1).
+__host__ __device__ inline void inverse_window(int j, int k, int n, int& lo, int& hi) {
+  lo = (j - k + 1 <= 0) ? 0 : j - k + 1 + k / 2;
+  hi = (j >= n - k) ? n - 1 : j + k / 2;
+}
+
+__device__ __forceinline__ float to_f32(float x) { return x; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 x) { return __bfloat162float(x); }
+template <typename T> __device__ __forceinline__ T from_f32(float x);
+template <> __device__ __forceinline__ float from_f32<float>(float x) { return x; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float x) { return __float2bfloat16_rn(x); }
+
+// Optional per-kernel timing (strata_na3d_set_profiling): launchers call prof_begin/prof_end around
+// each kernel; both are no-ops unless profiling is on for this host thread.
+void prof_begin(const char* name, cudaStream_t stream);
+void prof_end(cudaStream_t stream);
+
+// ---- launchers (each enqueues on `stream`, returns the launch error, adds to *launches) ----
+// rope.cu: y = R(sign*phi) x for up to two tensors at once; in/out dtype tags 0 f32, 1 bf16.
+cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1, int in_dtype,
+                               void* y0, void* y1, int out_dtype, const float* coords,
+                               const float* freqs, float sign, cudaStream_t stream, int* launches);
+
+// na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
+cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
+                            void* o, float* lse, cudaStream_t stream, int* launches);
+cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
+                            const void* o, const void* d_o, const float* lse, float* delta,
+                            float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches);
+
+// na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands.
+bool tc_fwd_supported(const Problem& p);
+cudaError_t launch_fwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
+                          float* lse, cudaStream_t stream, int* launches);
+
+}  // namespace strata

@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path through the C ABI against the CPU float64 oracle, element by element."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_31248_b200 import binding, workloads as wl
+from helpers import assert_parity, desc_of, device_inputs, to_f64
+
+pytestmark = pytest.mark.gpu
+
+IMPLS = [binding.IMPL_SIMT, binding.IMPL_AUTO]
+
+
+def run_fwd(w, inp, impl=binding.IMPL_AUTO, scale=0.0):
+    d = device_inputs(w, inp)
+    desc = desc_of(w, impl, scale)
+    o = torch.empty_like(d["q"])
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
+    ws = binding.alloc_workspace(binding.strata_na3d_workspace_bytes(desc, False), "cuda")
+    binding.strata_na3d_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], o, lse, ws)
+    torch.cuda.synchronize()
+    return d, o, lse
+
+
+def run_bwd(w, inp, d, o, lse, impl=binding.IMPL_AUTO, scale=0.0):
+    desc = desc_of(w, impl, scale)
+    dq, dk, dv = (torch.empty_like(d["q"]) for _ in range(3))
+    ws = binding.alloc_workspace(binding.strata_na3d_workspace_bytes(desc, True), "cuda")
+    binding.strata_na3d_bwd(desc, d["q"], d["k"], d["v"], o, d["do"], lse, d["coords"], d["freqs"], dq, dk, dv, ws)
+    torch.cuda.synchronize()
+    return dq, dk, dv
+
+
+def check_full(oracle_mod, w, impl, backward=True, scale=0.0):
+    inp = wl.make_inputs(w, with_do=True)
+    d, o, lse = run_fwd(w, inp, impl, scale)
+    coords = inp["coords"] if w.rope_axes else np.zeros((w.batch,) + w.grid + (0,), np.float32)
+    o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], coords, inp["freqs"], w.window,
+                                         scale=scale or None, pairing=w.rope_pairing)
+    assert_parity(to_f64(o), o_ref, w.dtype, f"{w.name} O")
+    assert_parity(to_f64(lse), lse_ref, "f32" if w.dtype == "f32" else "bf16", f"{w.name} LSE", rms_bound=1e-2)
+    if backward:
+        dq, dk, dv = run_bwd(w, inp, d, o, lse, impl, scale)
+        rq, rk, rv = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], coords, inp["freqs"], w.window,
+                                         scale=scale or None, pairing=w.rope_pairing)
+        # the GPU backward starts from the GPU's rounded O (bf16): allow 2e-2 relative RMS there
+        rb = None if w.dtype == "f32" else 2e-2
+        assert_parity(to_f64(dq), rq, w.dtype, f"{w.name} dQ", rms_bound=rb)
+        assert_parity(to_f64(dk), rk, w.dtype, f"{w.name} dK", rms_bound=rb)
+        assert_parity(to_f64(dv), rv, w.dtype, f"{w.name} dV", rms_bound=rb)
+
+
+# ------------------------------------------------------------------ BASELINE.json configs
+@pytest.mark.parametrize("impl", IMPLS)
+def test_config0_tiny_fp32_fwd_bwd(oracle_mod, impl):
+    check_full(oracle_mod, wl.config(0), impl)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_config1_bf16_fwd_full(oracle_mod, impl):
+    check_full(oracle_mod, wl.config(1), impl, backward=False)
+
+
+def test_config4_bf16_bwd_full(oracle_mod):
+    w = wl.config(4)
+    inp = wl.make_inputs(w, with_do=True)
+    d, o, lse = run_fwd(w, inp)
+    dq, dk, dv = run_bwd(w, inp, d, o, lse)
+    rq, rk, rv = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
+    for got, ref, nm in ((dq, rq, "dQ"), (dk, rk, "dK"), (dv, rv, "dV")):
+        assert_parity(to_f64(got), ref, "bf16", f"cfg4 {nm}", rms_bound=2e-2)
+
+
+def _sampled_fwd(oracle_mod, w, n_rows, impl=binding.IMPL_AUTO):
+    inp = wl.make_inputs(w)
+    d, o, lse = run_fwd(w, inp, impl)
+    total = w.batch * w.tokens * w.heads
+    rng = np.random.default_rng(w.seed + 1000)
+    idx = rng.choice(total, size=n_rows, replace=False)
+    # make sure borders (clamped windows) and the last tile / last batch element are in the sample
+    N, H = w.tokens, w.heads
+    corners = [0, H - 1, (N - 1) * H, total - 1, ((w.batch - 1) * N + w.grid[2] - 1) * H]
+    idx = np.unique(np.concatenate([idx, np.array(corners, dtype=np.int64)]))
+    o_ref, lse_ref = oracle_mod.na3d_fwd_queries(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window, idx)
+    o_got = to_f64(o.reshape(total, w.head_dim)[torch.from_numpy(idx).cuda()])
+    lse_flat = lse.reshape(w.batch, H, N).permute(0, 2, 1).reshape(total)
+    lse_got = to_f64(lse_flat[torch.from_numpy(idx).cuda()])
+    assert_parity(o_got, o_ref, w.dtype, f"{w.name} O (sampled rows)")
+    assert_parity(lse_got, lse_ref, "bf16", f"{w.name} LSE (sampled rows)")
+    # properties that hold at any size: finite everywhere, LSE within the softmax bounds
+    assert bool(torch.isfinite(o.float()).all()) and bool(torch.isfinite(lse).all())
+    return inp, d, o, lse
+
+
+def test_config2_bf16_wide_head_sampled(oracle_mod):
+    _sampled_fwd(oracle_mod, wl.config(2), 3000)
+
+
+def test_config3_bf16_global_rollout_sampled(oracle_mod):
+    _sampled_fwd(oracle_mod, wl.config(3), 4000)
+
+
+# ------------------------------------------------------------------ shape / option sweep
+SWEEP = [
+    dict(grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32),
+    dict(grid=(5, 9, 11), window=(3, 5, 7), heads=3, head_dim=64, batch=2),
+    dict(grid=(2, 10, 9), window=(2, 4, 6), heads=1, head_dim=32),                 # even windows
+    dict(grid=(4, 5, 6), window=(4, 5, 6), heads=2, head_dim=32),                  # window = grid: dense
+    dict(grid=(3, 5, 5), window=(1, 1, 1), heads=2, head_dim=32),                  # k = 1
+    dict(grid=(1, 12, 13), window=(1, 5, 5), heads=2, head_dim=64),                # 2D
+    dict(grid=(1, 1, 40), window=(1, 1, 9), heads=2, head_dim=32),                 # 1D
+    dict(grid=(9, 17, 19), window=(5, 9, 9), heads=2, head_dim=128),               # wide head, ragged tiles
+    dict(grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32, rope_pairing=1),  # HALF pairing
+    dict(grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=64, rope_pairing=1),
+    dict(grid=(4, 6, 7), window=(3, 3, 3), heads=2, head_dim=32, rope_axes=3),     # level axis rotated too
+    dict(grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32, rope_axes=0),     # no RoPE
+    dict(grid=(8, 18, 21), window=(3, 7, 7), heads=2, head_dim=64, batch=2),       # several tiles + ragged tail
+]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("case", range(len(SWEEP)))
+def test_shape_sweep_fwd_bwd(oracle_mod, case, dtype):
+    w = wl.small(name=f"sweep{case}_{dtype}", dtype=dtype, **SWEEP[case])
+    check_full(oracle_mod, w, binding.IMPL_AUTO)
+
+
+def test_qknorm_logits_bf16(oracle_mod):
+    """What QK-RMSNorm hands the kernel: |q| = |k| = sqrt(d), logits up to +-sqrt(d)."""
+    w = wl.small(name="qknorm", dtype="bf16", value_scale="qknorm", grid=(8, 16, 16), window=(3, 7, 7),
+                 heads=2, head_dim=64)
+    check_full(oracle_mod, w, binding.IMPL_AUTO)
+
+
+def test_explicit_scale(oracle_mod):
+    w = wl.small(name="scale", dtype="f32", grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32)
+    check_full(oracle_mod, w, binding.IMPL_AUTO, scale=0.31)
+
+
+# ------------------------------------------------------------------ API behaviour on the device
+def test_host_entry_points(oracle_mod):
+    w = wl.small(name="host", dtype="bf16", grid=(4, 9, 10), window=(3, 5, 5), heads=2, head_dim=64, batch=2)
+    inp = wl.make_inputs(w, with_do=True)
+    h = device_inputs(w, inp, device="cpu")
+    h = {n: (t.pin_memory() if t is not None else None) for n, t in h.items()}
+    desc = desc_of(w)
+    o = torch.empty_like(h["q"]).pin_memory()
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32).pin_memory()
+    ws = binding.alloc_workspace(binding.strata_na3d_host_workspace_bytes(desc, False), "cuda")
+    binding.strata_na3d_fwd_host(desc, h["q"], h["k"], h["v"], h["coords"], h["freqs"], o, lse, ws)
+    torch.cuda.synchronize()
+    o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window)
+    assert_parity(to_f64(o), o_ref, "bf16", "host O")
+    assert_parity(to_f64(lse), lse_ref, "bf16", "host LSE")
+    dq, dk, dv = (torch.empty_like(h["q"]).pin_memory() for _ in range(3))
+    ws = binding.alloc_workspace(binding.strata_na3d_host_workspace_bytes(desc, True), "cuda")
+    binding.strata_na3d_bwd_host(desc, h["q"], h["k"], h["v"], o, h["do"], lse, h["coords"], h["freqs"], dq, dk, dv, ws)
+    torch.cuda.synchronize()
+    ref = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
+    for got, r, nm in zip((dq, dk, dv), ref, ("dQ", "dK", "dV")):
+        assert_parity(to_f64(got), r, "bf16", f"host {nm}", rms_bound=2e-2)
+
+
+def test_device_error_paths_and_stream():
+    w = wl.small(name="err", dtype="f32", grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32)
+    inp = wl.make_inputs(w)
+    d = device_inputs(w, inp)
+    desc = desc_of(w)
+    o = torch.empty_like(d["q"])
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
+    need = binding.strata_na3d_workspace_bytes(desc, False)
+    small = binding.alloc_workspace(need - 256, "cuda")
+    assert binding.strata_na3d_fwd_status(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], o, lse, small) == 3
+    ws = binding.alloc_workspace(need, "cuda")
+    mis = torch.empty(d["q"].numel() + 1, device="cuda")[1:].view_as(d["q"])      # 4-byte offset
+    assert binding.strata_na3d_fwd_status(desc, mis, d["k"], d["v"], d["coords"], d["freqs"], o, lse, ws) == 1
+    # asynchronous on a side stream; result identical to the default-stream call
+    binding.strata_na3d_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], o, lse, ws)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    o2, lse2 = torch.empty_like(o), torch.empty_like(lse)
+    with torch.cuda.stream(s):
+        binding.strata_na3d_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], o2, lse2, ws, stream=s)
+    s.synchronize()
+    assert torch.equal(o, o2) and torch.equal(lse, lse2)
+    assert binding.strata_na3d_last_launch_count() >= 2
