@@ -1,8 +1,520 @@
-// placeholder until the tcgen05 forward lands
+// na3d_tc_fwd.cu -- tcgen05 / TMEM / TMA forward kernel for 3D neighbourhood attention (sm_100a).
+//
+// Steps A3-A6 of DESIGN.md on pre-rotated bf16 operands (A1, A2 are done by rope.cu):
+//   one CTA owns a 3D query tile of TL x TY x TX = 2 x 8 x 8 = 128 queries of one (sample, head);
+//   the union of its neighbours' keys -- the halo box of (TL+kL-1) x (TY+kY-1) x (TX+kX-1) keys,
+//   trimmed to what the inward-clamped windows (R1) really reach -- is
+//   streamed through shared memory by TMA in chunks of CY = 8 key rows of one level plane;
+//   S = Qrot Krot^T and O += P V run on the 5th-gen tensor cores (tcgen05.mma, M = 128,
+//   accumulators in TMEM); the softmax is online, one query row per thread, with the window mask
+//   applied as an additive -inf bias and whole key rows / planes skipped per warp.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner,
+// warps 2-5 = softmax + epilogue (TMEM subpartition = warp index mod 4).
+// Pipelines (mbarriers): K/V stage full/empty (TMA <-> MMA), s_full (MMA1 -> softmax),
+// p_full (softmax -> MMA2), pv_done (MMA2 -> O rescale / epilogue).
+//
+// TMEM columns: O [0, D) fp32 | S [D, D+128) fp32 | P [D+128, D+192) bf16x2 (A operand of MMA2).
+#include <cuda.h>
+
 #include "common.cuh"
+
 namespace strata {
-bool tc_fwd_supported(const Problem&) { return false; }
-cudaError_t launch_fwd_tc(const Problem&, const void*, const void*, const void*, void*, float*, cudaStream_t, int*) {
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// Bounded wait: a protocol bug becomes a launch failure (trap), not a hung GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins > (1u << 26)) __trap();
+  }
+}
+__device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0,
+                                            int c1, int c2, int c3, int c4) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]
+__device__ __forceinline__ void umma_ss(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]
+__device__ __forceinline__ void umma_ts(uint32_t d, uint32_t a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d), "r"(a), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr) : "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+        "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);   // .x (low 16 bits) = lo
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// Shared-memory matrix descriptors (tcgen05, 128-byte swizzle, 8-row groups 1024 bytes apart).
+//   K-major  (rows = M or N index, 64 contiguous bf16 of the contraction per row): Q tile, K chunk.
+//   MN-major (rows = contraction index, 64 contiguous bf16 of N per row):          V chunk.
+// bits [0,14) start >> 4 | [16,30) leading byte offset >> 4 | [32,46) stride byte offset >> 4 |
+// [46,48) version = 1 | [61,64) layout = 2 (SWIZZLE_128B)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
+  return (uint64_t)((addr >> 4) & 0x3FFF) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+
+// Instruction descriptor, kind::f16: D fp32 (bit 4), A = B = bf16 (bits 7, 10), N>>3 at 17, M>>4 at 24.
+__host__ __device__ constexpr uint32_t instr_desc(int m, int n, bool b_mn_major) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)(m >> 4) << 24);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Configuration
+// ------------------------------------------------------------------------------------------------
+template <int D_, int KL_, int KY_, int KX_>
+struct Cfg {
+  static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
+  static constexpr int TL = 2, TY = 8, TX = 8, M = 128;            // query tile
+  static constexpr int HL = TL + KL - 1, HY = TY + KY - 1, HX = TX + KX - 1;   // halo box
+  static constexpr int CY = 8;                                     // key rows per chunk
+  static constexpr int NKEY = CY * HX;                             // keys per chunk (UMMA N of S)
+  static constexpr int DSUB = D / 64;                              // 128-byte sub-tiles per row
+  static constexpr int SUB_Q = M * 128, SUB_KV = NKEY * 128;       // bytes of one sub-tile
+  static constexpr int Q_BYTES = DSUB * SUB_Q, STAGE_BYTES = DSUB * SUB_KV;
+  static constexpr int NSTAGE = (2 * 3 * STAGE_BYTES + Q_BYTES <= 110 * 1024) ? 3 : 2;
+  static constexpr int TMEM_O = 0, TMEM_S = D, TMEM_P = D + 128;
+  static constexpr int TMEM_COLS = (D + 192 <= 256) ? 256 : 512;
+  static constexpr int BAR_BYTES = 256;
+  static constexpr int SMEM_BYTES = 1024 + Q_BYTES + 2 * NSTAGE * STAGE_BYTES + BAR_BYTES;
+  static constexpr int CTAS_PER_SM = (2 * SMEM_BYTES <= 227 * 1024 && TMEM_COLS == 256) ? 2 : 1;
+  static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1, "odd windows only (HX even, no pad keys)");
+  static_assert(NKEY % 16 == 0 && NKEY <= 128 && HX <= 16, "chunk must fit one UMMA N <= 128");
+  static_assert(D == 64 || D == 128, "head_dim 64 or 128");
+};
+
+struct TcParams {
+  int B, H, L, Y, X;
+  int ntl, nty, ntx;
+  long long N;
+  float scale_log2e;
+};
+
+constexpr int kThreads = 192;
+constexpr float kRescaleThreshold = 8.f;   // log2 units: P stays below 2^8 between rescales
+
+// ------------------------------------------------------------------------------------------------
+// Kernel
+// ------------------------------------------------------------------------------------------------
+template <class C>
+__global__ void __launch_bounds__(kThreads, C::CTAS_PER_SM)
+na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                   const __grid_constant__ CUtensorMap tm_v, __nv_bfloat16* __restrict__ o,
+                   float* __restrict__ lse, const TcParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t q_smem = base;
+  const uint32_t k_smem = q_smem + C::Q_BYTES;
+  const uint32_t v_smem = k_smem + C::NSTAGE * C::STAGE_BYTES;
+  const uint32_t bars = v_smem + C::NSTAGE * C::STAGE_BYTES;
+  // barrier slots (8 bytes each)
+  const uint32_t bar_q = bars;
+  auto bar_kfull = [&](int s) { return bars + 8u * (1 + s); };
+  auto bar_kempty = [&](int s) { return bars + 8u * (1 + C::NSTAGE + s); };
+  auto bar_vfull = [&](int s) { return bars + 8u * (1 + 2 * C::NSTAGE + s); };
+  auto bar_vempty = [&](int s) { return bars + 8u * (1 + 3 * C::NSTAGE + s); };
+  const uint32_t bar_sfull = bars + 8u * (1 + 4 * C::NSTAGE);
+  const uint32_t bar_pfull = bar_sfull + 8;
+  const uint32_t bar_pvdone = bar_sfull + 16;
+  const uint32_t tmem_slot = bar_sfull + 24;
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- tile of this CTA: x fastest, then y, level, head, sample (spatial neighbours co-resident)
+  int bid = blockIdx.x;
+  const int tx = bid % p.ntx; bid /= p.ntx;
+  const int ty = bid % p.nty; bid /= p.nty;
+  const int tl = bid % p.ntl; bid /= p.ntl;
+  const int h = bid % p.H;
+  const int b = bid / p.H;
+  const int x0 = tx * C::TX, y0 = ty * C::TY, l0 = tl * C::TL;
+  // halo box actually reached by the in-grid queries of the tile (A3, inward clamp)
+  const int xl = min(x0 + C::TX, p.X) - 1, yl = min(y0 + C::TY, p.Y) - 1, ll = min(l0 + C::TL, p.L) - 1;
+  const int hs_x = window_start(x0, C::KX, p.X), hs_y = window_start(y0, C::KY, p.Y), hs_l = window_start(l0, C::KL, p.L);
+  const int hy = window_start(yl, C::KY, p.Y) + C::KY - hs_y;      // <= HY
+  const int hl = window_start(ll, C::KL, p.L) + C::KL - hs_l;      // <= HL
+  (void)xl;
+  const int ncy = (hy + C::CY - 1) / C::CY;
+  const int nchunks = hl * ncy;
+
+  // ---- one-time setup
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_v);
+    mbar_init(bar_q, 1);
+    for (int s = 0; s < C::NSTAGE; ++s) {
+      mbar_init(bar_kfull(s), 1); mbar_init(bar_kempty(s), 1);
+      mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 1);
+    }
+    mbar_init(bar_sfull, 1);
+    mbar_init(bar_pfull, 128);
+    mbar_init(bar_pvdone, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // =========================== TMA producer ===========================
+    if (lane == 0) {
+      const int bl = b * p.L;
+      mbar_expect_tx(bar_q, C::Q_BYTES);
+      for (int j = 0; j < C::DSUB; ++j) tma_load_5d(q_smem + j * C::SUB_Q, &tm_q, bar_q, 64 * j, h, x0, y0, bl + l0);
+      int c = 0;
+      for (int pl = 0; pl < hl; ++pl)
+        for (int cy = 0; cy < ncy; ++cy, ++c) {
+          const int s = c % C::NSTAGE;
+          const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
+          mbar_wait(bar_kempty(s), ph ^ 1u);
+          mbar_expect_tx(bar_kfull(s), C::STAGE_BYTES);
+          for (int j = 0; j < C::DSUB; ++j)
+            tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_k, bar_kfull(s), 64 * j, h, hs_x,
+                        hs_y + cy * C::CY, bl + hs_l + pl);
+          mbar_wait(bar_vempty(s), ph ^ 1u);
+          mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
+          for (int j = 0; j < C::DSUB; ++j)
+            tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_v, bar_vfull(s), 64 * j, h, hs_x,
+                        hs_y + cy * C::CY, bl + hs_l + pl);
+        }
+    }
+  } else if (warp == 1) {
+    // =========================== MMA issuer ===========================
+    if (lane == 0) {
+      constexpr uint32_t idesc_qk = instr_desc(C::M, C::NKEY, false);
+      constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
+      mbar_wait(bar_q, 0);
+      tc_fence_after();
+      for (int c = 0; c < nchunks; ++c) {
+        const int s = c % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
+        // ---- S = Qrot Krot^T  (M = 128, N = NKEY, K = D in steps of 16)
+        mbar_wait(bar_kfull(s), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < C::D / 16; ++ks) {
+          const uint32_t off = (ks >> 2) * 1u, kin = (ks & 3) * 32u;      // sub-tile, byte offset in the row
+          const uint64_t ad = smem_desc(q_smem + off * C::SUB_Q + kin);
+          const uint64_t bd = smem_desc(k_smem + s * C::STAGE_BYTES + off * C::SUB_KV + kin);
+          umma_ss(tmem + C::TMEM_S, ad, bd, idesc_qk, ks > 0 ? 1u : 0u);
+        }
+        umma_commit(bar_kempty(s));
+        umma_commit(bar_sfull);
+        // ---- O += P V  (M = 128, N = 64 per sub-tile, K = NKEY in steps of 16 keys)
+        mbar_wait(bar_pfull, (uint32_t)c & 1u);
+        mbar_wait(bar_vfull(s), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < C::NKEY / 16; ++ks) {
+#pragma unroll
+          for (int j = 0; j < C::DSUB; ++j) {
+            const uint64_t bd = smem_desc(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
+            umma_ts(tmem + C::TMEM_O + 64 * j, tmem + C::TMEM_P + 8 * ks, bd, idesc_pv, (c > 0 || ks > 0) ? 1u : 0u);
+          }
+        }
+        umma_commit(bar_vempty(s));
+        umma_commit(bar_pvdone);
+      }
+    }
+  } else {
+    // =========================== softmax + epilogue ===========================
+    const int sp = warp & 3;                       // TMEM subpartition of this warp
+    const int row = sp * 32 + lane;                // query row of the tile == TMEM lane
+    const uint32_t lane_addr = (uint32_t)(sp * 32) << 16;
+    const int qx = row & 7, qy = (row >> 3) & 7, ql = row >> 6;
+    const bool active = (x0 + qx < p.X) && (y0 + qy < p.Y) && (l0 + ql < p.L);
+    const int ax = min(x0 + qx, p.X - 1), ay = min(y0 + qy, p.Y - 1), al = min(l0 + ql, p.L - 1);
+    // window of this query relative to the halo box
+    const int lo_x = window_start(ax, C::KX, p.X) - hs_x;
+    const int lo_y = window_start(ay, C::KY, p.Y) - hs_y;
+    const int lo_l = window_start(al, C::KL, p.L) - hs_l;
+    float xbias[C::HX];
+#pragma unroll
+    for (int j = 0; j < C::HX; ++j) xbias[j] = (j >= lo_x && j < lo_x + C::KX) ? 0.f : -INFINITY;
+    // key rows / planes any query of this warp needs (warp-uniform skip ranges)
+    const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
+    const int wl_lo = __reduce_min_sync(0xffffffffu, lo_l), wl_hi = __reduce_max_sync(0xffffffffu, lo_l + C::KL);
+
+    float m_ref = -INFINITY, lsum = 0.f;
+    const float cs = p.scale_log2e;
+    int c = 0;
+    for (int pl = 0; pl < hl; ++pl) {
+      const bool plane_needed = pl >= wl_lo && pl < wl_hi;
+      const bool plane_ok = pl >= lo_l && pl < lo_l + C::KL;
+      for (int cy = 0; cy < ncy; ++cy, ++c) {
+        mbar_wait(bar_sfull, (uint32_t)c & 1u);
+        tc_fence_after();
+        uint32_t pw[C::NKEY / 2];
+        float csum = 0.f;
+        for (int attempt = 0; attempt < 2; ++attempt) {
+          float cmax = -INFINITY;
+          csum = 0.f;
+#pragma unroll
+          for (int r = 0; r < C::CY; ++r) {
+            const int py = cy * C::CY + r;
+            if (plane_needed && py >= wy_lo && py < wy_hi) {
+              float sv[16];
+              tmem_ld16(tmem + lane_addr + C::TMEM_S + r * C::HX, sv);
+              tmem_wait_ld();
+              const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
+              float t[C::HX];
+              float rmax = -INFINITY;
+#pragma unroll
+              for (int j = 0; j < C::HX; ++j) { t[j] = fmaf(sv[j], cs, xbias[j]); rmax = fmaxf(rmax, t[j]); }
+              if (rowok) {
+                if (m_ref == -INFINITY) m_ref = rmax;     // first key row of this query: no rescale needed
+                cmax = fmaxf(cmax, rmax);
+              }
+              const float nb = rowok ? -m_ref : -INFINITY;
+              float rsum = 0.f;
+#pragma unroll
+              for (int j = 0; j < C::HX; j += 2) {
+                const float p0 = ex2(t[j] + nb), p1 = ex2(t[j + 1] + nb);
+                rsum += p0 + p1;
+                pw[(r * C::HX + j) >> 1] = pack_bf16(p0, p1);
+              }
+              csum += rsum;
+            } else {
+#pragma unroll
+              for (int j = 0; j < C::HX; j += 2) pw[(r * C::HX + j) >> 1] = 0u;
+            }
+          }
+          // optimistic pass used the old reference maximum; redo the chunk if it was too small
+          const bool need = cmax > m_ref + kRescaleThreshold;
+          if (attempt == 0 && __any_sync(0xffffffffu, need)) {
+            const float alpha = need ? ex2(m_ref - cmax) : 1.f;
+            if (c > 0) {                                    // O holds chunks 0..c-1: rescale its rows
+              mbar_wait(bar_pvdone, (uint32_t)(c - 1) & 1u);
+              tc_fence_after();
+#pragma unroll
+              for (int j = 0; j < C::D; j += 16) {
+                float ov[16];
+                tmem_ld16(tmem + lane_addr + C::TMEM_O + j, ov);
+                tmem_wait_ld();
+                uint32_t ow[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
+                tmem_st16(tmem + lane_addr + C::TMEM_O + j, ow);
+              }
+              tmem_wait_st();
+            }
+            lsum *= alpha;
+            if (need) m_ref = cmax;
+            continue;
+          }
+          break;
+        }
+        lsum += csum;
+        // P (bf16 pairs) -> TMEM, then hand the chunk to MMA2
+#pragma unroll
+        for (int j = 0; j < C::NKEY / 2; j += 8) tmem_st8(tmem + lane_addr + C::TMEM_P + j, &pw[j]);
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bar_pfull);
+      }
+    }
+    // ---- epilogue: O / l -> bf16 -> global, LSE
+    mbar_wait(bar_pvdone, (uint32_t)(nchunks - 1) & 1u);
+    tc_fence_after();
+    const float inv = 1.f / lsum;
+    const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
+    __nv_bfloat16* orow = o + (((long long)b * p.N + tok) * p.H + h) * C::D;
+#pragma unroll
+    for (int j = 0; j < C::D; j += 16) {
+      float ov[16];
+      tmem_ld16(tmem + lane_addr + C::TMEM_O + j, ov);
+      tmem_wait_ld();
+      if (active) {
+        uint4 w0, w1;
+        w0.x = pack_bf16(ov[0] * inv, ov[1] * inv);   w0.y = pack_bf16(ov[2] * inv, ov[3] * inv);
+        w0.z = pack_bf16(ov[4] * inv, ov[5] * inv);   w0.w = pack_bf16(ov[6] * inv, ov[7] * inv);
+        w1.x = pack_bf16(ov[8] * inv, ov[9] * inv);   w1.y = pack_bf16(ov[10] * inv, ov[11] * inv);
+        w1.z = pack_bf16(ov[12] * inv, ov[13] * inv); w1.w = pack_bf16(ov[14] * inv, ov[15] * inv);
+        reinterpret_cast<uint4*>(orow + j)[0] = w0;
+        reinterpret_cast<uint4*>(orow + j)[1] = w1;
+      }
+    }
+    if (active) lse[((long long)b * p.H + h) * p.N + tok] = (m_ref + log2f(lsum)) * 0.69314718055994531f;
+  }
+
+  // ---- teardown
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem, C::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host side: tensor maps + launch
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(sym);
+    (void)cudaGetLastError();
+  }
+  return fn;
+}
+
+// Tensor [B*L, Y, X, H, D] bf16 as a rank-5 map (fastest first: d, h, x, y, b*l); box = 64 channels of
+// one head x (bx, by, bl) tokens, 128-byte swizzle, out-of-bounds reads return zero.
+bool make_map(CUtensorMap* map, const void* ptr, const Problem& p, int bx, int by, int bl) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  const cuuint64_t dims[5] = {(cuuint64_t)p.D, (cuuint64_t)p.H, (cuuint64_t)p.X, (cuuint64_t)p.Y,
+                              (cuuint64_t)p.B * (cuuint64_t)p.L};
+  const cuuint64_t e = 2;
+  const cuuint64_t strides[4] = {(cuuint64_t)p.D * e, (cuuint64_t)p.H * p.D * e, (cuuint64_t)p.X * p.H * p.D * e,
+                                 (cuuint64_t)p.Y * p.X * p.H * p.D * e};
+  const cuuint32_t box[5] = {64, 1, (cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bl};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <class C>
+cudaError_t launch_cfg(const Problem& p, const void* qr, const void* kr, const void* v, void* o, float* lse,
+                       cudaStream_t stream, int* launches) {
+  CUtensorMap tq, tk, tv;
+  if (!make_map(&tq, qr, p, C::TX, C::TY, C::TL) || !make_map(&tk, kr, p, C::HX, C::CY, 1) ||
+      !make_map(&tv, v, p, C::HX, C::CY, 1))
+    return cudaErrorInvalidValue;
+  TcParams tp;
+  tp.B = p.B; tp.H = p.H; tp.L = p.L; tp.Y = p.Y; tp.X = p.X; tp.N = p.N;
+  tp.ntl = (p.L + C::TL - 1) / C::TL; tp.nty = (p.Y + C::TY - 1) / C::TY; tp.ntx = (p.X + C::TX - 1) / C::TX;
+  tp.scale_log2e = p.scale * 1.4426950408889634f;
+  const long long grid = (long long)p.B * p.H * tp.ntl * tp.nty * tp.ntx;
+  if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(na3d_fwd_tc_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  prof_begin("na3d_fwd_tcgen05", stream);
+  na3d_fwd_tc_kernel<C><<<(unsigned)grid, kThreads, C::SMEM_BYTES, stream>>>(tq, tk, tv, (__nv_bfloat16*)o, lse, tp);
+  prof_end(stream);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+// Shapes the tensor-core path covers: bf16, head_dim 64 / 128, the window sizes instantiated below.
+#define STRATA_TC_CONFIGS(X) \
+  X(64, 3, 7, 7)             \
+  X(128, 5, 9, 9)            \
+  X(64, 3, 5, 5)             \
+  X(64, 3, 3, 3)
+
+bool tc_fwd_supported(const Problem& p) {
+  if (p.dtype != 1) return false;
+#define X(D_, KL_, KY_, KX_) \
+  if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_) return true;
+  STRATA_TC_CONFIGS(X)
+#undef X
+  return false;
+}
+
+cudaError_t launch_fwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
+                          float* lse, cudaStream_t stream, int* launches) {
+#define X(D_, KL_, KY_, KX_)                                               \
+  if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)               \
+    return launch_cfg<Cfg<D_, KL_, KY_, KX_>>(p, qr, kr, v, o, lse, stream, launches);
+  STRATA_TC_CONFIGS(X)
+#undef X
   return cudaErrorNotSupported;
 }
+
 }  // namespace strata
