@@ -64,7 +64,12 @@ typedef enum { STRATA_ROPE_INTERLEAVED = 0, STRATA_ROPE_HALF = 1 } strata_rope_p
 
 /* Kernel family.  AUTO picks the tcgen05 tensor-core kernels when they cover the problem
  * (bf16, see strata_na3d_impl_selected) and the fp32 CUDA-core kernels otherwise. */
-typedef enum { STRATA_IMPL_AUTO = 0, STRATA_IMPL_SIMT = 1, STRATA_IMPL_TCGEN05 = 2 } strata_impl_t;
+typedef enum {
+  STRATA_IMPL_AUTO = 0,
+  STRATA_IMPL_SIMT = 1,
+  STRATA_IMPL_TCGEN05 = 2,      /* tensor-core kernels; level-sweep kernel where it applies */
+  STRATA_IMPL_TCGEN05_TILE = 3  /* tensor-core kernel with one query tile per CTA (any covered shape) */
+} strata_impl_t;
 
 typedef struct {
   int32_t batch, heads, head_dim; /* B, H, d; d in {32, 64, 128}                               */

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libstrata_na3d.so")
 STRATA_OK = 0
 DTYPE_F32, DTYPE_BF16 = 0, 1
 ROPE_INTERLEAVED, ROPE_HALF = 0, 1
-IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05 = 0, 1, 2
+IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_TILE = 0, 1, 2, 3
 
 EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
            "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",

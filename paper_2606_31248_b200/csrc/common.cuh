@@ -15,6 +15,7 @@ struct Problem {
   int A;        // rotary axes (0 = no RoPE)
   int pairing;  // 0: (2j, 2j+1)   1: (j, j + D/2)
   int dtype;    // 0 f32, 1 bf16
+  int force_tile;  // tcgen05: use the one-tile-per-CTA kernel even where the level-sweep kernel applies
   float scale;  // resolved softmax scale (> 0)
   long long N;  // L * Y * X
   __host__ __device__ long long rows() const { return (long long)B * N * H; }    // (b, token, h) rows
@@ -57,6 +58,11 @@ cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, 
 cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             const void* o, const void* d_o, const float* lse, float* delta,
                             float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches);
+
+// na3d_tc_fwd_sweep.cu: tcgen05 forward, one CTA per level column (head_dim 64, k_L = 3).
+bool tc_sweep_supported(const Problem& p);
+cudaError_t launch_fwd_sweep(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
+                             float* lse, cudaStream_t stream, int* launches);
 
 // na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands.
 bool tc_fwd_supported(const Problem& p);

@@ -31,7 +31,7 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
     if (d->grid[a] < 1 || d->window[a] < 1 || d->window[a] > d->grid[a]) return false;
   if (d->rope_axes < 0 || d->rope_pairing < 0 || d->rope_pairing > 1) return false;
   if (d->dtype != STRATA_DTYPE_F32 && d->dtype != STRATA_DTYPE_BF16) return false;
-  if (d->impl < STRATA_IMPL_AUTO || d->impl > STRATA_IMPL_TCGEN05) return false;
+  if (d->impl < STRATA_IMPL_AUTO || d->impl > STRATA_IMPL_TCGEN05_TILE) return false;
   *why = STRATA_ERR_UNSUPPORTED;
   if (d->head_dim != 32 && d->head_dim != 64 && d->head_dim != 128) return false;
   if (d->rope_axes > 3) return false;
@@ -39,6 +39,7 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
   p->L = d->grid[0]; p->Y = d->grid[1]; p->X = d->grid[2];
   p->kL = d->window[0]; p->kY = d->window[1]; p->kX = d->window[2];
   p->A = d->rope_axes; p->pairing = d->rope_pairing; p->dtype = d->dtype;
+  p->force_tile = d->impl == STRATA_IMPL_TCGEN05_TILE;
   p->scale = d->scale > 0.f ? d->scale : 1.0f / sqrtf((float)d->head_dim);
   p->N = (long long)p->L * p->Y * p->X;
   if ((double)p->rows() * p->D > 9.0e18) return false;
@@ -51,7 +52,7 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
 int select_impl(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
   const bool tc_ok = !backward && strata::tc_fwd_supported(p);
   if (d->impl == STRATA_IMPL_SIMT) return STRATA_IMPL_SIMT;
-  if (d->impl == STRATA_IMPL_TCGEN05) return tc_ok ? STRATA_IMPL_TCGEN05 : -1;
+  if (d->impl == STRATA_IMPL_TCGEN05 || d->impl == STRATA_IMPL_TCGEN05_TILE) return tc_ok ? STRATA_IMPL_TCGEN05 : -1;
   return tc_ok ? STRATA_IMPL_TCGEN05 : STRATA_IMPL_SIMT;
 }
 

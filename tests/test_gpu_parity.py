@@ -10,7 +10,7 @@ from helpers import assert_parity, desc_of, device_inputs, to_f64
 
 pytestmark = pytest.mark.gpu
 
-IMPLS = [binding.IMPL_SIMT, binding.IMPL_AUTO]
+IMPLS = [binding.IMPL_SIMT, binding.IMPL_AUTO, binding.IMPL_TCGEN05_TILE]
 
 
 def run_fwd(w, inp, impl=binding.IMPL_AUTO, scale=0.0):
@@ -53,7 +53,7 @@ def check_full(oracle_mod, w, impl, backward=True, scale=0.0):
 
 
 # ------------------------------------------------------------------ BASELINE.json configs
-@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("impl", IMPLS[:2])
 def test_config0_tiny_fp32_fwd_bwd(oracle_mod, impl):
     check_full(oracle_mod, wl.config(0), impl)
 
@@ -123,6 +123,11 @@ SWEEP = [
     dict(grid=(6, 16, 16), window=(5, 9, 9), heads=2, head_dim=128, batch=2),      # tcgen05 d=128, exact tiles
     dict(grid=(2, 40, 9), window=(1, 7, 7), heads=1, head_dim=64),                 # (1,7,7): SIMT fallback
     dict(grid=(8, 24, 32), window=(3, 7, 7), heads=2, head_dim=64, rope_axes=3),   # tcgen05 + 3-axis RoPE
+    dict(grid=(4, 9, 10), window=(3, 5, 5), heads=2, head_dim=64),                 # level sweep, 2 tiles
+    dict(grid=(6, 17, 9), window=(3, 3, 3), heads=2, head_dim=64, batch=2),        # level sweep, 3 tiles
+    dict(grid=(10, 20, 12), window=(3, 7, 7), heads=1, head_dim=64),               # level sweep, 5 tiles
+    dict(grid=(3, 8, 8), window=(3, 7, 7), heads=2, head_dim=64),                  # level sweep, L = k_L
+    dict(grid=(12, 7, 30), window=(3, 7, 7), heads=1, head_dim=64),                # level sweep, Y = k_Y
 ]
 
 
