@@ -52,6 +52,15 @@ cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1,
                                void* y0, void* y1, int out_dtype, const float* coords,
                                const float* freqs, float sign, cudaStream_t stream, int* launches);
 
+// rope.cu: A1 as a table, [B, L, Y, X, D/2] half2 (cos, sin), for the fused tensor-core kernels.
+cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
+                              cudaStream_t stream, int* launches);
+
+// na3d_fwd_fused.cu: tcgen05 forward with the rotation of Q and K fused in (un-rotated bf16 operands).
+bool fused_fwd_supported(const Problem& p);
+cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
+                             void* o, float* lse, cudaStream_t stream, int* launches);
+
 // na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
 cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             void* o, float* lse, cudaStream_t stream, int* launches);

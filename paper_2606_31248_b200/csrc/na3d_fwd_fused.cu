@@ -1,0 +1,697 @@
+// na3d_fwd_fused.cu -- fused StereoRoPE + 3D neighbourhood attention forward (tcgen05 / TMEM / TMA).
+//
+// Steps A2-A6 of DESIGN.md in ONE kernel (A1, the per-token cos/sin table, is rope.cu's small
+// pre-kernel): Q and K arrive un-rotated, are rotated in registers by a dedicated warpgroup and go
+// to the tensor cores from shared memory; the rotated copies never touch HBM.
+//
+// Work decomposition ("level sweep"): one CTA owns a level COLUMN of one (sample, head): the
+// TY x TX patch of every level, i.e. ceil(L / TL) query tiles of TL x TY x TX = 128 queries.  The
+// key / value planes of the column's halo ((TY+kY-1) x (TX+kX-1) keys per level) stream through
+// shared memory ONCE, level by level, in parts of CY key rows; every part is multiplied against the
+// (at most two) query tiles whose clamped level windows (R1) reach its plane.
+// Two independent tile pipelines ("slots") run inside the CTA: slot s owns tiles s, s+2, ...
+// (their plane ranges are disjoint and increasing, checked on the host).  Each slot has its own MMA
+// issuer thread, its own softmax warpgroup (one query row per thread = one TMEM lane) and 256 TMEM
+// columns: O [0, D) fp32 | S0 | S1 (S is double buffered; P (bf16) is written over the front of the
+// S buffer it came from and is the TMEM A-operand of the PV MMA).
+//
+// Warps (512 threads):
+//   0      TMA producer: K + rotary-table + V parts into a stage ring; Q tiles + their table rows
+//   1, 2   MMA issuer of slot 0 / 1
+//   3      TMEM owner
+//   4-7    rotation warpgroup: rotates every K part and every Q tile IN PLACE in shared memory
+//          (fp32 math on bf16 pairs, cos/sin from the fp16 table), then hands them to the MMA issuers
+//   8-11   softmax + epilogue of slot 0        12-15   softmax + epilogue of slot 1
+// Register budget via setmaxnreg: 56 / 88 / 184 / 184 per thread for the four warpgroups.
+//
+// Softmax: exp2 with a LAZY reference maximum -- the row maximum is computed only for the first
+// part that holds a valid key of the row and when a partial sum overflows 2^40; otherwise one pass
+// of FFMA2 (scale + column bias), FADD2 (row bias), MUFU.EX2, FADD2 (row sum), F2FP (bf16 pack):
+// 3 instructions per logit.
+#include <cuda_fp16.h>
+
+#include "tc_common.cuh"
+
+namespace strata {
+namespace {
+
+using namespace tc;
+
+template <int D_, int KL_, int KY_, int KX_, int TL_, int TY_, int TX_, int CY_, int NS_>
+struct FusedCfg {
+  static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
+  static constexpr int TL = TL_, TY = TY_, TX = TX_, M = 128;
+  static constexpr int HY = TY + KY - 1, HX = TX + KX - 1;
+  static constexpr int CY = CY_;                                   // key rows per part
+  static constexpr int NPARTS = (HY + CY - 1) / CY;
+  static constexpr int TAIL = HY - (NPARTS - 1) * CY;              // rows of the last part of a full halo
+  static constexpr int NMAX = (CY * HX + 15) / 16 * 16;            // UMMA N of a full part
+  static constexpr int DSUB = D / 64;                              // 128-byte sub-rows per head row
+  static constexpr int SUB_KV = NMAX * 128, SUB_Q = M * 128;       // bytes of one sub-tile
+  static constexpr int STAGE_BYTES = DSUB * SUB_KV, Q_BYTES = DSUB * SUB_Q;
+  static constexpr int NSTAGE = NS_;
+  static constexpr int NQBUF = (D == 64) ? 2 : 1;                  // Q buffers per slot
+  static constexpr int TMEM_SLOT = 256, TMEM_O = 0, TMEM_S = D;
+  static constexpr int NBARS = 5 * NSTAGE + 2 * 12 + 1;
+  static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16;
+  static_assert(TL * TY * TX == 128 && (TY * TX) % 32 == 0, "128 queries per tile, one level per warp");
+  static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1 && TX % 2 == 0, "odd windows only (HX even)");
+  static_assert(TL >= KL - 1, "tiles t and t+2 must reach disjoint planes");
+  static_assert(D == 64 || D == 128, "head_dim 64 or 128");
+  static_assert(HX <= 16 && (CY - 1) * HX + 16 <= NMAX, "row loads stay inside the S buffer");
+  static_assert(D + 2 * NMAX <= TMEM_SLOT, "TMEM columns of a slot");
+  static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+};
+
+struct FusedParams {
+  int B, H, L, Y, X;
+  int nty, ntx;
+  long long N;
+  float scale_log2e;
+  int rope;       // 0: no rotation (rope_axes == 0)
+  int pairing;    // 0: (2j, 2j+1)   1: (j, j + D/2)
+};
+
+constexpr int kFusedThreads = 512;
+constexpr float kBig = 1099511627776.f;   // 2^40: partial row sums above this trigger a new reference maximum
+
+// ------------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ffma2(float& d0, float& d1, float a0, float a1, float b, float c0, float c1) {
+  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %4};\n\tmov.b64 rc, {%5, %6};\n\t"
+      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b), "f"(c0), "f"(c1));
+}
+__device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ void ld16_issue(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr) : "memory");
+}
+// wait::ld with the loaded registers as in/out operands: no use of them can be scheduled above it.
+__device__ __forceinline__ void ld16_wait(uint32_t (&r)[16]) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;"
+               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                 "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+               :: "memory");
+}
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// A2 on one (a, b) bf16 pair held in `w` (a = low half) with (cos, sin) as a half2 in `t`.
+__device__ __forceinline__ uint32_t rot_pair(uint32_t w, uint32_t t) {
+  const float a = __uint_as_float(w << 16), b = __uint_as_float(w & 0xffff0000u);
+  const float2 cs = __half22float2(*reinterpret_cast<const __half2*>(&t));
+  return pack_bf16(fmaf(a, cs.x, -b * cs.y), fmaf(a, cs.y, b * cs.x));
+}
+// HALF pairing: `wa` holds channels (j, j+1), `wb` channels (j + D/2, j + 1 + D/2); t0 / t1 the (cos, sin) of pairs j / j+1.
+__device__ __forceinline__ void rot_half(uint32_t& wa, uint32_t& wb, uint32_t t0, uint32_t t1) {
+  const float a0 = __uint_as_float(wa << 16), a1 = __uint_as_float(wa & 0xffff0000u);
+  const float b0 = __uint_as_float(wb << 16), b1 = __uint_as_float(wb & 0xffff0000u);
+  const float2 c0 = __half22float2(*reinterpret_cast<const __half2*>(&t0));
+  const float2 c1 = __half22float2(*reinterpret_cast<const __half2*>(&t1));
+  wa = pack_bf16(fmaf(a0, c0.x, -b0 * c0.y), fmaf(a1, c1.x, -b1 * c1.y));
+  wb = pack_bf16(fmaf(a0, c0.y, b0 * c0.x), fmaf(a1, c1.y, b1 * c1.x));
+}
+
+// Rotate `rows` head rows in place.  x_smem / t_smem: operand tile and its table tile, both in the
+// TMA 128-byte-swizzled layout [sub][row][128 B] with `sub_stride` bytes between sub-tiles.  The
+// table tile has the operand's geometry (same box), so for the interleaved pairing the 16-byte
+// chunk at a physical offset of one holds the four (cos, sin) of the four pairs at that offset of
+// the other: the loop is linear over physical chunks.  128 threads, tid in [0, 128).
+template <int DSUB>
+__device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem, uint32_t sub_stride, int rows,
+                                               int pairing, int tid) {
+  if (pairing == 0) {
+    const int n = rows * 8;
+#pragma unroll
+    for (int sub = 0; sub < DSUB; ++sub) {
+      const uint32_t xb = x_smem + sub * sub_stride, tb = t_smem + sub * sub_stride;
+      for (int idx = tid; idx < n; idx += 256) {
+        const int idx2 = idx + 128;
+        const bool two = idx2 < n;
+        uint4 x0 = lds128(xb + idx * 16), t0 = lds128(tb + idx * 16);
+        uint4 x1 = make_uint4(0, 0, 0, 0), t1 = make_uint4(0, 0, 0, 0);
+        if (two) { x1 = lds128(xb + idx2 * 16); t1 = lds128(tb + idx2 * 16); }
+        x0.x = rot_pair(x0.x, t0.x); x0.y = rot_pair(x0.y, t0.y); x0.z = rot_pair(x0.z, t0.z); x0.w = rot_pair(x0.w, t0.w);
+        sts128(xb + idx * 16, x0);
+        if (two) {
+          x1.x = rot_pair(x1.x, t1.x); x1.y = rot_pair(x1.y, t1.y); x1.z = rot_pair(x1.z, t1.z); x1.w = rot_pair(x1.w, t1.w);
+          sts128(xb + idx2 * 16, x1);
+        }
+      }
+    }
+  } else {
+    // pair j = channels (j, j + D/2).  Work item = (row, c): the 8 pairs 8c .. 8c+7, c < D/16.
+    constexpr int CPR = DSUB * 4;                       // work items per row
+    const int n = rows * CPR;
+    for (int idx = tid; idx < n; idx += 128) {
+      const int row = idx / CPR, c = idx - row * CPR;
+      const uint32_t sw = (uint32_t)(row & 7), rowoff = (uint32_t)row * 128u;
+      uint32_t a_addr, b_addr;
+      if (DSUB == 1) {                                  // a: logical chunk c, b: logical chunk c + 4
+        a_addr = x_smem + rowoff + (((uint32_t)c ^ sw) << 4);
+        b_addr = x_smem + rowoff + (((uint32_t)(c + 4) ^ sw) << 4);
+      } else {                                          // a in sub-tile 0, b in sub-tile 1, same chunk
+        a_addr = x_smem + rowoff + (((uint32_t)c ^ sw) << 4);
+        b_addr = a_addr + sub_stride;
+      }
+      const int q0 = 2 * c, q1 = 2 * c + 1;             // table chunks (4 pairs each) of pairs 8c .. 8c+7
+      const uint32_t t0_addr = t_smem + (uint32_t)(q0 >> 3) * sub_stride + rowoff + (((uint32_t)(q0 & 7) ^ sw) << 4);
+      const uint32_t t1_addr = t_smem + (uint32_t)(q1 >> 3) * sub_stride + rowoff + (((uint32_t)(q1 & 7) ^ sw) << 4);
+      uint4 xa = lds128(a_addr), xbv = lds128(b_addr), t0 = lds128(t0_addr), t1 = lds128(t1_addr);
+      rot_half(xa.x, xbv.x, t0.x, t0.y); rot_half(xa.y, xbv.y, t0.z, t0.w);
+      rot_half(xa.z, xbv.z, t1.x, t1.y); rot_half(xa.w, xbv.w, t1.z, t1.w);
+      sts128(a_addr, xa); sts128(b_addr, xbv);
+    }
+  }
+}
+
+// Position of one slot in the global part stream (plane-major, part-minor).
+template <class C>
+struct SlotWalk {
+  int t;   // current tile of the slot
+  static __device__ __host__ __forceinline__ int plo(int t, int L) { return window_start(C::TL * t, C::KL, L); }
+  static __device__ __host__ __forceinline__ int phi(int t, int L) {
+    const int last = C::TL * t + C::TL - 1;
+    return window_start(last < L - 1 ? last : L - 1, C::KL, L) + C::KL;
+  }
+  __device__ __forceinline__ void classify(int plane, int part, int nparts, int ntl, int L, bool& needed,
+                                           bool& first, bool& last) {
+    while (t < ntl && plane >= phi(t, L)) t += 2;
+    needed = t < ntl && plane >= plo(t, L);
+    first = needed && plane == plo(t, L) && part == 0;
+    last = needed && plane == phi(t, L) - 1 && part == nparts - 1;
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
+// Kernel
+// ------------------------------------------------------------------------------------------------
+template <class C>
+__global__ void __launch_bounds__(kFusedThreads, 1)
+na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                      const __grid_constant__ CUtensorMap tm_kt, const __grid_constant__ CUtensorMap tm_v,
+                      const __grid_constant__ CUtensorMap tm_vt, const __grid_constant__ CUtensorMap tm_tq,
+                      const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tkt,
+                      __nv_bfloat16* __restrict__ o, float* __restrict__ lse, const FusedParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  const uint32_t q_smem = base;                                        // [slot][buf] x Q_BYTES
+  const uint32_t qt_smem = q_smem + 2 * C::NQBUF * C::Q_BYTES;         // table rows of the Q tile being rotated
+  const uint32_t k_smem = qt_smem + C::Q_BYTES;
+  const uint32_t t_smem = k_smem + C::NSTAGE * C::STAGE_BYTES;
+  const uint32_t v_smem = t_smem + C::NSTAGE * C::STAGE_BYTES;
+  const uint32_t bars = v_smem + C::NSTAGE * C::STAGE_BYTES;
+  auto bar_kfull = [&](int s) { return bars + 8u * s; };                          // TMA -> rotation
+  auto bar_krot = [&](int s) { return bars + 8u * (C::NSTAGE + s); };             // rotation -> MMA (128)
+  auto bar_kempty = [&](int s) { return bars + 8u * (2 * C::NSTAGE + s); };       // MMA (both slots) -> TMA
+  auto bar_vfull = [&](int s) { return bars + 8u * (3 * C::NSTAGE + s); };
+  auto bar_vempty = [&](int s) { return bars + 8u * (4 * C::NSTAGE + s); };
+  // per slot: 0,1 qfull[buf]  2,3 qrot[buf]  4,5 qfree[buf]  6,7 sfull[buf]  8,9 pfull[buf]  10,11 pvdone[buf]
+  // Every barrier that is not waited on in every phase is split by parity of its use count: a waiter
+  // may only test the parity of a phase when the barrier is known to be in that phase or the next.
+  auto bar_slot = [&](int slot, int which) { return bars + 8u * (5 * C::NSTAGE + 12 * slot + which); };
+  const uint32_t bar_qtempty = bars + 8u * (5 * C::NSTAGE + 24);
+  const uint32_t tmem_word = bars + 8u * C::NBARS;
+  uint32_t* tmem_word_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_word - raw));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- the level column of this CTA: x fastest, then y, head, sample
+  int bid = blockIdx.x;
+  const int tx = bid % p.ntx; bid /= p.ntx;
+  const int ty = bid % p.nty; bid /= p.nty;
+  const int h = bid % p.H;
+  const int b = bid / p.H;
+  const int x0 = tx * C::TX, y0 = ty * C::TY;
+  const int yl = min(y0 + C::TY, p.Y) - 1;
+  const int hs_x = window_start(x0, C::KX, p.X), hs_y = window_start(y0, C::KY, p.Y);
+  const int hy = window_start(yl, C::KY, p.Y) + C::KY - hs_y;     // key rows of the halo, <= HY
+  const int nparts = (hy + C::CY - 1) / C::CY;
+  const int ntl = (p.L + C::TL - 1) / C::TL;
+  const int bl = b * p.L;
+  const uint32_t op_tx = p.rope ? 2u : 1u;                        // operand + table bytes per barrier
+
+  // ---- one-time setup
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_kt);
+    tma_prefetch_desc(&tm_v); tma_prefetch_desc(&tm_vt);
+    if (p.rope) { tma_prefetch_desc(&tm_tq); tma_prefetch_desc(&tm_tk); tma_prefetch_desc(&tm_tkt); }
+    for (int s = 0; s < C::NSTAGE; ++s) {
+      mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 128); mbar_init(bar_kempty(s), 2);
+      mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 2);
+    }
+    for (int slot = 0; slot < 2; ++slot) {
+      mbar_init(bar_slot(slot, 0), 1); mbar_init(bar_slot(slot, 1), 1);
+      mbar_init(bar_slot(slot, 2), 128); mbar_init(bar_slot(slot, 3), 128);
+      mbar_init(bar_slot(slot, 4), 1); mbar_init(bar_slot(slot, 5), 1);
+      mbar_init(bar_slot(slot, 6), 1); mbar_init(bar_slot(slot, 7), 1);
+      mbar_init(bar_slot(slot, 8), 128); mbar_init(bar_slot(slot, 9), 128);
+      mbar_init(bar_slot(slot, 10), 1); mbar_init(bar_slot(slot, 11), 1);
+    }
+    mbar_init(bar_qtempty, 128);
+    fence_barrier_init();
+  }
+  if (warp == 3) tmem_alloc(tmem_word, 512);
+  // V stages start as zeros: rows of a stage that a (shorter) part does not overwrite are multiplied
+  // by P = 0 in the PV MMA and must therefore hold finite numbers.
+  for (uint32_t off = threadIdx.x * 16u; off < (uint32_t)(C::NSTAGE * C::STAGE_BYTES); off += kFusedThreads * 16u)
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(v_smem + off), "r"(0u) : "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_word_ptr;
+
+  if (warp < 4) {
+    reg_dec<56>();
+    if (warp == 0) {
+      // =========================== TMA producer ===========================
+      if (lane == 0) {
+        SlotWalk<C> walk[2] = {{0}, {1}};
+        int g = 0, qjob = 0;
+        for (int plane = 0; plane < p.L; ++plane)
+          for (int part = 0; part < nparts; ++part, ++g) {
+#pragma unroll
+            for (int slot = 0; slot < 2; ++slot) {
+              bool needed, first, last;
+              walk[slot].classify(plane, part, nparts, ntl, p.L, needed, first, last);
+              if (!first) continue;
+              const int nseq = (walk[slot].t - slot) >> 1;           // tiles of this slot so far
+              const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;  // use-th tile in this Q buffer
+              if (use >= 1) mbar_wait(bar_slot(slot, 4 + buf), (uint32_t)(use - 1) & 1u);   // its last QK^T is done
+              if (p.rope && qjob >= 1) mbar_wait(bar_qtempty, (uint32_t)(qjob - 1) & 1u);
+              const uint32_t bar = bar_slot(slot, buf);
+              mbar_expect_tx(bar, op_tx * C::Q_BYTES);
+              const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
+#pragma unroll
+              for (int j = 0; j < C::DSUB; ++j) {
+                tma_load_5d(qb + j * C::SUB_Q, &tm_q, bar, 64 * j, h, x0, y0, bl + C::TL * walk[slot].t);
+                if (p.rope) tma_load_5d(qt_smem + j * C::SUB_Q, &tm_tq, bar, 64 * j, 0, x0, y0, bl + C::TL * walk[slot].t);
+              }
+              ++qjob;
+            }
+            const int s = g % C::NSTAGE;
+            const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+            const int nrows = min(C::CY, hy - part * C::CY);
+            const bool tail = (C::TAIL < C::CY) && nrows <= C::TAIL;
+            const uint32_t bytes = (uint32_t)((tail ? C::TAIL : C::CY) * C::HX * 128 * C::DSUB);
+            const int cy0 = hs_y + part * C::CY;
+            mbar_wait(bar_kempty(s), ph ^ 1u);
+            mbar_expect_tx(bar_kfull(s), op_tx * bytes);
+#pragma unroll
+            for (int j = 0; j < C::DSUB; ++j) {
+              tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_kt : &tm_k, bar_kfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+              if (p.rope)
+                tma_load_5d(t_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_tkt : &tm_tk, bar_kfull(s), 64 * j, 0, hs_x, cy0, bl + plane);
+            }
+            mbar_wait(bar_vempty(s), ph ^ 1u);
+            mbar_expect_tx(bar_vfull(s), bytes);
+#pragma unroll
+            for (int j = 0; j < C::DSUB; ++j)
+              tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_vt : &tm_v, bar_vfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+          }
+      }
+    } else if (warp == 1 || warp == 2) {
+      // =========================== MMA issuer of one slot ===========================
+      if (lane == 0) {
+        const int slot = warp - 1;
+        const uint32_t tm = tmem + slot * C::TMEM_SLOT;
+        constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
+        struct Pending { int i, g, stage, n; uint32_t ph; bool first; };
+        Pending prev{};
+        bool have_prev = false;
+        auto issue_mma2 = [&](const Pending& it) {
+          mbar_wait(bar_slot(slot, 8 + (it.i & 1)), (uint32_t)(it.i >> 1) & 1u);   // P of item i is in TMEM
+          mbar_wait(bar_vfull(it.stage), it.ph);
+          tc_fence_after();
+          const uint32_t a_tmem = tm + C::TMEM_S + (it.i & 1) * C::NMAX;
+          for (int ks = 0; ks < it.n / 16; ++ks) {
+#pragma unroll
+            for (int j = 0; j < C::DSUB; ++j) {
+              const uint64_t bd = smem_desc(v_smem + it.stage * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
+              umma_ts(tm + C::TMEM_O + 64 * j, a_tmem + 8 * ks, bd, idesc_pv, (!it.first || ks > 0) ? 1u : 0u);
+            }
+          }
+          umma_commit(bar_vempty(it.stage));
+          umma_commit(bar_slot(slot, 10 + (it.i & 1)));
+        };
+
+        SlotWalk<C> walk{slot};
+        int i = 0, g = 0;
+        for (int plane = 0; plane < p.L; ++plane)
+          for (int part = 0; part < nparts; ++part, ++g) {
+            bool needed, first, last;
+            walk.classify(plane, part, nparts, ntl, p.L, needed, first, last);
+            const int s = g % C::NSTAGE;
+            const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+            if (!needed) {       // this slot does not use the part: release it once it is rotated / has landed
+              mbar_wait(bar_krot(s), ph);       // (one arrival per slot and phase, never ahead of the producer)
+              mbar_arrive(bar_kempty(s));
+              mbar_wait(bar_vfull(s), ph);
+              mbar_arrive(bar_vempty(s));
+              continue;
+            }
+            // never hold a V stage across a gap that could stall the producer (deadlock guard)
+            if (have_prev && g - prev.g >= C::NSTAGE - 1) { issue_mma2(prev); have_prev = false; }
+            const int nseq = (walk.t - slot) >> 1;
+            const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;
+            if (first) mbar_wait(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);     // Q tile rotated
+            mbar_wait(bar_krot(s), ph);
+            tc_fence_after();
+            const int nrows = min(C::CY, hy - part * C::CY);
+            const int n = (nrows * C::HX + 15) / 16 * 16;
+            const uint32_t idesc_qk = instr_desc(C::M, n, false);
+            const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < C::D / 16; ++ks) {
+              const uint32_t sub = (uint32_t)(ks >> 2), kin = (uint32_t)(ks & 3) * 32u;
+              umma_ss(tm + C::TMEM_S + (i & 1) * C::NMAX, smem_desc(qb + sub * C::SUB_Q + kin),
+                      smem_desc(k_smem + s * C::STAGE_BYTES + sub * C::SUB_KV + kin), idesc_qk, ks > 0 ? 1u : 0u);
+            }
+            umma_commit(bar_kempty(s));
+            umma_commit(bar_slot(slot, 6 + (i & 1)));
+            if (last) umma_commit(bar_slot(slot, 4 + buf));       // every QK^T of the tile is done: Q buffer free
+            if (have_prev) issue_mma2(prev);
+            prev = Pending{i, g, s, n, ph, first};
+            have_prev = true;
+            ++i;
+          }
+        if (have_prev) issue_mma2(prev);
+      }
+    }
+  } else if (warp < 8) {
+    // =========================== rotation warpgroup ===========================
+    reg_dec<88>();
+    const int tid = threadIdx.x - 128;
+    SlotWalk<C> walk[2] = {{0}, {1}};
+    int g = 0;
+    for (int plane = 0; plane < p.L; ++plane)
+      for (int part = 0; part < nparts; ++part, ++g) {
+#pragma unroll
+        for (int slot = 0; slot < 2; ++slot) {
+          bool needed, first, last;
+          walk[slot].classify(plane, part, nparts, ntl, p.L, needed, first, last);
+          if (!first) continue;
+          const int nseq = (walk[slot].t - slot) >> 1;
+          const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;
+          mbar_wait(bar_slot(slot, buf), (uint32_t)use & 1u);                      // Q tile (+ table) landed
+          if (p.rope) {
+            rotate_inplace<C::DSUB>(q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES, qt_smem, C::SUB_Q, C::M, p.pairing, tid);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_arrive(bar_qtempty);
+          }
+          mbar_arrive(bar_slot(slot, 2 + buf));
+        }
+        const int s = g % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+        mbar_wait(bar_kfull(s), ph);
+        if (p.rope) {
+          const int nrows = min(C::CY, hy - part * C::CY);
+          const bool tail = (C::TAIL < C::CY) && nrows <= C::TAIL;
+          rotate_inplace<C::DSUB>(k_smem + s * C::STAGE_BYTES, t_smem + s * C::STAGE_BYTES, C::SUB_KV,
+                                  (tail ? C::TAIL : C::CY) * C::HX, p.pairing, tid);
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        mbar_arrive(bar_krot(s));
+      }
+  } else {
+    // =========================== softmax + epilogue of one slot ===========================
+    reg_inc<184>();
+    const int slot = (warp - 8) >> 2;
+    const int sp = warp & 3;                       // TMEM subpartition
+    const int row = sp * 32 + lane;                // query row of the tile == TMEM lane
+    const uint32_t tm = tmem + slot * C::TMEM_SLOT + ((uint32_t)(sp * 32) << 16);
+    const int qx = row % C::TX, qy = (row / C::TX) % C::TY, ql = row / (C::TX * C::TY);
+    const int ax = min(x0 + qx, p.X - 1), ay = min(y0 + qy, p.Y - 1);
+    const bool active_xy = (x0 + qx < p.X) && (y0 + qy < p.Y);
+    const int lo_x = window_start(ax, C::KX, p.X) - hs_x;
+    const int lo_y = window_start(ay, C::KY, p.Y) - hs_y;
+    const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
+    const float cs = p.scale_log2e;
+    float xb[C::HX];                               // column bias: -m_ref inside the x window, -inf outside
+
+    int i = 0;
+    for (int tile = slot; tile < ntl; tile += 2) {
+      const int al = min(C::TL * tile + ql, p.L - 1);
+      const bool active = active_xy && (C::TL * tile + ql < p.L);
+      const int pw_lo = window_start(al, C::KL, p.L);              // planes of this query: [pw_lo, pw_lo + KL)
+      const int wl_lo = __reduce_min_sync(0xffffffffu, pw_lo), wl_hi = __reduce_max_sync(0xffffffffu, pw_lo + C::KL);
+      float m_ref = 0.f, lsum = 0.f;
+      bool inited = false;
+#pragma unroll
+      for (int j = 0; j < C::HX; ++j) xb[j] = (j >= lo_x && j < lo_x + C::KX) ? 0.f : -INFINITY;
+      const int plo = SlotWalk<C>::plo(tile, p.L), phi = SlotWalk<C>::phi(tile, p.L);
+      for (int plane = plo; plane < phi; ++plane) {
+        const bool plane_needed = plane >= wl_lo && plane < wl_hi;
+        const bool plane_ok = plane >= pw_lo && plane < pw_lo + C::KL;
+        for (int part = 0; part < nparts; ++part, ++i) {
+          const int r_base = part * C::CY;
+          const int nrows = min(C::CY, hy - r_base);
+          const int nwords = ((nrows * C::HX + 15) / 16 * 16) / 2;
+          const uint32_t s_addr = tm + C::TMEM_S + (i & 1) * C::NMAX;
+          const bool first_item = (plane == plo && part == 0);
+          // rows of this part that some query of the warp needs: [ra, rb)
+          const int ra = plane_needed ? max(0, wy_lo - r_base) : 0;
+          const int rb = plane_needed ? min(nrows, wy_hi - r_base) : 0;
+          const bool has_valid = plane_ok && lo_y < r_base + nrows && lo_y + C::KY > r_base;
+          mbar_wait(bar_slot(slot, 6 + (i & 1)), (uint32_t)(i >> 1) & 1u);
+          tc_fence_after();
+
+          // rolling double-buffered walk over the needed rows of S
+          auto for_rows = [&](auto&& body) {
+            uint32_t sva[16], svb[16];
+            if (0 >= ra && 0 < rb) ld16_issue(s_addr, sva);
+#pragma unroll
+            for (int r = 0; r < C::CY; ++r) {
+              uint32_t (&cur)[16] = (r & 1) ? svb : sva;
+              uint32_t (&nxt)[16] = (r & 1) ? sva : svb;
+              const bool need_r = r >= ra && r < rb;
+              if (need_r) ld16_wait(cur);
+              if (r + 1 < C::CY && r + 1 >= ra && r + 1 < rb) ld16_issue(s_addr + (r + 1) * C::HX, nxt);
+              body(r, need_r, cur);
+            }
+          };
+
+          uint32_t pw[C::NMAX / 2];
+          float csum = 0.f;
+          bool fix = __any_sync(0xffffffffu, has_valid && !inited);
+          while (true) {
+            if (fix) {
+              // ---- slow path: true maximum of the valid logits of this part -> new reference maximum
+              float cmax = -INFINITY;
+              for_rows([&](int r, bool need_r, uint32_t (&sv)[16]) {
+                if (need_r) {
+                  const int py = r_base + r;
+                  const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
+                  float rmax = -INFINITY;
+#pragma unroll
+                  for (int j = 0; j < C::HX; ++j) {
+                    const float t = (j >= lo_x && j < lo_x + C::KX) ? __uint_as_float(sv[j]) * cs : -INFINITY;
+                    rmax = fmaxf(rmax, t);
+                  }
+                  if (rowok) cmax = fmaxf(cmax, rmax);
+                }
+              });
+              const bool got = cmax > -INFINITY;
+              const float new_ref = got ? (inited ? fmaxf(m_ref, cmax) : cmax) : m_ref;
+              const float alpha = (inited && new_ref != m_ref) ? ex2(m_ref - new_ref) : 1.f;
+              if (!first_item && __any_sync(0xffffffffu, alpha != 1.f)) {
+                // O holds earlier parts of this tile: rescale its rows (all its PV MMAs are complete)
+                mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
+                tc_fence_after();
+#pragma unroll
+                for (int j = 0; j < C::D; j += 16) {
+                  float ov[16];
+                  tmem_ld16(tm + C::TMEM_O + j, ov);
+                  tmem_wait_ld();
+                  uint32_t ow[16];
+#pragma unroll
+                  for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
+                  tmem_st16(tm + C::TMEM_O + j, ow);
+                }
+                tmem_wait_st();
+              }
+              lsum *= alpha;
+              m_ref = new_ref;
+              inited = inited || got;
+#pragma unroll
+              for (int j = 0; j < C::HX; ++j) xb[j] = (j >= lo_x && j < lo_x + C::KX) ? -m_ref : -INFINITY;
+            }
+            // ---- fast path: p = 2^(s * cs - m_ref), masked by the additive biases
+            float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+            for_rows([&](int r, bool need_r, uint32_t (&sv)[16]) {
+              if (need_r) {
+                const int py = r_base + r;
+                const float rbias = (plane_ok && py >= lo_y && py < lo_y + C::KY) ? 0.f : -INFINITY;
+#pragma unroll
+                for (int j = 0; j < C::HX; j += 2) {
+                  float t0, t1;
+                  ffma2(t0, t1, __uint_as_float(sv[j]), __uint_as_float(sv[j + 1]), cs, xb[j], xb[j + 1]);
+                  fadd2(t0, t1, t0, t1, rbias, rbias);
+                  const float p0 = ex2(t0), p1 = ex2(t1);
+                  if ((j >> 1) & 1) fadd2(a2, a3, a2, a3, p0, p1);
+                  else fadd2(a0, a1, a0, a1, p0, p1);
+                  pw[(r * C::HX + j) >> 1] = pack_bf16(p0, p1);
+                }
+              } else {
+#pragma unroll
+                for (int j = 0; j < C::HX; j += 2) pw[(r * C::HX + j) >> 1] = 0u;
+              }
+            });
+            csum = (a0 + a1) + (a2 + a3);
+            if (fix) break;                                  // every valid p <= 1 after a fix
+            fix = __any_sync(0xffffffffu, !(csum <= kBig));
+            if (!fix) break;
+          }
+          lsum += csum;
+#pragma unroll
+          for (int j = C::CY * C::HX / 2; j < C::NMAX / 2; ++j) pw[j] = 0u;    // pad keys of a full part
+          // P (bf16 pairs) over the front of the S buffer, then hand the item to the PV MMA
+#pragma unroll
+          for (int j = 0; j < C::NMAX / 2; j += 8)
+            if (j < nwords) tmem_st8(s_addr + j, &pw[j]);
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bar_slot(slot, 8 + (i & 1)));
+        }
+      }
+      // ---- tile epilogue: O / l -> bf16 -> global, LSE
+      mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
+      tc_fence_after();
+      const float inv = 1.f / lsum;
+      const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
+      __nv_bfloat16* orow = o + (((long long)b * p.N + tok) * p.H + h) * C::D;
+#pragma unroll
+      for (int j = 0; j < C::D; j += 16) {
+        float ov[16];
+        tmem_ld16(tm + C::TMEM_O + j, ov);
+        tmem_wait_ld();
+        if (active) {
+          uint4 w0, w1;
+          w0.x = pack_bf16(ov[0] * inv, ov[1] * inv);   w0.y = pack_bf16(ov[2] * inv, ov[3] * inv);
+          w0.z = pack_bf16(ov[4] * inv, ov[5] * inv);   w0.w = pack_bf16(ov[6] * inv, ov[7] * inv);
+          w1.x = pack_bf16(ov[8] * inv, ov[9] * inv);   w1.y = pack_bf16(ov[10] * inv, ov[11] * inv);
+          w1.z = pack_bf16(ov[12] * inv, ov[13] * inv); w1.w = pack_bf16(ov[14] * inv, ov[15] * inv);
+          reinterpret_cast<uint4*>(orow + j)[0] = w0;
+          reinterpret_cast<uint4*>(orow + j)[1] = w1;
+        }
+      }
+      if (active) lse[((long long)b * p.H + h) * p.N + tok] = (m_ref + log2f(lsum)) * 0.69314718055994531f;
+      // the O reads above are complete before the next tile's first PV MMA overwrites O: that MMA
+      // waits for this warpgroup's next p_full arrival, which follows these (waited-for) loads.
+    }
+  }
+
+  // ---- teardown
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 3) {
+    tc_fence_after();
+    tmem_dealloc(tmem, 512);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host side
+// ------------------------------------------------------------------------------------------------
+template <class C>
+bool fused_shape_ok(const Problem& p) {
+  // the tiles of one slot must reach disjoint, increasing plane ranges (one pass over the levels)
+  const int ntl = (p.L + C::TL - 1) / C::TL;
+  for (int t = 0; t + 2 < ntl; ++t)
+    if (SlotWalk<C>::plo(t + 2, p.L) < SlotWalk<C>::phi(t, p.L)) return false;
+  return true;
+}
+
+template <class C>
+cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table, void* o,
+                         float* lse, cudaStream_t stream, int* launches) {
+  CUtensorMap tq, tk, tkt, tv, tvt, ttq, ttk, ttkt;
+  if (!make_map(&tq, q, p, C::TX, C::TY, C::TL) || !make_map(&tk, k, p, C::HX, C::CY, 1) ||
+      !make_map(&tkt, k, p, C::HX, C::TAIL, 1) || !make_map(&tv, v, p, C::HX, C::CY, 1) ||
+      !make_map(&tvt, v, p, C::HX, C::TAIL, 1))
+    return cudaErrorInvalidValue;
+  const bool rope = p.A > 0;
+  if (rope) {
+    Problem pt = p;
+    pt.H = 1;                                  // the table is [B, L, Y, X, D] 16-bit words: one "head"
+    if (!make_map(&ttq, table, pt, C::TX, C::TY, C::TL) || !make_map(&ttk, table, pt, C::HX, C::CY, 1) ||
+        !make_map(&ttkt, table, pt, C::HX, C::TAIL, 1))
+      return cudaErrorInvalidValue;
+  } else {
+    ttq = tq; ttk = tk; ttkt = tkt;            // never dereferenced
+  }
+  FusedParams fp;
+  fp.B = p.B; fp.H = p.H; fp.L = p.L; fp.Y = p.Y; fp.X = p.X; fp.N = p.N;
+  fp.nty = (p.Y + C::TY - 1) / C::TY; fp.ntx = (p.X + C::TX - 1) / C::TX;
+  fp.scale_log2e = p.scale * 1.4426950408889634f;
+  fp.rope = rope ? 1 : 0;
+  fp.pairing = p.pairing;
+  const long long grid = (long long)p.B * p.H * fp.nty * fp.ntx;
+  if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(na3d_fwd_fused_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  prof_begin("na3d_fwd_fused", stream);
+  na3d_fwd_fused_kernel<C><<<(unsigned)grid, kFusedThreads, C::SMEM_BYTES, stream>>>(
+      tq, tk, tkt, tv, tvt, ttq, ttk, ttkt, (__nv_bfloat16*)o, lse, fp);
+  prof_end(stream);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+// (D, kL, kY, kX, TL, TY, TX, CY, NSTAGE) instantiations.
+#define STRATA_FUSED_CONFIGS(X) \
+  X(64, 3, 7, 7, 2, 8, 8, 5, 4) \
+  X(64, 3, 5, 5, 2, 8, 8, 6, 4) \
+  X(64, 3, 3, 3, 2, 8, 8, 5, 4)
+
+bool fused_fwd_supported(const Problem& p) {
+  if (p.dtype != 1) return false;
+#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_)                   \
+  if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)          \
+    return fused_shape_ok<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_>>(p);
+  STRATA_FUSED_CONFIGS(X)
+#undef X
+  return false;
+}
+
+cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
+                             void* o, float* lse, cudaStream_t stream, int* launches) {
+#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_)                   \
+  if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)          \
+    return launch_fused<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_>>(p, q, k, v, table, o, lse, stream, launches);
+  STRATA_FUSED_CONFIGS(X)
+#undef X
+  return cudaErrorNotSupported;
+}
+
+}  // namespace strata

@@ -47,13 +47,24 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
   return true;
 }
 
-// AUTO -> tcgen05 when it covers the problem, else SIMT.  Returns -1 when `impl` asks for a
-// family that does not cover it.
-int select_impl(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
+// Kernel path of a call.  The public strata_impl_t only distinguishes SIMT from TCGEN05.
+enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_FUSED = 3 };
+
+// AUTO -> fused tcgen05 kernel when it covers the problem, else the tcgen05 tile kernel on pre-rotated
+// operands, else SIMT.  PATH_NONE when `impl` asks for a family that does not cover the problem.
+Path select_path(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
+  if (d->impl == STRATA_IMPL_SIMT) return PATH_SIMT;
+  const bool fused_ok = !backward && !p.force_tile && strata::fused_fwd_supported(p);
   const bool tc_ok = !backward && strata::tc_fwd_supported(p);
-  if (d->impl == STRATA_IMPL_SIMT) return STRATA_IMPL_SIMT;
-  if (d->impl == STRATA_IMPL_TCGEN05 || d->impl == STRATA_IMPL_TCGEN05_TILE) return tc_ok ? STRATA_IMPL_TCGEN05 : -1;
-  return tc_ok ? STRATA_IMPL_TCGEN05 : STRATA_IMPL_SIMT;
+  if (fused_ok) return PATH_TC_FUSED;
+  if (tc_ok) return PATH_TC_PREROT;
+  return d->impl == STRATA_IMPL_AUTO ? PATH_SIMT : PATH_NONE;
+}
+
+int select_impl(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
+  const Path path = select_path(d, p, backward);
+  if (path == PATH_NONE) return -1;
+  return path == PATH_SIMT ? STRATA_IMPL_SIMT : STRATA_IMPL_TCGEN05;
 }
 
 struct Carve {
@@ -65,11 +76,12 @@ struct Carve {
   }
 };
 
-size_t ws_bytes(const Problem& p, int impl, bool backward) {
+size_t ws_bytes(const Problem& p, Path path, bool backward) {
   const size_t e = (size_t)p.elems();
   const size_t stat = align_up((size_t)p.B * p.H * p.N * 4);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
-  if (impl == STRATA_IMPL_TCGEN05) return 2 * align_up(e * 2);           // qr, kr (bf16)
+  if (path == PATH_TC_FUSED) return align_up((size_t)p.B * p.N * p.D * 2);   // (cos, sin) half2 table
+  if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
   return 2 * align_up(e * 4);                                            // qr, kr (f32)
 }
 
@@ -122,20 +134,20 @@ int strata_na3d_profile_read(float* ms, const char** names, int capacity) {
 size_t strata_na3d_workspace_bytes(const strata_na3d_desc_t* desc, int backward) {
   Problem p; strata_status_t why;
   if (!make_problem(desc, &p, &why)) return 0;
-  const int impl = select_impl(desc, p, backward != 0);
-  if (impl < 0) return 0;
-  return ws_bytes(p, impl, backward != 0);
+  const Path path = select_path(desc, p, backward != 0);
+  if (path == PATH_NONE) return 0;
+  return ws_bytes(p, path, backward != 0);
 }
 
 size_t strata_na3d_host_workspace_bytes(const strata_na3d_desc_t* desc, int backward) {
   Problem p; strata_status_t why;
   if (!make_problem(desc, &p, &why)) return 0;
-  const int impl = select_impl(desc, p, backward != 0);
-  if (impl < 0) return 0;
+  const Path path = select_path(desc, p, backward != 0);
+  if (path == PATH_NONE) return 0;
   const size_t t = align_up(tensor_bytes(p)), s = align_up(stat_bytes(p));
   const size_t geo = align_up(coords_bytes(p)) + align_up(freqs_bytes(p));
   const size_t staged = backward ? 8 * t + s + geo : 4 * t + s + geo;
-  return staged + ws_bytes(p, impl, backward != 0);
+  return staged + ws_bytes(p, path, backward != 0);
 }
 
 int strata_na3d_impl_selected(const strata_na3d_desc_t* desc, int backward) {
@@ -154,14 +166,21 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
   if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) ||
       misaligned(coords) || misaligned(freqs) || misaligned(workspace))
     return STRATA_ERR_INVALID_ARG;
-  const int impl = select_impl(desc, p, false);
-  if (impl < 0) return STRATA_ERR_UNSUPPORTED;
-  if (!workspace || workspace_bytes < ws_bytes(p, impl, false)) return STRATA_ERR_WORKSPACE;
+  const Path path = select_path(desc, p, false);
+  if (path == PATH_NONE) return STRATA_ERR_UNSUPPORTED;
+  if (!workspace || workspace_bytes < ws_bytes(p, path, false)) return STRATA_ERR_WORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   Carve ws{reinterpret_cast<char*>(workspace), 0};
   int launches = 0;
   cudaError_t e;
-  if (impl == STRATA_IMPL_TCGEN05) {
+  if (path == PATH_TC_FUSED) {
+    void* table = ws.take<char>((size_t)p.B * p.N * p.D * 2);
+    if (p.A > 0) {
+      e = strata::launch_rope_table(p, table, coords, freqs, st, &launches);
+      if (e != cudaSuccess) return cuda_status(e);
+    }
+    e = strata::launch_fwd_fused(p, q, k, v, table, o, lse, st, &launches);
+  } else if (path == PATH_TC_PREROT) {
     void* qr = ws.take<char>((size_t)p.elems() * 2);
     void* kr = ws.take<char>((size_t)p.elems() * 2);
     e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
@@ -191,9 +210,9 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, c
       misaligned(lse) || misaligned(coords) || misaligned(freqs) || misaligned(dq) ||
       misaligned(dk) || misaligned(dv) || misaligned(workspace))
     return STRATA_ERR_INVALID_ARG;
-  const int impl = select_impl(desc, p, true);
-  if (impl < 0) return STRATA_ERR_UNSUPPORTED;
-  if (!workspace || workspace_bytes < ws_bytes(p, impl, true)) return STRATA_ERR_WORKSPACE;
+  const Path path = select_path(desc, p, true);
+  if (path == PATH_NONE) return STRATA_ERR_UNSUPPORTED;
+  if (!workspace || workspace_bytes < ws_bytes(p, path, true)) return STRATA_ERR_WORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   Carve ws{reinterpret_cast<char*>(workspace), 0};
   const size_t eb = (size_t)p.elems() * 4;
