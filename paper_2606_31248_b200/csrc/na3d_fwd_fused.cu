@@ -7,8 +7,10 @@
 // Work decomposition ("level sweep"): one CTA owns a level COLUMN of one (sample, head): the
 // TY x TX patch of every level, i.e. ceil(L / TL) query tiles of TL x TY x TX = 128 queries.  The
 // key / value planes of the column's halo ((TY+kY-1) x (TX+kX-1) keys per level) stream through
-// shared memory ONCE, level by level, in parts of CY key rows; every part is multiplied against the
-// (at most two) query tiles whose clamped level windows (R1) reach its plane.
+// shared memory ONCE, level by level, in three parts of key rows ([0, G), [G, G+kY-1), [G+kY-1, HY)
+// with G = 32 / TX query rows per softmax warp, so that away from the grid border a warp needs either
+// every row of a part or none); every part is multiplied against the (at most two) query tiles
+// whose clamped level windows (R1) reach its plane.
 // Two independent tile pipelines ("slots") run inside the CTA: slot s owns tiles s, s+2, ...
 // (their plane ranges are disjoint and increasing, checked on the host).  Each slot has its own MMA
 // issuer thread, its own softmax warpgroup (one query row per thread = one TMEM lane) and 256 TMEM
@@ -25,10 +27,14 @@
 // Register budget via setmaxnreg: 56 / 88 / 184 / 184 per thread for the four warpgroups.
 //
 // Softmax: exp2 with a LAZY reference maximum -- the row maximum is computed only for the first
-// part that holds a valid key of the row and when a partial sum overflows 2^40; otherwise one pass
-// of FFMA2 (scale + column bias), FADD2 (row bias), MUFU.EX2, FADD2 (row sum), F2FP (bf16 pack):
-// 3 instructions per logit.
+// part that holds a valid key of the row and when a partial sum overflows 2^40.  The x window of a
+// query covers kX of the HX halo columns; with kX <= HX/2 at most one of the columns c and c + HX/2
+// is inside it, so the two halves of every key row are FOLDED with a per-thread bit select before
+// the exponential (half the MUFU work) and un-folded again when P is packed to bf16.
 #include <cuda_fp16.h>
+
+#include <cstdlib>
+#include <type_traits>
 
 #include "tc_common.cuh"
 
@@ -37,15 +43,19 @@ namespace {
 
 using namespace tc;
 
-template <int D_, int KL_, int KY_, int KX_, int TL_, int TY_, int TX_, int CY_, int NS_>
+template <int D_, int KL_, int KY_, int KX_, int TL_, int TY_, int TX_, int NS_>
 struct FusedCfg {
   static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
   static constexpr int TL = TL_, TY = TY_, TX = TX_, M = 128;
-  static constexpr int HY = TY + KY - 1, HX = TX + KX - 1;
-  static constexpr int CY = CY_;                                   // key rows per part
-  static constexpr int NPARTS = (HY + CY - 1) / CY;
-  static constexpr int TAIL = HY - (NPARTS - 1) * CY;              // rows of the last part of a full halo
-  static constexpr int NMAX = (CY * HX + 15) / 16 * 16;            // UMMA N of a full part
+  static constexpr int HY = TY + KY - 1, HX = TX + KX - 1, HALF = HX / 2;
+  static constexpr int G = 32 / TX;                                // query rows (y) per softmax warp
+  static constexpr int NPARTS = 3;                                 // key-row parts of a halo plane
+  static constexpr int RA = G, RB = KY - 1;                        // rows of parts 0 / 2 and of part 1
+  static constexpr int RMAX = RA > RB ? RA : RB;
+  __host__ __device__ static constexpr int part_begin(int p) { return p <= 0 ? 0 : p == 1 ? G : p == 2 ? G + KY - 1 : HY; }
+  static constexpr int NKEYMAX = (RMAX * HX + 15) / 16 * 16;       // UMMA N of the largest part
+  static constexpr int NLD = ((RMAX - 1) * HX + 16 + 15) / 16 * 16;  // columns the 16-wide row loads touch
+  static constexpr int NMAX = NKEYMAX > NLD ? NKEYMAX : NLD;       // columns (= smem rows) of an S buffer / stage
   static constexpr int DSUB = D / 64;                              // 128-byte sub-rows per head row
   static constexpr int SUB_KV = NMAX * 128, SUB_Q = M * 128;       // bytes of one sub-tile
   static constexpr int STAGE_BYTES = DSUB * SUB_KV, Q_BYTES = DSUB * SUB_Q;
@@ -53,12 +63,14 @@ struct FusedCfg {
   static constexpr int NQBUF = (D == 64) ? 2 : 1;                  // Q buffers per slot
   static constexpr int TMEM_SLOT = 256, TMEM_O = 0, TMEM_S = D;
   static constexpr int NBARS = 5 * NSTAGE + 2 * 12 + 1;
-  static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16;
-  static_assert(TL * TY * TX == 128 && (TY * TX) % 32 == 0, "128 queries per tile, one level per warp");
-  static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1 && TX % 2 == 0, "odd windows only (HX even)");
+  static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 512;
+  static constexpr bool FULLFOLD = (KX == HALF);                   // exactly one of the columns c, c + HALF is in the window
+  static_assert(TL * TY * TX == 128 && (TY * TX) % 32 == 0 && TY == 2 * G, "128 queries per tile, one level per warp, two warps per level");
+  static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1 && TX % 2 == 0 && KY >= 3, "odd windows only (HX even)");
+  static_assert(KX <= HALF, "the x fold needs kX <= HX / 2");
   static_assert(TL >= KL - 1, "tiles t and t+2 must reach disjoint planes");
   static_assert(D == 64 || D == 128, "head_dim 64 or 128");
-  static_assert(HX <= 16 && (CY - 1) * HX + 16 <= NMAX, "row loads stay inside the S buffer");
+  static_assert(HX <= 16 && (RMAX - 1) * HX + 16 <= NMAX, "row loads stay inside the S buffer");
   static_assert(D + 2 * NMAX <= TMEM_SLOT, "TMEM columns of a slot");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
@@ -70,9 +82,21 @@ struct FusedParams {
   float scale_log2e;
   int rope;       // 0: no rotation (rope_axes == 0)
   int pairing;    // 0: (2j, 2j+1)   1: (j, j + D/2)
+#ifdef STRATA_TRACE
+  unsigned long long* trace;   // debug: clock64 stamps of one CTA, [event][index]
+  int trace_cta;
+#endif
 };
 
 constexpr int kFusedThreads = 512;
+#ifdef STRATA_TRACE
+#define TRACE(ev, idx)                                                                     \
+  do {                                                                                     \
+    if (p.trace && (int)blockIdx.x == p.trace_cta && (idx) < 256) p.trace[(ev) * 256 + (idx)] = clock64(); \
+  } while (0)
+#else
+#define TRACE(ev, idx) do {} while (0)
+#endif
 constexpr float kBig = 1099511627776.f;   // 2^40: partial row sums above this trigger a new reference maximum
 
 // ------------------------------------------------------------------------------------------------
@@ -147,17 +171,21 @@ __device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem,
 #pragma unroll
     for (int sub = 0; sub < DSUB; ++sub) {
       const uint32_t xb = x_smem + sub * sub_stride, tb = t_smem + sub * sub_stride;
-      for (int idx = tid; idx < n; idx += 256) {
-        const int idx2 = idx + 128;
-        const bool two = idx2 < n;
-        uint4 x0 = lds128(xb + idx * 16), t0 = lds128(tb + idx * 16);
-        uint4 x1 = make_uint4(0, 0, 0, 0), t1 = make_uint4(0, 0, 0, 0);
-        if (two) { x1 = lds128(xb + idx2 * 16); t1 = lds128(tb + idx2 * 16); }
-        x0.x = rot_pair(x0.x, t0.x); x0.y = rot_pair(x0.y, t0.y); x0.z = rot_pair(x0.z, t0.z); x0.w = rot_pair(x0.w, t0.w);
-        sts128(xb + idx * 16, x0);
-        if (two) {
-          x1.x = rot_pair(x1.x, t1.x); x1.y = rot_pair(x1.y, t1.y); x1.z = rot_pair(x1.z, t1.z); x1.w = rot_pair(x1.w, t1.w);
-          sts128(xb + idx2 * 16, x1);
+      for (int base = tid; base < n; base += 512) {       // four chunks per thread in flight
+        uint4 x[4], t[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int idx = base + 128 * u;
+          if (idx < n) { x[u] = lds128(xb + idx * 16); t[u] = lds128(tb + idx * 16); }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int idx = base + 128 * u;
+          if (idx < n) {
+            x[u].x = rot_pair(x[u].x, t[u].x); x[u].y = rot_pair(x[u].y, t[u].y);
+            x[u].z = rot_pair(x[u].z, t[u].z); x[u].w = rot_pair(x[u].w, t[u].w);
+            sts128(xb + idx * 16, x[u]);
+          }
         }
       }
     }
@@ -205,15 +233,47 @@ struct SlotWalk {
   }
 };
 
+// (a & m) | (b & ~m)
+__device__ __forceinline__ uint32_t bitsel(uint32_t m, uint32_t a, uint32_t b) {
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, 0xCA;" : "=r"(d) : "r"(m), "r"(a), "r"(b));
+  return d;
+}
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+}
+__device__ __forceinline__ void tmem_st1(uint32_t taddr, uint32_t r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(r) : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t* r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld1(uint32_t taddr, uint32_t& r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr) : "memory");
+}
+// N (< 8) consecutive words as x4 + x2 + x1 stores
+template <int N> __device__ __forceinline__ void tmem_st_words(uint32_t taddr, const uint32_t* r) {
+  if (N & 4) tmem_st4(taddr, r);
+  if (N & 2) tmem_st2(taddr + (N & 4), r + (N & 4));
+  if (N & 1) tmem_st1(taddr + (N & 6), r[N & 6]);
+}
+
+// flags of one part for one slot, packed in a nibble of the per-CTA schedule table
+constexpr uint32_t kNeeded = 1u, kFirst = 2u, kLast = 4u;
+constexpr int kMaxChunks = 512;
+
 // ------------------------------------------------------------------------------------------------
 // Kernel
 // ------------------------------------------------------------------------------------------------
 template <class C>
 __global__ void __launch_bounds__(kFusedThreads, 1)
-na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                      const __grid_constant__ CUtensorMap tm_kt, const __grid_constant__ CUtensorMap tm_v,
-                      const __grid_constant__ CUtensorMap tm_vt, const __grid_constant__ CUtensorMap tm_tq,
-                      const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tkt,
+na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_ka,
+                      const __grid_constant__ CUtensorMap tm_kb, const __grid_constant__ CUtensorMap tm_va,
+                      const __grid_constant__ CUtensorMap tm_vb, const __grid_constant__ CUtensorMap tm_tq,
+                      const __grid_constant__ CUtensorMap tm_ta, const __grid_constant__ CUtensorMap tm_tb,
                       __nv_bfloat16* __restrict__ o, float* __restrict__ lse, const FusedParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -236,6 +296,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   const uint32_t bar_qtempty = bars + 8u * (5 * C::NSTAGE + 24);
   const uint32_t tmem_word = bars + 8u * C::NBARS;
   uint32_t* tmem_word_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_word - raw));
+  uint8_t* sched = smem_raw + (tmem_word + 16 - raw);                  // [L * nparts] nibble pairs
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -249,16 +310,20 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   const int yl = min(y0 + C::TY, p.Y) - 1;
   const int hs_x = window_start(x0, C::KX, p.X), hs_y = window_start(y0, C::KY, p.Y);
   const int hy = window_start(yl, C::KY, p.Y) + C::KY - hs_y;     // key rows of the halo, <= HY
-  const int nparts = (hy + C::CY - 1) / C::CY;
+  const int nparts = hy > C::part_begin(2) ? 3 : hy > C::part_begin(1) ? 2 : 1;
+  const int nchunks = p.L * nparts;
   const int ntl = (p.L + C::TL - 1) / C::TL;
   const int bl = b * p.L;
   const uint32_t op_tx = p.rope ? 2u : 1u;                        // operand + table bytes per barrier
+  // rows of part `part` that exist in this halo, and the rows its TMA box brings in
+  auto part_rows = [&](int part) { return min(C::part_begin(part + 1), hy) - C::part_begin(part); };
+  auto box_rows = [&](int part) { return part == 1 ? C::RB : C::RA; };
 
   // ---- one-time setup
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_kt);
-    tma_prefetch_desc(&tm_v); tma_prefetch_desc(&tm_vt);
-    if (p.rope) { tma_prefetch_desc(&tm_tq); tma_prefetch_desc(&tm_tk); tma_prefetch_desc(&tm_tkt); }
+    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_ka); tma_prefetch_desc(&tm_kb);
+    tma_prefetch_desc(&tm_va); tma_prefetch_desc(&tm_vb);
+    if (p.rope) { tma_prefetch_desc(&tm_tq); tma_prefetch_desc(&tm_ta); tma_prefetch_desc(&tm_tb); }
     for (int s = 0; s < C::NSTAGE; ++s) {
       mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 128); mbar_init(bar_kempty(s), 2);
       mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 2);
@@ -275,6 +340,20 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     fence_barrier_init();
   }
   if (warp == 3) tmem_alloc(tmem_word, 512);
+  // schedule table: which slot needs part g, and whether it is the first / last part of its tile
+  for (int g = threadIdx.x; g < nchunks; g += kFusedThreads) {
+    const int plane = g / nparts, part = g - plane * nparts;
+    uint32_t e = 0;
+    for (int t = 0; t < ntl; ++t) {
+      const int lo = SlotWalk<C>::plo(t, p.L), hi = SlotWalk<C>::phi(t, p.L);
+      if (plane < lo || plane >= hi) continue;
+      uint32_t f = kNeeded;
+      if (plane == lo && part == 0) f |= kFirst;
+      if (plane == hi - 1 && part == nparts - 1) f |= kLast;
+      e |= f << (4 * (t & 1));
+    }
+    sched[g] = (uint8_t)e;
+  }
   // V stages start as zeros: rows of a stage that a (shorter) part does not overwrite are multiplied
   // by P = 0 in the PV MMA and must therefore hold finite numbers.
   for (uint32_t off = threadIdx.x * 16u; off < (uint32_t)(C::NSTAGE * C::STAGE_BYTES); off += kFusedThreads * 16u)
@@ -290,49 +369,50 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     if (warp == 0) {
       // =========================== TMA producer ===========================
       if (lane == 0) {
-        SlotWalk<C> walk[2] = {{0}, {1}};
-        int g = 0, qjob = 0;
-        for (int plane = 0; plane < p.L; ++plane)
-          for (int part = 0; part < nparts; ++part, ++g) {
+        int nseq[2] = {0, 0};
+        int qjob = 0, part = 0, plane = 0;
+        for (int g = 0; g < nchunks; ++g) {
+          const uint32_t e = sched[g];
 #pragma unroll
-            for (int slot = 0; slot < 2; ++slot) {
-              bool needed, first, last;
-              walk[slot].classify(plane, part, nparts, ntl, p.L, needed, first, last);
-              if (!first) continue;
-              const int nseq = (walk[slot].t - slot) >> 1;           // tiles of this slot so far
-              const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;  // use-th tile in this Q buffer
-              if (use >= 1) mbar_wait(bar_slot(slot, 4 + buf), (uint32_t)(use - 1) & 1u);   // its last QK^T is done
-              if (p.rope && qjob >= 1) mbar_wait(bar_qtempty, (uint32_t)(qjob - 1) & 1u);
-              const uint32_t bar = bar_slot(slot, buf);
-              mbar_expect_tx(bar, op_tx * C::Q_BYTES);
-              const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
-#pragma unroll
-              for (int j = 0; j < C::DSUB; ++j) {
-                tma_load_5d(qb + j * C::SUB_Q, &tm_q, bar, 64 * j, h, x0, y0, bl + C::TL * walk[slot].t);
-                if (p.rope) tma_load_5d(qt_smem + j * C::SUB_Q, &tm_tq, bar, 64 * j, 0, x0, y0, bl + C::TL * walk[slot].t);
-              }
-              ++qjob;
-            }
-            const int s = g % C::NSTAGE;
-            const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
-            const int nrows = min(C::CY, hy - part * C::CY);
-            const bool tail = (C::TAIL < C::CY) && nrows <= C::TAIL;
-            const uint32_t bytes = (uint32_t)((tail ? C::TAIL : C::CY) * C::HX * 128 * C::DSUB);
-            const int cy0 = hs_y + part * C::CY;
-            mbar_wait(bar_kempty(s), ph ^ 1u);
-            mbar_expect_tx(bar_kfull(s), op_tx * bytes);
+          for (int slot = 0; slot < 2; ++slot) {
+            if (!((e >> (4 * slot)) & kFirst)) continue;
+            const int n = nseq[slot]++;                               // tiles of this slot so far
+            const int buf = n % C::NQBUF, use = n / C::NQBUF;         // use-th tile in this Q buffer
+            if (use >= 1) mbar_wait(bar_slot(slot, 4 + buf), (uint32_t)(use - 1) & 1u);   // its last QK^T is done
+            if (p.rope && qjob >= 1) mbar_wait(bar_qtempty, (uint32_t)(qjob - 1) & 1u);
+            const uint32_t bar = bar_slot(slot, buf);
+            mbar_expect_tx(bar, op_tx * C::Q_BYTES);
+            const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
+            const int l0 = bl + C::TL * (slot + 2 * n);
 #pragma unroll
             for (int j = 0; j < C::DSUB; ++j) {
-              tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_kt : &tm_k, bar_kfull(s), 64 * j, h, hs_x, cy0, bl + plane);
-              if (p.rope)
-                tma_load_5d(t_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_tkt : &tm_tk, bar_kfull(s), 64 * j, 0, hs_x, cy0, bl + plane);
+              tma_load_5d(qb + j * C::SUB_Q, &tm_q, bar, 64 * j, h, x0, y0, l0);
+              if (p.rope) tma_load_5d(qt_smem + j * C::SUB_Q, &tm_tq, bar, 64 * j, 0, x0, y0, l0);
             }
-            mbar_wait(bar_vempty(s), ph ^ 1u);
-            mbar_expect_tx(bar_vfull(s), bytes);
-#pragma unroll
-            for (int j = 0; j < C::DSUB; ++j)
-              tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, tail ? &tm_vt : &tm_v, bar_vfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+            ++qjob;
           }
+          const int s = g % C::NSTAGE;
+          const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+          const bool mid = part == 1;
+          const uint32_t bytes = (uint32_t)(box_rows(part) * C::HX * 128 * C::DSUB);
+          const int cy0 = hs_y + C::part_begin(part);
+          mbar_wait(bar_kempty(s), ph ^ 1u);
+          TRACE(0, g);
+          mbar_expect_tx(bar_kfull(s), op_tx * bytes);
+#pragma unroll
+          for (int j = 0; j < C::DSUB; ++j) {
+            tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_kb : &tm_ka, bar_kfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+            if (p.rope)
+              tma_load_5d(t_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_tb : &tm_ta, bar_kfull(s), 64 * j, 0, hs_x, cy0, bl + plane);
+          }
+          mbar_wait(bar_vempty(s), ph ^ 1u);
+          TRACE(1, g);
+          mbar_expect_tx(bar_vfull(s), bytes);
+#pragma unroll
+          for (int j = 0; j < C::DSUB; ++j)
+            tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_vb : &tm_va, bar_vfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+          if (++part == nparts) { part = 0; ++plane; }
+        }
       }
     } else if (warp == 1 || warp == 2) {
       // =========================== MMA issuer of one slot ===========================
@@ -340,103 +420,106 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const int slot = warp - 1;
         const uint32_t tm = tmem + slot * C::TMEM_SLOT;
         constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
-        struct Pending { int i, g, stage, n; uint32_t ph; bool first; };
-        Pending prev{};
-        bool have_prev = false;
-        auto issue_mma2 = [&](const Pending& it) {
-          mbar_wait(bar_slot(slot, 8 + (it.i & 1)), (uint32_t)(it.i >> 1) & 1u);   // P of item i is in TMEM
-          mbar_wait(bar_vfull(it.stage), it.ph);
+        // PV MMA of a pending item: {i, g, n, first}; issued one item late so that QK^T of item i+1 is
+        // already queued on the tensor pipe while the softmax of item i runs
+        int pi = 0, pg = -1, pn = 0;
+        bool pfirst = false;
+        auto issue_mma2 = [&]() {
+          const int stage = pg % C::NSTAGE;
+          mbar_wait(bar_slot(slot, 8 + (pi & 1)), (uint32_t)(pi >> 1) & 1u);   // P of item i is in TMEM
+          TRACE(8 + slot, pg);
+          mbar_wait(bar_vfull(stage), (uint32_t)(pg / C::NSTAGE) & 1u);
           tc_fence_after();
-          const uint32_t a_tmem = tm + C::TMEM_S + (it.i & 1) * C::NMAX;
-          for (int ks = 0; ks < it.n / 16; ++ks) {
+          const uint32_t a_tmem = tm + C::TMEM_S + (pi & 1) * C::NMAX;
+          for (int ks = 0; ks < pn / 16; ++ks) {
 #pragma unroll
             for (int j = 0; j < C::DSUB; ++j) {
-              const uint64_t bd = smem_desc(v_smem + it.stage * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
-              umma_ts(tm + C::TMEM_O + 64 * j, a_tmem + 8 * ks, bd, idesc_pv, (!it.first || ks > 0) ? 1u : 0u);
+              const uint64_t bd = smem_desc(v_smem + stage * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
+              umma_ts(tm + C::TMEM_O + 64 * j, a_tmem + 8 * ks, bd, idesc_pv, (!pfirst || ks > 0) ? 1u : 0u);
             }
           }
-          umma_commit(bar_vempty(it.stage));
-          umma_commit(bar_slot(slot, 10 + (it.i & 1)));
+          umma_commit(bar_vempty(stage));
+          umma_commit(bar_slot(slot, 10 + (pi & 1)));
+          TRACE(10 + slot, pg);
+          pg = -1;
         };
 
-        SlotWalk<C> walk{slot};
-        int i = 0, g = 0;
-        for (int plane = 0; plane < p.L; ++plane)
-          for (int part = 0; part < nparts; ++part, ++g) {
-            bool needed, first, last;
-            walk.classify(plane, part, nparts, ntl, p.L, needed, first, last);
-            const int s = g % C::NSTAGE;
-            const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
-            if (!needed) {       // this slot does not use the part: release it once it is rotated / has landed
-              mbar_wait(bar_krot(s), ph);       // (one arrival per slot and phase, never ahead of the producer)
-              mbar_arrive(bar_kempty(s));
-              mbar_wait(bar_vfull(s), ph);
-              mbar_arrive(bar_vempty(s));
-              continue;
-            }
-            // never hold a V stage across a gap that could stall the producer (deadlock guard)
-            if (have_prev && g - prev.g >= C::NSTAGE - 1) { issue_mma2(prev); have_prev = false; }
-            const int nseq = (walk.t - slot) >> 1;
-            const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;
-            if (first) mbar_wait(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);     // Q tile rotated
-            mbar_wait(bar_krot(s), ph);
-            tc_fence_after();
-            const int nrows = min(C::CY, hy - part * C::CY);
-            const int n = (nrows * C::HX + 15) / 16 * 16;
-            const uint32_t idesc_qk = instr_desc(C::M, n, false);
-            const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
-#pragma unroll
-            for (int ks = 0; ks < C::D / 16; ++ks) {
-              const uint32_t sub = (uint32_t)(ks >> 2), kin = (uint32_t)(ks & 3) * 32u;
-              umma_ss(tm + C::TMEM_S + (i & 1) * C::NMAX, smem_desc(qb + sub * C::SUB_Q + kin),
-                      smem_desc(k_smem + s * C::STAGE_BYTES + sub * C::SUB_KV + kin), idesc_qk, ks > 0 ? 1u : 0u);
-            }
-            umma_commit(bar_kempty(s));
-            umma_commit(bar_slot(slot, 6 + (i & 1)));
-            if (last) umma_commit(bar_slot(slot, 4 + buf));       // every QK^T of the tile is done: Q buffer free
-            if (have_prev) issue_mma2(prev);
-            prev = Pending{i, g, s, n, ph, first};
-            have_prev = true;
-            ++i;
+        int i = 0, nseq = -1, part = 0;
+        for (int g = 0; g < nchunks; ++g) {
+          const uint32_t e = (sched[g] >> (4 * slot)) & 15u;
+          const int s = g % C::NSTAGE;
+          const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+          const int cur_part = part;
+          if (++part == nparts) part = 0;
+          if (!(e & kNeeded)) {       // this slot does not use the part: release it once it is rotated / has landed
+            mbar_wait(bar_krot(s), ph);       // (one arrival per slot and phase, never ahead of the producer)
+            mbar_arrive(bar_kempty(s));
+            mbar_wait(bar_vfull(s), ph);
+            mbar_arrive(bar_vempty(s));
+            continue;
           }
-        if (have_prev) issue_mma2(prev);
+          // never hold a V stage across a gap that could stall the producer (deadlock guard)
+          if (pg >= 0 && g - pg >= C::NSTAGE - 1) issue_mma2();
+          if (e & kFirst) ++nseq;
+          const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;
+          if (e & kFirst) mbar_wait(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);     // Q tile rotated
+          mbar_wait(bar_krot(s), ph);
+          TRACE(4 + slot, g);
+          tc_fence_after();
+          const int n = (part_rows(cur_part) * C::HX + 15) / 16 * 16;
+          const uint32_t idesc_qk = instr_desc(C::M, n, false);
+          const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
+#pragma unroll
+          for (int ks = 0; ks < C::D / 16; ++ks) {
+            const uint32_t sub = (uint32_t)(ks >> 2), kin = (uint32_t)(ks & 3) * 32u;
+            umma_ss(tm + C::TMEM_S + (i & 1) * C::NMAX, smem_desc(qb + sub * C::SUB_Q + kin),
+                    smem_desc(k_smem + s * C::STAGE_BYTES + sub * C::SUB_KV + kin), idesc_qk, ks > 0 ? 1u : 0u);
+          }
+          umma_commit(bar_kempty(s));
+          umma_commit(bar_slot(slot, 6 + (i & 1)));
+          TRACE(6 + slot, g);
+          if (e & kLast) umma_commit(bar_slot(slot, 4 + buf));      // every QK^T of the tile is done: Q buffer free
+          if (pg >= 0) issue_mma2();
+          pi = i; pg = g; pn = n; pfirst = (e & kFirst) != 0;
+          ++i;
+        }
+        if (pg >= 0) issue_mma2();
       }
     }
   } else if (warp < 8) {
     // =========================== rotation warpgroup ===========================
     reg_dec<88>();
     const int tid = threadIdx.x - 128;
-    SlotWalk<C> walk[2] = {{0}, {1}};
-    int g = 0;
-    for (int plane = 0; plane < p.L; ++plane)
-      for (int part = 0; part < nparts; ++part, ++g) {
+    int nseq[2] = {0, 0};
+    int part = 0;
+    for (int g = 0; g < nchunks; ++g) {
+      const uint32_t e = sched[g];
 #pragma unroll
-        for (int slot = 0; slot < 2; ++slot) {
-          bool needed, first, last;
-          walk[slot].classify(plane, part, nparts, ntl, p.L, needed, first, last);
-          if (!first) continue;
-          const int nseq = (walk[slot].t - slot) >> 1;
-          const int buf = nseq % C::NQBUF, use = nseq / C::NQBUF;
-          mbar_wait(bar_slot(slot, buf), (uint32_t)use & 1u);                      // Q tile (+ table) landed
-          if (p.rope) {
-            rotate_inplace<C::DSUB>(q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES, qt_smem, C::SUB_Q, C::M, p.pairing, tid);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_arrive(bar_qtempty);
-          }
-          mbar_arrive(bar_slot(slot, 2 + buf));
-        }
-        const int s = g % C::NSTAGE;
-        const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
-        mbar_wait(bar_kfull(s), ph);
+      for (int slot = 0; slot < 2; ++slot) {
+        if (!((e >> (4 * slot)) & kFirst)) continue;
+        const int n = nseq[slot]++;
+        const int buf = n % C::NQBUF, use = n / C::NQBUF;
+        mbar_wait(bar_slot(slot, buf), (uint32_t)use & 1u);                      // Q tile (+ table) landed
         if (p.rope) {
-          const int nrows = min(C::CY, hy - part * C::CY);
-          const bool tail = (C::TAIL < C::CY) && nrows <= C::TAIL;
-          rotate_inplace<C::DSUB>(k_smem + s * C::STAGE_BYTES, t_smem + s * C::STAGE_BYTES, C::SUB_KV,
-                                  (tail ? C::TAIL : C::CY) * C::HX, p.pairing, tid);
+          rotate_inplace<C::DSUB>(q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES, qt_smem, C::SUB_Q, C::M, p.pairing, tid);
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_arrive(bar_qtempty);
         }
-        mbar_arrive(bar_krot(s));
+        mbar_arrive(bar_slot(slot, 2 + buf));
       }
+      const int s = g % C::NSTAGE;
+      const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+      mbar_wait(bar_kfull(s), ph);
+      if (tid == 0) TRACE(2, g);
+      if (p.rope) {
+        rotate_inplace<C::DSUB>(k_smem + s * C::STAGE_BYTES, t_smem + s * C::STAGE_BYTES, C::SUB_KV,
+                                box_rows(part) * C::HX, p.pairing, tid);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      }
+      if (tid == 0) TRACE(3, g);
+      mbar_arrive(bar_krot(s));
+      if (++part == nparts) part = 0;
+    }
   } else {
     // =========================== softmax + epilogue of one slot ===========================
     reg_inc<184>();
@@ -451,7 +534,16 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int lo_y = window_start(ay, C::KY, p.Y) - hs_y;
     const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
     const float cs = p.scale_log2e;
-    float xb[C::HX];                               // column bias: -m_ref inside the x window, -inf outside
+    // x fold: of the halo columns c and c + HALF at most one lies in this query's window
+    uint32_t m_lo[C::HALF], m_hi[C::HALF];
+    float xz[C::HALF];                             // 0 if one of the two is in the window, else -inf
+#pragma unroll
+    for (int c = 0; c < C::HALF; ++c) {
+      const bool in_lo = c >= lo_x && c < lo_x + C::KX, in_hi = c + C::HALF >= lo_x && c + C::HALF < lo_x + C::KX;
+      m_lo[c] = in_lo ? 0xffffffffu : 0u;
+      m_hi[c] = in_hi ? 0xffffffffu : 0u;
+      xz[c] = (in_lo || in_hi) ? 0.f : -INFINITY;
+    }
 
     int i = 0;
     for (int tile = slot; tile < ntl; tile += 2) {
@@ -461,68 +553,39 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       const int wl_lo = __reduce_min_sync(0xffffffffu, pw_lo), wl_hi = __reduce_max_sync(0xffffffffu, pw_lo + C::KL);
       float m_ref = 0.f, lsum = 0.f;
       bool inited = false;
-#pragma unroll
-      for (int j = 0; j < C::HX; ++j) xb[j] = (j >= lo_x && j < lo_x + C::KX) ? 0.f : -INFINITY;
       const int plo = SlotWalk<C>::plo(tile, p.L), phi = SlotWalk<C>::phi(tile, p.L);
       for (int plane = plo; plane < phi; ++plane) {
         const bool plane_needed = plane >= wl_lo && plane < wl_hi;
         const bool plane_ok = plane >= pw_lo && plane < pw_lo + C::KL;
         for (int part = 0; part < nparts; ++part, ++i) {
-          const int r_base = part * C::CY;
-          const int nrows = min(C::CY, hy - r_base);
+          const int pb = C::part_begin(part);
+          const int nrows = part_rows(part);
           const int nwords = ((nrows * C::HX + 15) / 16 * 16) / 2;
           const uint32_t s_addr = tm + C::TMEM_S + (i & 1) * C::NMAX;
           const bool first_item = (plane == plo && part == 0);
-          // rows of this part that some query of the warp needs: [ra, rb)
-          const int ra = plane_needed ? max(0, wy_lo - r_base) : 0;
-          const int rb = plane_needed ? min(nrows, wy_hi - r_base) : 0;
-          const bool has_valid = plane_ok && lo_y < r_base + nrows && lo_y + C::KY > r_base;
+          // rows of this part some query of the warp needs: [ra, rb) (warp-uniform)
+          const int ra = plane_needed ? max(0, wy_lo - pb) : 0;
+          const int rb = plane_needed ? min(nrows, wy_hi - pb) : 0;
+          // rows of this part inside this query's window: [ya, yb)
+          const int ya = plane_ok ? max(0, lo_y - pb) : 0;
+          const int yb = plane_ok ? min(nrows, lo_y + C::KY - pb) : 0;
           mbar_wait(bar_slot(slot, 6 + (i & 1)), (uint32_t)(i >> 1) & 1u);
+          if (sp == 0 && lane == 0) TRACE(12 + slot, i);
           tc_fence_after();
 
-          // rolling double-buffered walk over the needed rows of S
-          auto for_rows = [&](auto&& body) {
-            uint32_t sva[16], svb[16];
-            if (0 >= ra && 0 < rb) ld16_issue(s_addr, sva);
+          // folded logits of key row r (already waited for) -> v[0 .. HALF)
+          auto fold = [&](const uint32_t (&sv)[16], float (&v)[C::HALF]) {
 #pragma unroll
-            for (int r = 0; r < C::CY; ++r) {
-              uint32_t (&cur)[16] = (r & 1) ? svb : sva;
-              uint32_t (&nxt)[16] = (r & 1) ? sva : svb;
-              const bool need_r = r >= ra && r < rb;
-              if (need_r) ld16_wait(cur);
-              if (r + 1 < C::CY && r + 1 >= ra && r + 1 < rb) ld16_issue(s_addr + (r + 1) * C::HX, nxt);
-              body(r, need_r, cur);
-            }
+            for (int c = 0; c < C::HALF; ++c) v[c] = __uint_as_float(bitsel(m_lo[c], sv[c], sv[c + C::HALF]));
           };
-
-          uint32_t pw[C::NMAX / 2];
-          float csum = 0.f;
-          bool fix = __any_sync(0xffffffffu, has_valid && !inited);
-          while (true) {
-            if (fix) {
-              // ---- slow path: true maximum of the valid logits of this part -> new reference maximum
-              float cmax = -INFINITY;
-              for_rows([&](int r, bool need_r, uint32_t (&sv)[16]) {
-                if (need_r) {
-                  const int py = r_base + r;
-                  const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
-                  float rmax = -INFINITY;
-#pragma unroll
-                  for (int j = 0; j < C::HX; ++j) {
-                    const float t = (j >= lo_x && j < lo_x + C::KX) ? __uint_as_float(sv[j]) * cs : -INFINITY;
-                    rmax = fmaxf(rmax, t);
-                  }
-                  if (rowok) cmax = fmaxf(cmax, rmax);
-                }
-              });
-              const bool got = cmax > -INFINITY;
-              const float new_ref = got ? (inited ? fmaxf(m_ref, cmax) : cmax) : m_ref;
-              const float alpha = (inited && new_ref != m_ref) ? ex2(m_ref - new_ref) : 1.f;
-              if (!first_item && __any_sync(0xffffffffu, alpha != 1.f)) {
+          // new reference maximum m_new >= m_ref for this row: rescale what was accumulated so far
+          auto rescale = [&](float new_ref, int rows_done_from, int rows_done_to) {
+            const float alpha = (inited && new_ref != m_ref) ? ex2(m_ref - new_ref) : 1.f;
+            if (__any_sync(0xffffffffu, alpha != 1.f)) {
+              if (!first_item) {
                 // O holds earlier parts of this tile: rescale its rows (all its PV MMAs are complete)
                 mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
                 tc_fence_after();
-#pragma unroll
                 for (int j = 0; j < C::D; j += 16) {
                   float ov[16];
                   tmem_ld16(tm + C::TMEM_O + j, ov);
@@ -532,49 +595,118 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                   for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
                   tmem_st16(tm + C::TMEM_O + j, ow);
                 }
-                tmem_wait_st();
               }
-              lsum *= alpha;
-              m_ref = new_ref;
-              inited = inited || got;
-#pragma unroll
-              for (int j = 0; j < C::HX; ++j) xb[j] = (j >= lo_x && j < lo_x + C::KX) ? -m_ref : -INFINITY;
-            }
-            // ---- fast path: p = 2^(s * cs - m_ref), masked by the additive biases
-            float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-            for_rows([&](int r, bool need_r, uint32_t (&sv)[16]) {
-              if (need_r) {
-                const int py = r_base + r;
-                const float rbias = (plane_ok && py >= lo_y && py < lo_y + C::KY) ? 0.f : -INFINITY;
-#pragma unroll
-                for (int j = 0; j < C::HX; j += 2) {
-                  float t0, t1;
-                  ffma2(t0, t1, __uint_as_float(sv[j]), __uint_as_float(sv[j + 1]), cs, xb[j], xb[j + 1]);
-                  fadd2(t0, t1, t0, t1, rbias, rbias);
-                  const float p0 = ex2(t0), p1 = ex2(t1);
-                  if ((j >> 1) & 1) fadd2(a2, a3, a2, a3, p0, p1);
-                  else fadd2(a0, a1, a0, a1, p0, p1);
-                  pw[(r * C::HX + j) >> 1] = pack_bf16(p0, p1);
+              // P rows of this part that are already stored with the old reference
+              tmem_wait_st();
+              for (int r = rows_done_from; r < rows_done_to; ++r)
+                for (int j = 0; j < C::HALF; ++j) {
+                  uint32_t w;
+                  tmem_ld1(s_addr + r * C::HALF + j, w);
+                  tmem_wait_ld();
+                  w = pack_bf16(__uint_as_float(w << 16) * alpha, __uint_as_float(w & 0xffff0000u) * alpha);
+                  tmem_st1(s_addr + r * C::HALF + j, w);
                 }
-              } else {
+              tmem_wait_st();
+            }
+            lsum *= alpha;
+            m_ref = new_ref;
+          };
+
+          float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;            // partial sums of this part (times 2^-m_ref)
+          if (ra < rb) {
+            if (__any_sync(0xffffffffu, ya < yb && !inited)) {
+              // ---- first valid keys of some query: reference maximum = true maximum of this part
+              float cmax = -INFINITY;
+              for (int r = ra; r < rb; ++r) {
+                uint32_t sv[16];
+                ld16_issue(s_addr + r * C::HX, sv);
+                ld16_wait(sv);
+                float v[C::HALF];
+                fold(sv, v);
+                float rmax = -INFINITY;
 #pragma unroll
-                for (int j = 0; j < C::HX; j += 2) pw[(r * C::HX + j) >> 1] = 0u;
+                for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[c] * cs : v[c] * cs + xz[c]);
+                if (r >= ya && r < yb) cmax = fmaxf(cmax, rmax);
               }
-            });
-            csum = (a0 + a1) + (a2 + a3);
-            if (fix) break;                                  // every valid p <= 1 after a fix
-            fix = __any_sync(0xffffffffu, !(csum <= kBig));
-            if (!fix) break;
+              const bool got = cmax > -INFINITY;
+              rescale(got ? (inited ? fmaxf(m_ref, cmax) : cmax) : m_ref, 0, 0);
+              inited = inited || got;
+            }
+            // ---- p = 2^(s * cs - m_ref) on the folded rows, two rows per iteration
+            for (int r0 = ra; r0 < rb; r0 += 2) {
+              uint32_t sva[16], svb[16];
+              const bool two = r0 + 1 < rb;
+              ld16_issue(s_addr + r0 * C::HX, sva);
+              if (two) ld16_issue(s_addr + (r0 + 1) * C::HX, svb);
+              ld16_wait(sva);
+              if (two) ld16_wait(svb);
+#pragma unroll
+              for (int u = 0; u < 2; ++u) {
+                if (u == 1 && !two) break;
+                const int r = r0 + u;
+                float v[C::HALF], pv[C::HALF];
+                fold(u ? svb : sva, v);
+                float br = (r >= ya && r < yb) ? -m_ref : -INFINITY;
+                auto expo = [&]() {
+                  float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
+#pragma unroll
+                  for (int c = 0; c < C::HALF; c += 2) {
+                    if (c + 1 < C::HALF) {
+                      float t0, t1;
+                      if (C::FULLFOLD) ffma2(t0, t1, v[c], v[c + 1], cs, br, br);
+                      else ffma2(t0, t1, v[c], v[c + 1], cs, br + xz[c], br + xz[c + 1]);
+                      pv[c] = ex2(t0); pv[c + 1] = ex2(t1);
+                      if ((c >> 1) & 1) fadd2(e2, e3, e2, e3, pv[c], pv[c + 1]);
+                      else fadd2(e0, e1, e0, e1, pv[c], pv[c + 1]);
+                    } else {
+                      pv[c] = ex2(fmaf(v[c], cs, C::FULLFOLD ? br : br + xz[c]));
+                      e0 += pv[c];
+                    }
+                  }
+                  return (e0 + e1) + (e2 + e3);
+                };
+                float rs = expo();
+                if (__any_sync(0xffffffffu, !(rs <= kBig))) {
+                  // ---- a logit far above the reference: move the reference to this row's maximum
+                  float rmax = -INFINITY;
+#pragma unroll
+                  for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[c] * cs : v[c] * cs + xz[c]);
+                  const bool mine = !(rs <= kBig);
+                  const float part_sum = (a0 + a1) + (a2 + a3);
+                  const float old_ref = m_ref;
+                  rescale(mine ? fmaxf(m_ref, rmax) : m_ref, ra, r);
+                  const float al2 = ex2(old_ref - m_ref);
+                  a0 = part_sum * al2; a1 = 0.f; a2 = 0.f; a3 = 0.f;
+                  br = (r >= ya && r < yb) ? -m_ref : -INFINITY;
+                  rs = expo();
+                }
+                a0 += rs;
+                // un-fold: slot k < HALF takes p[k] if column k is the valid one, slot k + HALF otherwise
+                uint32_t pw[C::HALF];
+#pragma unroll
+                for (int j = 0; j < C::HALF; ++j) {
+                  const int k0 = 2 * j, k1 = 2 * j + 1;
+                  const uint32_t s0 = k0 < C::HALF ? (__float_as_uint(pv[k0]) & m_lo[k0]) : (__float_as_uint(pv[k0 - C::HALF]) & m_hi[k0 - C::HALF]);
+                  const uint32_t s1 = k1 < C::HALF ? (__float_as_uint(pv[k1]) & m_lo[k1]) : (__float_as_uint(pv[k1 - C::HALF]) & m_hi[k1 - C::HALF]);
+                  pw[j] = pack_bf16(__uint_as_float(s0), __uint_as_float(s1));
+                }
+                tmem_st_words<C::HALF>(s_addr + r * C::HALF, pw);
+              }
+            }
+            lsum += (a0 + a1) + (a2 + a3);
+            // rows outside [ra, rb) and the pad keys are zero in P (stored last: P overlays S)
+            for (int j = 0; j < ra * C::HALF; ++j) tmem_st1(s_addr + j, 0u);
+            for (int j = rb * C::HALF; j < nwords; ++j) tmem_st1(s_addr + j, 0u);
+          } else {
+            // no query of this warp attends a key of this part: P = 0
+            uint32_t z[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) z[u] = 0u;
+            for (int j = 0; j < nwords; j += 8) tmem_st8(s_addr + j, z);
           }
-          lsum += csum;
-#pragma unroll
-          for (int j = C::CY * C::HX / 2; j < C::NMAX / 2; ++j) pw[j] = 0u;    // pad keys of a full part
-          // P (bf16 pairs) over the front of the S buffer, then hand the item to the PV MMA
-#pragma unroll
-          for (int j = 0; j < C::NMAX / 2; j += 8)
-            if (j < nwords) tmem_st8(s_addr + j, &pw[j]);
           tmem_wait_st();
           tc_fence_before();
+          if (sp == 0 && lane == 0) TRACE(14 + slot, i);
           mbar_arrive(bar_slot(slot, 8 + (i & 1)));
         }
       }
@@ -584,7 +716,6 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       const float inv = 1.f / lsum;
       const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
       __nv_bfloat16* orow = o + (((long long)b * p.N + tok) * p.H + h) * C::D;
-#pragma unroll
       for (int j = 0; j < C::D; j += 16) {
         float ov[16];
         tmem_ld16(tm + C::TMEM_O + j, ov);
@@ -621,6 +752,7 @@ template <class C>
 bool fused_shape_ok(const Problem& p) {
   // the tiles of one slot must reach disjoint, increasing plane ranges (one pass over the levels)
   const int ntl = (p.L + C::TL - 1) / C::TL;
+  if (p.L * C::NPARTS > kMaxChunks) return false;                    // per-CTA schedule table
   for (int t = 0; t + 2 < ntl; ++t)
     if (SlotWalk<C>::plo(t + 2, p.L) < SlotWalk<C>::phi(t, p.L)) return false;
   return true;
@@ -629,20 +761,20 @@ bool fused_shape_ok(const Problem& p) {
 template <class C>
 cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table, void* o,
                          float* lse, cudaStream_t stream, int* launches) {
-  CUtensorMap tq, tk, tkt, tv, tvt, ttq, ttk, ttkt;
-  if (!make_map(&tq, q, p, C::TX, C::TY, C::TL) || !make_map(&tk, k, p, C::HX, C::CY, 1) ||
-      !make_map(&tkt, k, p, C::HX, C::TAIL, 1) || !make_map(&tv, v, p, C::HX, C::CY, 1) ||
-      !make_map(&tvt, v, p, C::HX, C::TAIL, 1))
+  CUtensorMap tq, tka, tkb, tva, tvb, ttq, tta, ttb;
+  if (!make_map(&tq, q, p, C::TX, C::TY, C::TL) || !make_map(&tka, k, p, C::HX, C::RA, 1) ||
+      !make_map(&tkb, k, p, C::HX, C::RB, 1) || !make_map(&tva, v, p, C::HX, C::RA, 1) ||
+      !make_map(&tvb, v, p, C::HX, C::RB, 1))
     return cudaErrorInvalidValue;
   const bool rope = p.A > 0;
   if (rope) {
     Problem pt = p;
     pt.H = 1;                                  // the table is [B, L, Y, X, D] 16-bit words: one "head"
-    if (!make_map(&ttq, table, pt, C::TX, C::TY, C::TL) || !make_map(&ttk, table, pt, C::HX, C::CY, 1) ||
-        !make_map(&ttkt, table, pt, C::HX, C::TAIL, 1))
+    if (!make_map(&ttq, table, pt, C::TX, C::TY, C::TL) || !make_map(&tta, table, pt, C::HX, C::RA, 1) ||
+        !make_map(&ttb, table, pt, C::HX, C::RB, 1))
       return cudaErrorInvalidValue;
   } else {
-    ttq = tq; ttk = tk; ttkt = tkt;            // never dereferenced
+    ttq = tq; tta = tka; ttb = tkb;            // never dereferenced
   }
   FusedParams fp;
   fp.B = p.B; fp.H = p.H; fp.L = p.L; fp.Y = p.Y; fp.X = p.X; fp.N = p.N;
@@ -650,6 +782,14 @@ cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const v
   fp.scale_log2e = p.scale * 1.4426950408889634f;
   fp.rope = rope ? 1 : 0;
   fp.pairing = p.pairing;
+#ifdef STRATA_TRACE
+  {
+    const char* e = getenv("STRATA_TRACE_PTR");
+    fp.trace = e ? (unsigned long long*)strtoull(e, nullptr, 0) : nullptr;
+    const char* c = getenv("STRATA_TRACE_CTA");
+    fp.trace_cta = c ? atoi(c) : 0;
+  }
+#endif
   const long long grid = (long long)p.B * p.H * fp.nty * fp.ntx;
   if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
   static bool attr_set = false;
@@ -660,7 +800,7 @@ cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const v
   }
   prof_begin("na3d_fwd_fused", stream);
   na3d_fwd_fused_kernel<C><<<(unsigned)grid, kFusedThreads, C::SMEM_BYTES, stream>>>(
-      tq, tk, tkt, tv, tvt, ttq, ttk, ttkt, (__nv_bfloat16*)o, lse, fp);
+      tq, tka, tkb, tva, tvb, ttq, tta, ttb, (__nv_bfloat16*)o, lse, fp);
   prof_end(stream);
   if (launches) ++*launches;
   return cudaGetLastError();
@@ -668,17 +808,17 @@ cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const v
 
 }  // namespace
 
-// (D, kL, kY, kX, TL, TY, TX, CY, NSTAGE) instantiations.
+// (D, kL, kY, kX, TL, TY, TX, NSTAGE) instantiations.
 #define STRATA_FUSED_CONFIGS(X) \
-  X(64, 3, 7, 7, 2, 8, 8, 5, 4) \
-  X(64, 3, 5, 5, 2, 8, 8, 6, 4) \
-  X(64, 3, 3, 3, 2, 8, 8, 5, 4)
+  X(64, 3, 7, 7, 2, 8, 8, 4)    \
+  X(64, 3, 5, 5, 2, 8, 8, 4)    \
+  X(64, 3, 3, 3, 2, 8, 8, 4)
 
 bool fused_fwd_supported(const Problem& p) {
   if (p.dtype != 1) return false;
-#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_)                   \
+#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, NS_)                        \
   if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)          \
-    return fused_shape_ok<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_>>(p);
+    return fused_shape_ok<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, NS_>>(p);
   STRATA_FUSED_CONFIGS(X)
 #undef X
   return false;
@@ -686,9 +826,9 @@ bool fused_fwd_supported(const Problem& p) {
 
 cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
                              void* o, float* lse, cudaStream_t stream, int* launches) {
-#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_)                   \
+#define X(D_, KL_, KY_, KX_, TL_, TY_, TX_, NS_)                        \
   if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)          \
-    return launch_fused<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, CY_, NS_>>(p, q, k, v, table, o, lse, stream, launches);
+    return launch_fused<FusedCfg<D_, KL_, KY_, KX_, TL_, TY_, TX_, NS_>>(p, q, k, v, table, o, lse, stream, launches);
   STRATA_FUSED_CONFIGS(X)
 #undef X
   return cudaErrorNotSupported;
