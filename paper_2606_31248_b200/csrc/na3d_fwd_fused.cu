@@ -22,17 +22,21 @@
 //   1, 2   MMA issuer of slot 0 / 1
 //   3      TMEM owner
 //   4-7    rotation warpgroup: rotates every K part and every Q tile IN PLACE in shared memory
-//          (fp32 math on bf16 pairs, cos/sin from the fp16 table), then hands them to the MMA issuers
+//          (packed bf16x2 multiply-adds against the bf16 cos/sin table), then hands them to the MMA
+//          issuers.  For the interleaved pairing the two halves of a pair are first gathered into
+//          separate words and the rotated words are stored in that order: the same permutation of
+//          the 8 channels of every 16-byte chunk is applied to Q and K, which leaves Q K^T unchanged.
 //   8-11   softmax + epilogue of slot 0        12-15   softmax + epilogue of slot 1
 // Register budget via setmaxnreg: 56 / 88 / 184 / 184 per thread for the four warpgroups.
 //
-// Softmax: exp2 with a LAZY reference maximum -- the row maximum is computed only for the first
-// part that holds a valid key of the row and when a partial sum overflows 2^40.  The x window of a
-// query covers kX of the HX halo columns; with kX <= HX/2 at most one of the columns c and c + HX/2
-// is inside it, so the two halves of every key row are FOLDED with a per-thread bit select before
-// the exponential (half the MUFU work) and un-folded again when P is packed to bf16.
-#include <cuda_fp16.h>
-
+// Softmax: a thread (= query row) takes the whole S part (R key rows x HX columns) into registers with
+// one batch of tcgen05.ld, and everything up to the P store is branch-free.  exp2 with a LAZY
+// reference maximum -- the row maximum is computed only for the first part that holds a valid key
+// of the row and when the part's sum overflows 2^40 (checked once per part, before P is stored).
+// The x window of a query covers kX of the HX halo columns; with kX <= HX/2 at most one of the
+// columns c and c + HX/2 is inside it, so the two halves of every key row are FOLDED with a
+// per-thread bit select before the exponential (half the MUFU work); P is packed to bf16 folded and
+// un-folded by one byte permute per output word (a masked slot replicates the zero sign bit).
 #include <cstdlib>
 #include <type_traits>
 
@@ -53,9 +57,10 @@ struct FusedCfg {
   static constexpr int RA = G, RB = KY - 1;                        // rows of parts 0 / 2 and of part 1
   static constexpr int RMAX = RA > RB ? RA : RB;
   __host__ __device__ static constexpr int part_begin(int p) { return p <= 0 ? 0 : p == 1 ? G : p == 2 ? G + KY - 1 : HY; }
-  static constexpr int NKEYMAX = (RMAX * HX + 15) / 16 * 16;       // UMMA N of the largest part
-  static constexpr int NLD = ((RMAX - 1) * HX + 16 + 15) / 16 * 16;  // columns the 16-wide row loads touch
-  static constexpr int NMAX = NKEYMAX > NLD ? NKEYMAX : NLD;       // columns (= smem rows) of an S buffer / stage
+  static constexpr int NA = (RA * HX + 15) / 16 * 16;              // UMMA N of parts 0 / 2 (whole TMA box)
+  static constexpr int NB = (RB * HX + 15) / 16 * 16;              // UMMA N of part 1
+  static constexpr int NMAX = NA > NB ? NA : NB;                   // columns (= smem rows) of an S buffer / stage
+  static constexpr int NF = (HALF + 1) / 2;                        // packed folded P words per key row
   static constexpr int DSUB = D / 64;                              // 128-byte sub-rows per head row
   static constexpr int SUB_KV = NMAX * 128, SUB_Q = M * 128;       // bytes of one sub-tile
   static constexpr int STAGE_BYTES = DSUB * SUB_KV, Q_BYTES = DSUB * SUB_Q;
@@ -70,7 +75,7 @@ struct FusedCfg {
   static_assert(KX <= HALF, "the x fold needs kX <= HX / 2");
   static_assert(TL >= KL - 1, "tiles t and t+2 must reach disjoint planes");
   static_assert(D == 64 || D == 128, "head_dim 64 or 128");
-  static_assert(HX <= 16 && (RMAX - 1) * HX + 16 <= NMAX, "row loads stay inside the S buffer");
+  static_assert(HX <= 16, "halo row of at most 16 keys");
   static_assert(D + 2 * NMAX <= TMEM_SLOT, "TMEM columns of a slot");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
@@ -142,26 +147,41 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
-// A2 on one (a, b) bf16 pair held in `w` (a = low half) with (cos, sin) as a half2 in `t`.
-__device__ __forceinline__ uint32_t rot_pair(uint32_t w, uint32_t t) {
-  const float a = __uint_as_float(w << 16), b = __uint_as_float(w & 0xffff0000u);
-  const float2 cs = __half22float2(*reinterpret_cast<const __half2*>(&t));
-  return pack_bf16(fmaf(a, cs.x, -b * cs.y), fmaf(a, cs.y, b * cs.x));
+// ---- A2 in packed bf16x2 arithmetic.  Table words (rope.cu): C = (cos m, cos m+1), S = (sin m, sin m+1).
+__device__ __forceinline__ uint32_t bmul2(uint32_t a, uint32_t b) {
+  uint32_t d;
+  asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+  return d;
 }
-// HALF pairing: `wa` holds channels (j, j+1), `wb` channels (j + D/2, j + 1 + D/2); t0 / t1 the (cos, sin) of pairs j / j+1.
-__device__ __forceinline__ void rot_half(uint32_t& wa, uint32_t& wb, uint32_t t0, uint32_t t1) {
-  const float a0 = __uint_as_float(wa << 16), a1 = __uint_as_float(wa & 0xffff0000u);
-  const float b0 = __uint_as_float(wb << 16), b1 = __uint_as_float(wb & 0xffff0000u);
-  const float2 c0 = __half22float2(*reinterpret_cast<const __half2*>(&t0));
-  const float2 c1 = __half22float2(*reinterpret_cast<const __half2*>(&t1));
-  wa = pack_bf16(fmaf(a0, c0.x, -b0 * c0.y), fmaf(a1, c1.x, -b1 * c1.y));
-  wb = pack_bf16(fmaf(a0, c0.y, b0 * c0.x), fmaf(a1, c1.y, b1 * c1.x));
+__device__ __forceinline__ uint32_t bfma2(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t d;
+  asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+  uint32_t d;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+  return d;
+}
+// (a, b) -> (a cos - b sin, a sin + b cos) on two pairs at once: A = (a_m, a_m+1), B = (b_m, b_m+1).
+__device__ __forceinline__ void rot2(uint32_t& A, uint32_t& B, uint32_t C, uint32_t S) {
+  const uint32_t nB = B ^ 0x80008000u;
+  const uint32_t ra = bfma2(nB, S, bmul2(A, C));
+  const uint32_t rb = bfma2(A, S, bmul2(B, C));
+  A = ra; B = rb;
+}
+// Interleaved pairing: w0 = (a_m, b_m), w1 = (a_m+1, b_m+1).  The rotated pairs are left gathered,
+// w0 = (a'_m, a'_m+1), w1 = (b'_m, b'_m+1): the same channel permutation for Q and K (see the header).
+__device__ __forceinline__ void rot_interleaved(uint32_t& w0, uint32_t& w1, uint32_t C, uint32_t S) {
+  uint32_t A = prmt(w0, w1, 0x5410u), B = prmt(w0, w1, 0x7632u);
+  rot2(A, B, C, S);
+  w0 = A; w1 = B;
 }
 
 // Rotate `rows` head rows in place.  x_smem / t_smem: operand tile and its table tile, both in the
 // TMA 128-byte-swizzled layout [sub][row][128 B] with `sub_stride` bytes between sub-tiles.  The
 // table tile has the operand's geometry (same box), so for the interleaved pairing the 16-byte
-// chunk at a physical offset of one holds the four (cos, sin) of the four pairs at that offset of
+// chunk at a physical offset of one holds the (C, S, C, S) words of the four pairs at that offset of
 // the other: the loop is linear over physical chunks.  128 threads, tid in [0, 128).
 template <int DSUB>
 __device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem, uint32_t sub_stride, int rows,
@@ -182,8 +202,8 @@ __device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem,
         for (int u = 0; u < 4; ++u) {
           const int idx = base + 128 * u;
           if (idx < n) {
-            x[u].x = rot_pair(x[u].x, t[u].x); x[u].y = rot_pair(x[u].y, t[u].y);
-            x[u].z = rot_pair(x[u].z, t[u].z); x[u].w = rot_pair(x[u].w, t[u].w);
+            rot_interleaved(x[u].x, x[u].y, t[u].x, t[u].y);
+            rot_interleaved(x[u].z, x[u].w, t[u].z, t[u].w);
             sts128(xb + idx * 16, x[u]);
           }
         }
@@ -208,8 +228,8 @@ __device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem,
       const uint32_t t0_addr = t_smem + (uint32_t)(q0 >> 3) * sub_stride + rowoff + (((uint32_t)(q0 & 7) ^ sw) << 4);
       const uint32_t t1_addr = t_smem + (uint32_t)(q1 >> 3) * sub_stride + rowoff + (((uint32_t)(q1 & 7) ^ sw) << 4);
       uint4 xa = lds128(a_addr), xbv = lds128(b_addr), t0 = lds128(t0_addr), t1 = lds128(t1_addr);
-      rot_half(xa.x, xbv.x, t0.x, t0.y); rot_half(xa.y, xbv.y, t0.z, t0.w);
-      rot_half(xa.z, xbv.z, t1.x, t1.y); rot_half(xa.w, xbv.w, t1.z, t1.w);
+      rot2(xa.x, xbv.x, t0.x, t0.y); rot2(xa.y, xbv.y, t0.z, t0.w);
+      rot2(xa.z, xbv.z, t1.x, t1.y); rot2(xa.w, xbv.w, t1.z, t1.w);
       sts128(a_addr, xa); sts128(b_addr, xbv);
     }
   }
@@ -300,12 +320,13 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-  // ---- the level column of this CTA: x fastest, then y, head, sample
+  // ---- the level column of this CTA: head fastest (the H heads of a token are one contiguous
+  // H*D*2-byte run in HBM), then x, y, sample
   int bid = blockIdx.x;
+  const int h = bid % p.H; bid /= p.H;
   const int tx = bid % p.ntx; bid /= p.ntx;
-  const int ty = bid % p.nty; bid /= p.nty;
-  const int h = bid % p.H;
-  const int b = bid / p.H;
+  const int ty = bid % p.nty;
+  const int b = bid / p.nty;
   const int x0 = tx * C::TX, y0 = ty * C::TY;
   const int yl = min(y0 + C::TY, p.Y) - 1;
   const int hs_x = window_start(x0, C::KX, p.X), hs_y = window_start(y0, C::KY, p.Y);
@@ -466,8 +487,8 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           mbar_wait(bar_krot(s), ph);
           TRACE(4 + slot, g);
           tc_fence_after();
-          const int n = (part_rows(cur_part) * C::HX + 15) / 16 * 16;
-          const uint32_t idesc_qk = instr_desc(C::M, n, false);
+          const int n = cur_part == 1 ? C::NB : C::NA;           // the whole TMA box (rows past the halo are zeros)
+          const uint32_t idesc_qk = cur_part == 1 ? instr_desc(C::M, C::NB, false) : instr_desc(C::M, C::NA, false);
           const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
 #pragma unroll
           for (int ks = 0; ks < C::D / 16; ++ks) {
@@ -535,14 +556,27 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
     const float cs = p.scale_log2e;
     // x fold: of the halo columns c and c + HALF at most one lies in this query's window
-    uint32_t m_lo[C::HALF], m_hi[C::HALF];
+    uint32_t m_lo[C::HALF];                        // all ones: column c is the one (else c + HALF, or neither)
     float xz[C::HALF];                             // 0 if one of the two is in the window, else -inf
 #pragma unroll
     for (int c = 0; c < C::HALF; ++c) {
       const bool in_lo = c >= lo_x && c < lo_x + C::KX, in_hi = c + C::HALF >= lo_x && c + C::HALF < lo_x + C::KX;
       m_lo[c] = in_lo ? 0xffffffffu : 0u;
-      m_hi[c] = in_hi ? 0xffffffffu : 0u;
       xz[c] = (in_lo || in_hi) ? 0.f : -INFINITY;
+    }
+    // un-fold: P word j holds the halo columns (2j, 2j+1).  Column col comes from the folded value
+    // fc = col mod HALF, which sits in half (fc & 1) of the packed word F[fc / 2]; psel[j] is the byte
+    // selector of prmt(F[fc(2j) / 2], F[fc(2j+1) / 2]).  A column outside the window selects "sign of a
+    // high byte", which is 0x00 because every P value is >= +0.
+    uint32_t psel[C::HX / 2];
+#pragma unroll
+    for (int j = 0; j < C::HX / 2; ++j) {
+      const int c0 = 2 * j, c1 = 2 * j + 1;
+      const int f0 = c0 % C::HALF, f1 = c1 % C::HALF;
+      const bool v0 = c0 >= lo_x && c0 < lo_x + C::KX, v1 = c1 >= lo_x && c1 < lo_x + C::KX;
+      const uint32_t n0 = v0 ? (uint32_t)(2 * (f0 & 1)) | ((uint32_t)(2 * (f0 & 1) + 1) << 4) : 0x99u;
+      const uint32_t n1 = v1 ? (uint32_t)(4 + 2 * (f1 & 1)) | ((uint32_t)(5 + 2 * (f1 & 1)) << 4) : 0xDDu;
+      psel[j] = n0 | (n1 << 8);
     }
 
     int i = 0;
@@ -560,12 +594,10 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         for (int part = 0; part < nparts; ++part, ++i) {
           const int pb = C::part_begin(part);
           const int nrows = part_rows(part);
-          const int nwords = ((nrows * C::HX + 15) / 16 * 16) / 2;
           const uint32_t s_addr = tm + C::TMEM_S + (i & 1) * C::NMAX;
           const bool first_item = (plane == plo && part == 0);
-          // rows of this part some query of the warp needs: [ra, rb) (warp-uniform)
-          const int ra = plane_needed ? max(0, wy_lo - pb) : 0;
-          const int rb = plane_needed ? min(nrows, wy_hi - pb) : 0;
+          // does some query of the warp attend a key row of this part? (warp-uniform)
+          const bool warp_needs = plane_needed && max(0, wy_lo - pb) < min(nrows, wy_hi - pb);
           // rows of this part inside this query's window: [ya, yb)
           const int ya = plane_ok ? max(0, lo_y - pb) : 0;
           const int yb = plane_ok ? min(nrows, lo_y + C::KY - pb) : 0;
@@ -573,19 +605,73 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           if (sp == 0 && lane == 0) TRACE(12 + slot, i);
           tc_fence_after();
 
-          // folded logits of key row r (already waited for) -> v[0 .. HALF)
-          auto fold = [&](const uint32_t (&sv)[16], float (&v)[C::HALF]) {
+          // One part of R key rows (the whole TMA box: rows past the halo are zero keys, masked by [ya, yb)).
+          auto do_part = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+            constexpr int NCOL = R * C::HX, NW = ((NCOL + 15) / 16 * 16) / 2;
+            float v[R][C::HALF];                     // folded logits
+            {
+              uint32_t sv[NCOL];
+              tmem_ld_n<NCOL>(s_addr, sv);
 #pragma unroll
-            for (int c = 0; c < C::HALF; ++c) v[c] = __uint_as_float(bitsel(m_lo[c], sv[c], sv[c + C::HALF]));
-          };
-          // new reference maximum m_new >= m_ref for this row: rescale what was accumulated so far
-          auto rescale = [&](float new_ref, int rows_done_from, int rows_done_to) {
-            const float alpha = (inited && new_ref != m_ref) ? ex2(m_ref - new_ref) : 1.f;
-            if (__any_sync(0xffffffffu, alpha != 1.f)) {
+              for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int c = 0; c < C::HALF; ++c)
+                  v[r][c] = __uint_as_float(bitsel(m_lo[c], sv[r * C::HX + c], sv[r * C::HX + c + C::HALF]));
+            }
+            // maximum of this query's valid logits of the part (log2 units)
+            auto part_max = [&]() {
+              float cmax = -INFINITY;
+#pragma unroll
+              for (int r = 0; r < R; ++r) {
+                float rmax = -INFINITY;
+#pragma unroll
+                for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[r][c] * cs : fmaf(v[r][c], cs, xz[c]));
+                if (r >= ya && r < yb) cmax = fmaxf(cmax, rmax);
+              }
+              return cmax;
+            };
+            if (__any_sync(0xffffffffu, ya < yb && !inited)) {
+              // ---- first valid keys of some query: its reference is the true maximum of this part
+              const float cmax = part_max();
+              if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
+            }
+            float pr[R][C::HALF];                    // folded probabilities (times 2^-m_ref)
+            float rs;
+#pragma unroll 1
+            for (int attempt = 0;; ++attempt) {
+              // ---- p = 2^(s * cs - m_ref), branch-free over the whole part
+              float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
+#pragma unroll
+              for (int r = 0; r < R; ++r) {
+                const float br = (r >= ya && r < yb) ? -m_ref : -INFINITY;
+#pragma unroll
+                for (int c = 0; c < C::HALF; c += 2) {
+                  if (c + 1 < C::HALF) {
+                    float t0, t1;
+                    if (C::FULLFOLD) ffma2(t0, t1, v[r][c], v[r][c + 1], cs, br, br);
+                    else ffma2(t0, t1, v[r][c], v[r][c + 1], cs, br + xz[c], br + xz[c + 1]);
+                    pr[r][c] = ex2(t0); pr[r][c + 1] = ex2(t1);
+                    if ((c >> 1) & 1) fadd2(e2, e3, e2, e3, pr[r][c], pr[r][c + 1]);
+                    else fadd2(e0, e1, e0, e1, pr[r][c], pr[r][c + 1]);
+                  } else {
+                    pr[r][c] = ex2(fmaf(v[r][c], cs, C::FULLFOLD ? br : br + xz[c]));
+                    e0 += pr[r][c];
+                  }
+                }
+              }
+              rs = (e0 + e1) + (e2 + e3);
+              if (attempt > 0 || !__any_sync(0xffffffffu, !(rs <= kBig))) break;
+              // ---- a logit far above the reference: move the reference to the true maximum and
+              // rescale what was accumulated so far (P of this part is not stored yet)
+              const bool mine = !(rs <= kBig);
+              const float new_ref = mine ? fmaxf(m_ref, part_max()) : m_ref;
+              const float alpha = new_ref != m_ref ? ex2(m_ref - new_ref) : 1.f;
               if (!first_item) {
-                // O holds earlier parts of this tile: rescale its rows (all its PV MMAs are complete)
+                // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
                 mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
                 tc_fence_after();
+#pragma unroll 1
                 for (int j = 0; j < C::D; j += 16) {
                   float ov[16];
                   tmem_ld16(tm + C::TMEM_O + j, ov);
@@ -595,113 +681,38 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                   for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
                   tmem_st16(tm + C::TMEM_O + j, ow);
                 }
+                tmem_wait_st();
               }
-              // P rows of this part that are already stored with the old reference
-              tmem_wait_st();
-              for (int r = rows_done_from; r < rows_done_to; ++r)
-                for (int j = 0; j < C::HALF; ++j) {
-                  uint32_t w;
-                  tmem_ld1(s_addr + r * C::HALF + j, w);
-                  tmem_wait_ld();
-                  w = pack_bf16(__uint_as_float(w << 16) * alpha, __uint_as_float(w & 0xffff0000u) * alpha);
-                  tmem_st1(s_addr + r * C::HALF + j, w);
-                }
-              tmem_wait_st();
+              lsum *= alpha;
+              m_ref = new_ref;
             }
-            lsum *= alpha;
-            m_ref = new_ref;
+            lsum += rs;
+            // ---- pack folded pairs to bf16x2, un-fold with one byte permute per output word; P overlays
+            // the front of S (every S column of the part is in registers by now)
+            uint32_t pw[NW];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+              uint32_t f[C::NF];
+#pragma unroll
+              for (int m = 0; m < C::NF; ++m) f[m] = pack_bf16(pr[r][2 * m], 2 * m + 1 < C::HALF ? pr[r][2 * m + 1] : 0.f);
+#pragma unroll
+              for (int j = 0; j < C::HX / 2; ++j)
+                pw[r * (C::HX / 2) + j] = prmt(f[((2 * j) % C::HALF) / 2], f[((2 * j + 1) % C::HALF) / 2], psel[j]);
+            }
+#pragma unroll
+            for (int j = R * (C::HX / 2); j < NW; ++j) pw[j] = 0u;     // pad keys
+            tmem_st_n<NW>(s_addr, pw);
           };
 
-          float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;            // partial sums of this part (times 2^-m_ref)
-          if (ra < rb) {
-            if (__any_sync(0xffffffffu, ya < yb && !inited)) {
-              // ---- first valid keys of some query: reference maximum = true maximum of this part
-              float cmax = -INFINITY;
-              for (int r = ra; r < rb; ++r) {
-                uint32_t sv[16];
-                ld16_issue(s_addr + r * C::HX, sv);
-                ld16_wait(sv);
-                float v[C::HALF];
-                fold(sv, v);
-                float rmax = -INFINITY;
-#pragma unroll
-                for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[c] * cs : v[c] * cs + xz[c]);
-                if (r >= ya && r < yb) cmax = fmaxf(cmax, rmax);
-              }
-              const bool got = cmax > -INFINITY;
-              rescale(got ? (inited ? fmaxf(m_ref, cmax) : cmax) : m_ref, 0, 0);
-              inited = inited || got;
-            }
-            // ---- p = 2^(s * cs - m_ref) on the folded rows, two rows per iteration
-            for (int r0 = ra; r0 < rb; r0 += 2) {
-              uint32_t sva[16], svb[16];
-              const bool two = r0 + 1 < rb;
-              ld16_issue(s_addr + r0 * C::HX, sva);
-              if (two) ld16_issue(s_addr + (r0 + 1) * C::HX, svb);
-              ld16_wait(sva);
-              if (two) ld16_wait(svb);
-#pragma unroll
-              for (int u = 0; u < 2; ++u) {
-                if (u == 1 && !two) break;
-                const int r = r0 + u;
-                float v[C::HALF], pv[C::HALF];
-                fold(u ? svb : sva, v);
-                float br = (r >= ya && r < yb) ? -m_ref : -INFINITY;
-                auto expo = [&]() {
-                  float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
-#pragma unroll
-                  for (int c = 0; c < C::HALF; c += 2) {
-                    if (c + 1 < C::HALF) {
-                      float t0, t1;
-                      if (C::FULLFOLD) ffma2(t0, t1, v[c], v[c + 1], cs, br, br);
-                      else ffma2(t0, t1, v[c], v[c + 1], cs, br + xz[c], br + xz[c + 1]);
-                      pv[c] = ex2(t0); pv[c + 1] = ex2(t1);
-                      if ((c >> 1) & 1) fadd2(e2, e3, e2, e3, pv[c], pv[c + 1]);
-                      else fadd2(e0, e1, e0, e1, pv[c], pv[c + 1]);
-                    } else {
-                      pv[c] = ex2(fmaf(v[c], cs, C::FULLFOLD ? br : br + xz[c]));
-                      e0 += pv[c];
-                    }
-                  }
-                  return (e0 + e1) + (e2 + e3);
-                };
-                float rs = expo();
-                if (__any_sync(0xffffffffu, !(rs <= kBig))) {
-                  // ---- a logit far above the reference: move the reference to this row's maximum
-                  float rmax = -INFINITY;
-#pragma unroll
-                  for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[c] * cs : v[c] * cs + xz[c]);
-                  const bool mine = !(rs <= kBig);
-                  const float part_sum = (a0 + a1) + (a2 + a3);
-                  const float old_ref = m_ref;
-                  rescale(mine ? fmaxf(m_ref, rmax) : m_ref, ra, r);
-                  const float al2 = ex2(old_ref - m_ref);
-                  a0 = part_sum * al2; a1 = 0.f; a2 = 0.f; a3 = 0.f;
-                  br = (r >= ya && r < yb) ? -m_ref : -INFINITY;
-                  rs = expo();
-                }
-                a0 += rs;
-                // un-fold: slot k < HALF takes p[k] if column k is the valid one, slot k + HALF otherwise
-                uint32_t pw[C::HALF];
-#pragma unroll
-                for (int j = 0; j < C::HALF; ++j) {
-                  const int k0 = 2 * j, k1 = 2 * j + 1;
-                  const uint32_t s0 = k0 < C::HALF ? (__float_as_uint(pv[k0]) & m_lo[k0]) : (__float_as_uint(pv[k0 - C::HALF]) & m_hi[k0 - C::HALF]);
-                  const uint32_t s1 = k1 < C::HALF ? (__float_as_uint(pv[k1]) & m_lo[k1]) : (__float_as_uint(pv[k1 - C::HALF]) & m_hi[k1 - C::HALF]);
-                  pw[j] = pack_bf16(__uint_as_float(s0), __uint_as_float(s1));
-                }
-                tmem_st_words<C::HALF>(s_addr + r * C::HALF, pw);
-              }
-            }
-            lsum += (a0 + a1) + (a2 + a3);
-            // rows outside [ra, rb) and the pad keys are zero in P (stored last: P overlays S)
-            for (int j = 0; j < ra * C::HALF; ++j) tmem_st1(s_addr + j, 0u);
-            for (int j = rb * C::HALF; j < nwords; ++j) tmem_st1(s_addr + j, 0u);
+          if (warp_needs) {
+            if (part == 1) do_part(std::integral_constant<int, C::RB>{});
+            else do_part(std::integral_constant<int, C::RA>{});
           } else {
             // no query of this warp attends a key of this part: P = 0
             uint32_t z[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) z[u] = 0u;
+            const int nwords = (part == 1 ? C::NB : C::NA) / 2;
             for (int j = 0; j < nwords; j += 8) tmem_st8(s_addr + j, z);
           }
           tmem_wait_st();

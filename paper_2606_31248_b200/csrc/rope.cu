@@ -7,8 +7,6 @@
 // The angle is accumulated in fp64 and reduced to [-pi, pi] before the fp32 sincos: coordinates
 // are in native-cell units (|x| up to ~1.5e3 for cfg 0), so an fp32 product would already carry
 // ~1e-4 rad of rounding -- the whole fp32 error budget of BASELINE.json.
-#include <cuda_fp16.h>
-
 #include "common.cuh"
 
 namespace strata {
@@ -70,21 +68,31 @@ rope_rotate_kernel(const TIn* __restrict__ x0, const TIn* __restrict__ x1, TOut*
   }
 }
 
-// A1 for the fused tensor-core kernels: table[t][j] = (cos phi[t][j], sin phi[t][j]) as a half2, one
-// 2*D-byte row per token (all heads of a token share it).  One thread per (token, pair).
+// A1 for the fused tensor-core kernels: one 2*D-byte table row per token (all heads of a token share
+// it) of bf16x2 words, two per pair of rotary pairs (m, m+1), m even:
+//   word m     = (cos phi[t][m], cos phi[t][m+1])      word m + 1 = (sin phi[t][m], sin phi[t][m+1])
+// -- the operand layout of the packed bf16x2 rotation in na3d_fwd_fused.cu.  One thread per (token, m).
 __global__ void __launch_bounds__(256)
-rope_table_kernel(__half2* __restrict__ table, const float* __restrict__ coords, const float* __restrict__ freqs,
+rope_table_kernel(uint2* __restrict__ table, const float* __restrict__ coords, const float* __restrict__ freqs,
                   long long tokens, int half, int A) {
+  const int quarter = half >> 1;
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= tokens * half) return;
-  const long long t = gid / half;
-  const int j = (int)(gid - t * half);
-  double phi = 0.0;
-  for (int a = 0; a < A; ++a) phi += (double)coords[t * A + a] * (double)freqs[a * half + j];
-  const double r = phi - 6.283185307179586477 * rint(phi * 0.15915494309189533577);
-  float sn, cs;
-  sincosf((float)r, &sn, &cs);
-  table[gid] = __floats2half2_rn(cs, sn);
+  if (gid >= tokens * quarter) return;
+  const long long t = gid / quarter;
+  const int m = 2 * (int)(gid - t * quarter);
+  float cs[2], sn[2];
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    double phi = 0.0;
+    for (int a = 0; a < A; ++a) phi += (double)coords[t * A + a] * (double)freqs[a * half + m + u];
+    const double r = phi - 6.283185307179586477 * rint(phi * 0.15915494309189533577);
+    sincosf((float)r, &sn[u], &cs[u]);
+  }
+  const __nv_bfloat162 c2 = __floats2bfloat162_rn(cs[0], cs[1]), s2 = __floats2bfloat162_rn(sn[0], sn[1]);
+  uint2 w;
+  w.x = *reinterpret_cast<const uint32_t*>(&c2);
+  w.y = *reinterpret_cast<const uint32_t*>(&s2);
+  table[gid] = w;
 }
 
 }  // namespace
@@ -92,12 +100,12 @@ rope_table_kernel(__half2* __restrict__ table, const float* __restrict__ coords,
 cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
                               cudaStream_t stream, int* launches) {
   const long long tokens = (long long)p.B * p.N;
-  const long long threads = tokens * (p.D / 2);
+  const long long threads = tokens * (p.D / 4);
   const int block = 256;
   const long long grid = (threads + block - 1) / block;
   if (grid <= 0 || grid > 0x7fffffffLL) return cudaErrorInvalidValue;
   prof_begin("rope_table", stream);
-  rope_table_kernel<<<(unsigned)grid, block, 0, stream>>>((__half2*)table, coords, freqs, tokens, p.D / 2, p.A);
+  rope_table_kernel<<<(unsigned)grid, block, 0, stream>>>((uint2*)table, coords, freqs, tokens, p.D / 2, p.A);
   prof_end(stream);
   if (launches) ++*launches;
   return cudaGetLastError();
