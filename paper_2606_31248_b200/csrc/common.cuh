@@ -68,6 +68,13 @@ cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, 
                             const void* o, const void* d_o, const float* lse, float* delta,
                             float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches);
 
+// na3d_bwd_tc.cu: tcgen05 backward on pre-rotated bf16 operands (head_dim 64); dqr / dkr are fp32 gradients
+// w.r.t. the rotated operands, stat is [B, H, N] float2 scratch.
+bool tc_bwd_supported(const Problem& p);
+cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
+                          const void* d_o, const float* lse, void* stat, float* dqr, float* dkr, void* dv,
+                          cudaStream_t stream, int* launches);
+
 // na3d_tc_fwd_sweep.cu: tcgen05 forward, one CTA per level column (head_dim 64, k_L = 3).
 bool tc_sweep_supported(const Problem& p);
 cudaError_t launch_fwd_sweep(const Problem& p, const void* qr, const void* kr, const void* v, void* o,

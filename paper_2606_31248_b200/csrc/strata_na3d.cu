@@ -55,7 +55,7 @@ enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_FUSED = 3
 Path select_path(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
   if (d->impl == STRATA_IMPL_SIMT) return PATH_SIMT;
   const bool fused_ok = !backward && !p.force_tile && strata::fused_fwd_supported(p);
-  const bool tc_ok = !backward && strata::tc_fwd_supported(p);
+  const bool tc_ok = backward ? strata::tc_bwd_supported(p) : strata::tc_fwd_supported(p);
   if (fused_ok) return PATH_TC_FUSED;
   if (tc_ok) return PATH_TC_PREROT;
   return d->impl == STRATA_IMPL_AUTO ? PATH_SIMT : PATH_NONE;
@@ -79,6 +79,7 @@ struct Carve {
 size_t ws_bytes(const Problem& p, Path path, bool backward) {
   const size_t e = (size_t)p.elems();
   const size_t stat = align_up((size_t)p.B * p.H * p.N * 4);
+  if (backward && path == PATH_TC_PREROT) return 2 * align_up(e * 2) + 2 * align_up(e * 4) + 2 * stat;   // qr, kr (bf16), dqr, dkr, stat
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
   if (path == PATH_TC_FUSED) return align_up((size_t)p.B * p.N * p.D * 2);   // (cos, sin) half2 table
   if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
@@ -216,13 +217,29 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, c
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   Carve ws{reinterpret_cast<char*>(workspace), 0};
   const size_t eb = (size_t)p.elems() * 4;
+  int launches = 0;
+  cudaError_t e;
+  if (path == PATH_TC_PREROT) {
+    void* qr = ws.take<char>(eb / 2);
+    void* kr = ws.take<char>(eb / 2);
+    float* dqr = ws.take<float>(eb);
+    float* dkr = ws.take<float>(eb);
+    void* stat = ws.take<char>(2 * stat_bytes(p));
+    e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
+    if (e != cudaSuccess) return cuda_status(e);
+    e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, lse, stat, dqr, dkr, dv, st, &launches);
+    if (e != cudaSuccess) return cuda_status(e);
+    e = strata::launch_rope_rotate(p, dqr, dkr, 0, dq, dk, p.dtype, coords, freqs, -1.f, st, &launches);
+    if (e != cudaSuccess) return cuda_status(e);
+    g_last_launches = launches;
+    return STRATA_OK;
+  }
   float* qr = ws.take<float>(eb);
   float* kr = ws.take<float>(eb);
   float* dqr = ws.take<float>(eb);
   float* dkr = ws.take<float>(eb);
   float* delta = ws.take<float>(stat_bytes(p));
-  int launches = 0;
-  cudaError_t e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 0, coords, freqs, 1.f, st, &launches);
+  e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 0, coords, freqs, 1.f, st, &launches);
   if (e != cudaSuccess) return cuda_status(e);
   e = strata::launch_bwd_simt(p, qr, kr, v, o, d_o, lse, delta, dqr, dkr, dv, st, &launches);
   if (e != cudaSuccess) return cuda_status(e);

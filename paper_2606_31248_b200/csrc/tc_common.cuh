@@ -2,6 +2,9 @@
 // helper shared by the tensor-core kernels.  sm_100a only.
 #pragma once
 #include <cuda.h>
+#ifdef STRATA_DEBUG_SYNC
+#include <cstdio>
+#endif
 
 #include "common.cuh"
 
@@ -36,7 +39,12 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity, uin
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > 20000u) __trap();
+    if (++spins > 20000u) {
+#ifdef STRATA_DEBUG_SYNC
+      printf("mbar timeout: block %d thread %d bar 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
+#endif
+      __trap();
+    }
   }
 }
 // One lane of a converged warp (all 32 lanes must execute this).

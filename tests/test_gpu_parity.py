@@ -128,6 +128,8 @@ SWEEP = [
     dict(grid=(10, 20, 12), window=(3, 7, 7), heads=1, head_dim=64),               # level sweep, 5 tiles
     dict(grid=(3, 8, 8), window=(3, 7, 7), heads=2, head_dim=64),                  # level sweep, L = k_L
     dict(grid=(12, 7, 30), window=(3, 7, 7), heads=1, head_dim=64),                # level sweep, Y = k_Y
+    dict(grid=(4, 20, 20), window=(3, 7, 7), heads=2, head_dim=64),                # tcgen05 bwd: inverse halo wider than one chunk
+    dict(grid=(7, 12, 20), window=(3, 5, 5), heads=1, head_dim=64, batch=2),       # tcgen05 bwd (3,5,5), odd L, ragged y
 ]
 
 
@@ -165,6 +167,7 @@ def test_tcgen05_is_selected_for_the_bf16_configs():
     for i in (1, 2, 3):
         assert binding.strata_na3d_impl_selected(desc_of(wl.config(i))) == binding.IMPL_TCGEN05
     assert binding.strata_na3d_impl_selected(desc_of(wl.config(0))) == binding.IMPL_SIMT
+    assert binding.strata_na3d_impl_selected(desc_of(wl.config(4)), True) == binding.IMPL_TCGEN05
 
 
 def test_explicit_scale(oracle_mod):
