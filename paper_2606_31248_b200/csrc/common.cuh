@@ -56,6 +56,10 @@ cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1,
 cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
                               cudaStream_t stream, int* launches);
 
+// rope.cu: A1 as an fp32 table [B, L, Y, X, D/2] float2 (cos, sin), for the backward epilogues (B4).
+cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* coords, const float* freqs,
+                                  cudaStream_t stream, int* launches);
+
 // na3d_fwd_fused.cu: tcgen05 forward with the rotation of Q and K fused in (un-rotated bf16 operands).
 bool fused_fwd_supported(const Problem& p);
 cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
@@ -68,12 +72,12 @@ cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, 
                             const void* o, const void* d_o, const float* lse, float* delta,
                             float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches);
 
-// na3d_bwd_tc.cu: tcgen05 backward on pre-rotated bf16 operands (head_dim 64); dqr / dkr are fp32 gradients
-// w.r.t. the rotated operands, stat is [B, H, N] float2 scratch.
+// na3d_bwd_tc.cu: tcgen05 backward on pre-rotated bf16 operands (head_dim 64).  stat is [B, H, N] float2
+// scratch; rtab the fp32 rotary table (nullptr: no rotation): the epilogues apply B4 and write bf16 dq, dk.
 bool tc_bwd_supported(const Problem& p);
 cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
-                          const void* d_o, const float* lse, void* stat, float* dqr, float* dkr, void* dv,
-                          cudaStream_t stream, int* launches);
+                          const void* d_o, const float* lse, void* stat, const void* rtab, void* dq, void* dk,
+                          void* dv, cudaStream_t stream, int* launches);
 
 // na3d_tc_fwd_sweep.cu: tcgen05 forward, one CTA per level column (head_dim 64, k_L = 3).
 bool tc_sweep_supported(const Problem& p);

@@ -1,7 +1,7 @@
 // na3d_bwd_tc.cu -- tcgen05 / TMEM / TMA backward kernels for 3D neighbourhood attention (sm_100a).
 //
-// Steps B1-B3 of DESIGN.md on pre-rotated bf16 operands (rope.cu rotates Q, K before and un-rotates
-// dQrot, dKrot after: B4).  PAPER.md gives no backward; BASELINE.json config 4 and SURVEY.md §8(a)
+// Steps B1-B4 of DESIGN.md on pre-rotated bf16 operands (rope.cu rotates Q, K before; the transpose
+// rotation B4 of dQrot, dKrot is fused into the epilogues, from an fp32 cos/sin table).  PAPER.md gives no backward; BASELINE.json config 4 and SURVEY.md §8(a)
 // rows B1-B4 define it:
 //   B1  D_i    = sum_c dO_ic O_ic                       (bwd_stat_kernel, stored with lse * log2 e)
 //   B2  p_ij   = exp(scale qrot_i . krot_j - lse_i),  dP_ij = dO_i . v_j,  dS_ij = p_ij (dP_ij - D_i)
@@ -27,6 +27,7 @@
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 = elementwise + epilogue.
 // TMEM (256 columns): acc1 [0,64) | acc2 [64,128) | S' -> P [128,192) | dP' -> dS [192,256).
 #include <cstdio>
+#include <type_traits>
 
 #include "tc_common.cuh"
 
@@ -60,6 +61,7 @@ struct BwdParams {
   int ntl, nty, ntx;
   long long N;
   float scale, scale_log2e;
+  int pairing;   // strata_rope_pairing_t of the fused un-rotation
 };
 
 constexpr int kBwdThreads = 192;
@@ -82,8 +84,8 @@ template <class C, int MODE>
 __global__ void __launch_bounds__(kBwdThreads, 2)
 na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_constant__ CUtensorMap tm_a2,
                    const __grid_constant__ CUtensorMap tm_b1, const __grid_constant__ CUtensorMap tm_b2,
-                   const float2* __restrict__ stat,
-                   float* __restrict__ out1, __nv_bfloat16* __restrict__ out2, const BwdParams p) {
+                   const float2* __restrict__ stat, const float4* __restrict__ rtab,
+                   __nv_bfloat16* __restrict__ out1, __nv_bfloat16* __restrict__ out2, const BwdParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -305,19 +307,43 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
           mbar_arrive(bar_pfull);
         }
     }
-    // ---- epilogue: acc1 * scale -> fp32 rows of dQrot / dKrot (un-rotated by rope.cu), acc2 -> bf16 dV
+    // ---- epilogue: B4 fused -- dx = R(-phi) (scale * acc1), (a, b) -> (a cos + b sin, b cos - a sin) on every
+    // rotary pair of the row, rounded to bf16; acc2 -> bf16 dV
     mbar_wait(bar_done, 0);
     tc_fence_after();
-    float* r1 = out1 + (((long long)b * p.N + tok) * p.H + h) * C::D;
+    {
+      __nv_bfloat16* r1 = out1 + (((long long)b * p.N + tok) * p.H + h) * C::D;
+      const float4* trow = rtab ? rtab + ((long long)b * p.N + tok) * (C::D / 4) : nullptr;   // 2 pairs per float4
+      float av[C::D];
 #pragma unroll
-    for (int j = 0; j < C::D; j += 16) {
-      float av[16];
-      tmem_ld16(tm + C::TMEM_ACC1 + j, av);
+      for (int j = 0; j < C::D; j += 16) tmem_ld16(tm + C::TMEM_ACC1 + j, *reinterpret_cast<float(*)[16]>(&av[j]));
       tmem_wait_ld();
-      if (active) {
 #pragma unroll
-        for (int u = 0; u < 16; u += 4)
-          reinterpret_cast<float4*>(r1 + j)[u >> 2] = make_float4(av[u] * p.scale, av[u + 1] * p.scale, av[u + 2] * p.scale, av[u + 3] * p.scale);
+      for (int j = 0; j < C::D; ++j) av[j] *= p.scale;
+      if (active) {
+        if (trow) {
+          auto rot = [&](auto half_pairing) {
+            constexpr bool HP = decltype(half_pairing)::value;
+#pragma unroll
+            for (int m = 0; m < C::D / 2; m += 2) {               // pairs m, m + 1
+              const float4 t = __ldg(trow + (m >> 1));            // (cos m, sin m, cos m+1, sin m+1)
+              constexpr int dummy = 0; (void)dummy;
+              const int a0 = HP ? m : 2 * m, b0 = HP ? m + C::D / 2 : 2 * m + 1;
+              const int a1 = HP ? m + 1 : 2 * m + 2, b1 = HP ? m + 1 + C::D / 2 : 2 * m + 3;
+              const float xa0 = av[a0], xb0 = av[b0], xa1 = av[a1], xb1 = av[b1];
+              av[a0] = fmaf(xb0, t.y, xa0 * t.x); av[b0] = fmaf(-xa0, t.y, xb0 * t.x);
+              av[a1] = fmaf(xb1, t.w, xa1 * t.z); av[b1] = fmaf(-xa1, t.w, xb1 * t.z);
+            }
+          };
+          if (p.pairing) rot(std::true_type{}); else rot(std::false_type{});
+        }
+#pragma unroll
+        for (int j = 0; j < C::D; j += 8) {
+          uint4 w;
+          w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
+          w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
+          reinterpret_cast<uint4*>(r1)[j >> 3] = w;
+        }
       }
     }
     if (MODE == 1) {
@@ -381,7 +407,7 @@ bwd_stat_kernel(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __rest
 
 template <class C>
 cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
-                           const void* d_o, const float* lse, float2* stat, float* dqr, float* dkr, void* dv,
+                           const void* d_o, const float* lse, float2* stat, const void* rtab, void* dq, void* dk, void* dv,
                            cudaStream_t stream, int* launches) {
   CUtensorMap tq_t, tdo_t, tk_c, tv_c, tk_t, tv_t, tq_c, tdo_c;
   if (!make_map(&tq_t, qr, p, C::TX, C::TY, C::TL) || !make_map(&tdo_t, d_o, p, C::TX, C::TY, C::TL) ||
@@ -392,7 +418,7 @@ cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, con
   BwdParams bp;
   bp.B = p.B; bp.H = p.H; bp.L = p.L; bp.Y = p.Y; bp.X = p.X; bp.N = p.N;
   bp.ntl = (p.L + C::TL - 1) / C::TL; bp.nty = (p.Y + C::TY - 1) / C::TY; bp.ntx = (p.X + C::TX - 1) / C::TX;
-  bp.scale = p.scale; bp.scale_log2e = p.scale * 1.4426950408889634f;
+  bp.scale = p.scale; bp.scale_log2e = p.scale * 1.4426950408889634f; bp.pairing = p.pairing;
   const long long grid = (long long)p.B * p.H * bp.ntl * bp.nty * bp.ntx;
   const long long rows = p.rows(), sgrid = (rows * 8 + 255) / 256;
   if (grid > 0x7fffffffLL || sgrid > 0x7fffffffLL) return cudaErrorInvalidValue;
@@ -415,11 +441,12 @@ cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, con
   prof_end(stream);
   STRATA_DBG("stat");
   prof_begin("na3d_bwd_dq_tcgen05", stream);
-  na3d_bwd_tc_kernel<C, 0><<<(unsigned)grid, kBwdThreads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, dqr, nullptr, bp);
+  na3d_bwd_tc_kernel<C, 0><<<(unsigned)grid, kBwdThreads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, (const float4*)rtab, (__nv_bfloat16*)dq,
+                                                                                  nullptr, bp);
   prof_end(stream);
   STRATA_DBG("dq");
   prof_begin("na3d_bwd_dkdv_tcgen05", stream);
-  na3d_bwd_tc_kernel<C, 1><<<(unsigned)grid, kBwdThreads, C::SMEM_BYTES, stream>>>(tk_t, tv_t, tq_c, tdo_c, stat, dkr,
+  na3d_bwd_tc_kernel<C, 1><<<(unsigned)grid, kBwdThreads, C::SMEM_BYTES, stream>>>(tk_t, tv_t, tq_c, tdo_c, stat, (const float4*)rtab, (__nv_bfloat16*)dk,
                                                                                   (__nv_bfloat16*)dv, bp);
   prof_end(stream);
   STRATA_DBG("dkdv");
@@ -446,11 +473,11 @@ bool tc_bwd_supported(const Problem& p) {
 }
 
 cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
-                          const void* d_o, const float* lse, void* stat, float* dqr, float* dkr, void* dv,
-                          cudaStream_t stream, int* launches) {
+                          const void* d_o, const float* lse, void* stat, const void* rtab, void* dq, void* dk,
+                          void* dv, cudaStream_t stream, int* launches) {
 #define X(KL_, KY_, KX_)                                        \
   if (p.kL == KL_ && p.kY == KY_ && p.kX == KX_)                \
-    return launch_bwd_cfg<BwdCfg<KL_, KY_, KX_>>(p, qr, kr, v, o, d_o, lse, (float2*)stat, dqr, dkr, dv, stream, launches);
+    return launch_bwd_cfg<BwdCfg<KL_, KY_, KX_>>(p, qr, kr, v, o, d_o, lse, (float2*)stat, rtab, dq, dk, dv, stream, launches);
   STRATA_BWD_CONFIGS(X)
 #undef X
   return cudaErrorNotSupported;

@@ -95,7 +95,36 @@ rope_table_kernel(uint2* __restrict__ table, const float* __restrict__ coords, c
   table[gid] = w;
 }
 
+// A1 as an fp32 table for the backward epilogues (B4): table[t][j] = (cos phi[t][j], sin phi[t][j]).
+__global__ void __launch_bounds__(256)
+rope_table_f32_kernel(float2* __restrict__ table, const float* __restrict__ coords, const float* __restrict__ freqs,
+                      long long tokens, int half, int A) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= tokens * half) return;
+  const long long t = gid / half;
+  const int j = (int)(gid - t * half);
+  double phi = 0.0;
+  for (int a = 0; a < A; ++a) phi += (double)coords[t * A + a] * (double)freqs[a * half + j];
+  const double r = phi - 6.283185307179586477 * rint(phi * 0.15915494309189533577);
+  float sn, cs;
+  sincosf((float)r, &sn, &cs);
+  table[gid] = make_float2(cs, sn);
+}
+
 }  // namespace
+
+cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* coords, const float* freqs,
+                                  cudaStream_t stream, int* launches) {
+  const long long tokens = (long long)p.B * p.N;
+  const long long threads = tokens * (p.D / 2);
+  const long long grid = (threads + 255) / 256;
+  if (grid <= 0 || grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+  prof_begin("rope_table_f32", stream);
+  rope_table_f32_kernel<<<(unsigned)grid, 256, 0, stream>>>((float2*)table, coords, freqs, tokens, p.D / 2, p.A);
+  prof_end(stream);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
                               cudaStream_t stream, int* launches) {

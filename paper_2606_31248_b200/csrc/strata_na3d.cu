@@ -79,7 +79,8 @@ struct Carve {
 size_t ws_bytes(const Problem& p, Path path, bool backward) {
   const size_t e = (size_t)p.elems();
   const size_t stat = align_up((size_t)p.B * p.H * p.N * 4);
-  if (backward && path == PATH_TC_PREROT) return 2 * align_up(e * 2) + 2 * align_up(e * 4) + 2 * stat;   // qr, kr (bf16), dqr, dkr, stat
+  if (backward && path == PATH_TC_PREROT)                               // qr, kr (bf16), stat (float2), fp32 rotary table
+    return 2 * align_up(e * 2) + align_up(2 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
   if (path == PATH_TC_FUSED) return align_up((size_t)p.B * p.N * p.D * 2);   // (cos, sin) half2 table
   if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
@@ -222,14 +223,15 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, c
   if (path == PATH_TC_PREROT) {
     void* qr = ws.take<char>(eb / 2);
     void* kr = ws.take<char>(eb / 2);
-    float* dqr = ws.take<float>(eb);
-    float* dkr = ws.take<float>(eb);
-    void* stat = ws.take<char>(2 * stat_bytes(p));
+    void* stat = ws.take<char>(2 * align_up(stat_bytes(p)));
+    void* rtab = ws.take<char>((size_t)p.B * p.N * (p.D / 2) * 8);
     e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
-    e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, lse, stat, dqr, dkr, dv, st, &launches);
-    if (e != cudaSuccess) return cuda_status(e);
-    e = strata::launch_rope_rotate(p, dqr, dkr, 0, dq, dk, p.dtype, coords, freqs, -1.f, st, &launches);
+    if (p.A > 0) {
+      e = strata::launch_rope_table_f32(p, rtab, coords, freqs, st, &launches);
+      if (e != cudaSuccess) return cuda_status(e);
+    }
+    e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, lse, stat, p.A > 0 ? rtab : nullptr, dq, dk, dv, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
     g_last_launches = launches;
     return STRATA_OK;
