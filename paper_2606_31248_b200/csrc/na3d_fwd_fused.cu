@@ -69,7 +69,7 @@ struct FusedCfg {
   static constexpr int NSTAGE = NS_;
   static constexpr int NQBUF = (D == 64) ? 2 : 1;                  // Q buffers per slot
   static constexpr int TMEM_SLOT = 256, TMEM_O = 0, TMEM_S = D;
-  static constexpr int NBARS = 5 * NSTAGE + 2 * 12 + 1;
+  static constexpr int NBARS = 5 * NSTAGE + 2 * 14 + 1;
   static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 512;
   static constexpr bool FULLFOLD = (KX == HALF);                   // exactly one of the columns c, c + HALF is in the window
   static_assert(TL * TY * TX == 128 && (TY * TX) % 32 == 0 && TY == 2 * G, "128 queries per tile, one level per warp, two warps per level");
@@ -313,10 +313,12 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   auto bar_vfull = [&](int s) { return bars + 8u * (3 * C::NSTAGE + s); };
   auto bar_vempty = [&](int s) { return bars + 8u * (4 * C::NSTAGE + s); };
   // per slot: 0,1 qfull[buf]  2,3 qrot[buf]  4,5 qfree[buf]  6,7 sfull[buf]  8,9 pfull[buf]  10,11 pvdone[buf]
+  // 12,13 pvissued[buf] (the PV MMA that reads P from S buffer `buf` has been ISSUED: MMAs execute in issue order,
+  // so the next QK^T into that buffer may be issued without waiting for the PV MMA to complete)
   // Every barrier that is not waited on in every phase is split by parity of its use count: a waiter
   // may only test the parity of a phase when the barrier is known to be in that phase or the next.
-  auto bar_slot = [&](int slot, int which) { return bars + 8u * (5 * C::NSTAGE + 12 * slot + which); };
-  const uint32_t bar_qtempty = bars + 8u * (5 * C::NSTAGE + 24);
+  auto bar_slot = [&](int slot, int which) { return bars + 8u * (5 * C::NSTAGE + 14 * slot + which); };
+  const uint32_t bar_qtempty = bars + 8u * (5 * C::NSTAGE + 28);
   const uint32_t tmem_word = bars + 8u * C::NBARS;
   uint32_t* tmem_word_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_word - raw));
   uint8_t* sched = smem_raw + (tmem_word + 16 - raw);                  // [L * nparts] nibble pairs
@@ -359,6 +361,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       mbar_init(bar_slot(slot, 6), 1); mbar_init(bar_slot(slot, 7), 1);
       mbar_init(bar_slot(slot, 8), 128); mbar_init(bar_slot(slot, 9), 128);
       mbar_init(bar_slot(slot, 10), 1); mbar_init(bar_slot(slot, 11), 1);
+      mbar_init(bar_slot(slot, 12), 1); mbar_init(bar_slot(slot, 13), 1);
     }
     mbar_init(bar_qtempty, 128);
     fence_barrier_init();
@@ -470,8 +473,8 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           const int buf = nseq[slot] % C::NQBUF, use = nseq[slot] / C::NQBUF;
           if (es & kFirst) mbar_wait(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);       // Q tile rotated
           const int i = it[slot]++;
-          if (i >= 2) {     // S buffer (i & 1) is free once the PV MMA of item i - 2 has read its P
-            mbar_wait(bar_slot(slot, 10 + (i & 1)), (uint32_t)((i - 2) >> 1) & 1u);
+          if (i >= 2) {     // S buffer (i & 1) may be overwritten by MMAs issued after the PV MMA of item i - 2
+            mbar_wait(bar_slot(slot, 12 + (i & 1)), (uint32_t)((i - 2) >> 1) & 1u);
             tc_fence_after();
           }
           const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
@@ -526,6 +529,8 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
           umma_commit(bar_vempty(s));
           umma_commit(bar_slot(slot, 10 + (i & 1)));
+          tc_fence_before();
+          mbar_arrive(bar_slot(slot, 12 + (i & 1)));
         }
         __syncwarp();
         if (lane == 0) TRACE(10 + slot, g);
@@ -649,20 +654,24 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                   v[r][c] = __uint_as_float(bitsel(m_lo[c], sv[r * C::HX + c], sv[r * C::HX + c + C::HALF]));
             }
             // maximum of this query's valid logits of the part (log2 units)
-            auto part_max = [&]() {
+            // (csm: the scale as an opaque register, so that the compiler cannot hoist this rarely needed
+            // computation out of its branch into the exponential pass)
+            auto part_max = [&](float csm) {
               float cmax = -INFINITY;
 #pragma unroll
               for (int r = 0; r < R; ++r) {
                 float rmax = -INFINITY;
 #pragma unroll
-                for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[r][c] * cs : fmaf(v[r][c], cs, xz[c]));
+                for (int c = 0; c < C::HALF; ++c) rmax = fmaxf(rmax, C::FULLFOLD ? v[r][c] * csm : fmaf(v[r][c], csm, xz[c]));
                 if (r >= ya && r < yb) cmax = fmaxf(cmax, rmax);
               }
               return cmax;
             };
             if (__any_sync(0xffffffffu, ya < yb && !inited)) {
               // ---- first valid keys of some query: its reference is the true maximum of this part
-              const float cmax = part_max();
+              float cso = cs;
+              asm volatile("mov.f32 %0, %0;" : "+f"(cso));
+              const float cmax = part_max(cso);
               if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
             }
             float pr[R][C::HALF];                    // folded probabilities (times 2^-m_ref)
@@ -694,7 +703,9 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               // ---- a logit far above the reference: move the reference to the true maximum and
               // rescale what was accumulated so far (P of this part is not stored yet)
               const bool mine = !(rs <= kBig);
-              const float new_ref = mine ? fmaxf(m_ref, part_max()) : m_ref;
+              float cso = cs;
+              asm volatile("mov.f32 %0, %0;" : "+f"(cso));
+              const float new_ref = mine ? fmaxf(m_ref, part_max(cso)) : m_ref;
               const float alpha = new_ref != m_ref ? ex2(m_ref - new_ref) : 1.f;
               if (!first_item) {
                 // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
