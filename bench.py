@@ -221,6 +221,20 @@ class Session:
                                    self.ws_host)
 
 
+def max_over_ranks(torch, ms: float, dist, device) -> float:
+    """Whole-job step time = the slowest rank's (all-reduce MAX; identity when not distributed)."""
+    if dist is None:
+        return ms
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate(per_rank_units: float, world: int, ms: float) -> float:
+    """Replicas only: every rank processes the same units in `ms`; whole-job rate."""
+    return world * per_rank_units / (ms * 1e-3)
+
+
 def time_steps(torch, fn, steps, dist=None):
     if dist is not None:
         dist.barrier()
@@ -233,10 +247,8 @@ def time_steps(torch, fn, steps, dist=None):
     torch.cuda.synchronize()
     ms = s.elapsed_time(e) / steps
     if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = max_over_ranks(torch, ms, dist, "cuda")
         dist.barrier()
-        ms = float(t.item())
     return ms
 
 
@@ -289,8 +301,8 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
     per_kernel = {k: sum(v) / len(v) for k, v in per_kernel.items()}
     n_gpus = args.gpus
     flops, bytes_ = flops_of(w), w.compulsory_bytes()
-    tflops = n_gpus * flops / (ms * 1e-3) / 1e12
-    tok_s = n_gpus * w.batch * w.tokens / (ms * 1e-3)
+    tflops = aggregate(flops, n_gpus, ms) / 1e12
+    tok_s = aggregate(w.batch * w.tokens, n_gpus, ms)
     # roofline of the dominant kernel: all five configs are HBM-bound by SURVEY.md §8(d)
     dom = max(per_kernel, key=per_kernel.get) if per_kernel else None
     dom_ms = per_kernel.get(dom, ms)

@@ -139,6 +139,13 @@ int strata_na3d_last_launch_count(void);
 void strata_na3d_set_profiling(int enable);
 int strata_na3d_profile_read(float* ms, const char** names, int capacity);
 
+/* Host-side index helpers the kernels use, exported so that CPU tests can hold them against brute
+ * force.  strata_na3d_window_start: A3, first key of query i's window on an axis of n tokens with
+ * window k.  strata_na3d_inverse_window: B3, the queries whose window holds key j form the interval
+ * [*lo, *hi] (inclusive).  Both return -1 on invalid arguments (k < 1, k > n, index outside [0, n)). */
+int strata_na3d_window_start(int i, int k, int n);
+int strata_na3d_inverse_window(int j, int k, int n, int* lo, int* hi);
+
 const char* strata_status_string(strata_status_t status);
 int strata_version(void);
 

@@ -24,7 +24,7 @@ IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_TILE = 0, 1, 2, 3
 EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
            "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",
            "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
-           "strata_status_string", "strata_version")
+           "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_status_string", "strata_version")
 
 
 class StrataError(RuntimeError):
@@ -102,6 +102,10 @@ def lib() -> ctypes.CDLL:
         L.strata_na3d_set_profiling.argtypes = [i32]
         L.strata_na3d_profile_read.restype = i32
         L.strata_na3d_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_char_p), i32]
+        L.strata_na3d_window_start.restype = i32
+        L.strata_na3d_window_start.argtypes = [i32, i32, i32]
+        L.strata_na3d_inverse_window.restype = i32
+        L.strata_na3d_inverse_window.argtypes = [i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i32)]
         L.strata_status_string.restype = ctypes.c_char_p
         L.strata_status_string.argtypes = [i32]
         L.strata_version.restype = i32
@@ -136,6 +140,18 @@ def _stream_handle(stream) -> Optional[int]:
 # ------------------------------------------------------------------ 1:1 wrappers of the C entry points
 def strata_version() -> int:
     return int(lib().strata_version())
+
+
+def strata_na3d_window_start(i: int, k: int, n: int) -> int:
+    return int(lib().strata_na3d_window_start(int(i), int(k), int(n)))
+
+
+def strata_na3d_inverse_window(j: int, k: int, n: int):
+    """(lo, hi) inclusive, or None on invalid arguments."""
+    lo, hi = ctypes.c_int(0), ctypes.c_int(0)
+    if lib().strata_na3d_inverse_window(int(j), int(k), int(n), ctypes.byref(lo), ctypes.byref(hi)) != 0:
+        return None
+    return lo.value, hi.value
 
 
 def strata_na3d_workspace_bytes(desc: NA3DDesc, backward: bool = False) -> int:

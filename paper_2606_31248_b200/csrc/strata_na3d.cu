@@ -330,6 +330,17 @@ strata_status_t strata_na3d_bwd_host(const strata_na3d_desc_t* desc, const void*
 
 int strata_na3d_last_launch_count(void) { return g_last_launches; }
 
+int strata_na3d_window_start(int i, int k, int n) {
+  if (k < 1 || k > n || i < 0 || i >= n) return -1;
+  return strata::window_start(i, k, n);
+}
+
+int strata_na3d_inverse_window(int j, int k, int n, int* lo, int* hi) {
+  if (k < 1 || k > n || j < 0 || j >= n || !lo || !hi) return -1;
+  strata::inverse_window(j, k, n, *lo, *hi);
+  return 0;
+}
+
 const char* strata_status_string(strata_status_t s) {
   switch (s) {
     case STRATA_OK: return "ok";

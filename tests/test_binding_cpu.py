@@ -66,6 +66,41 @@ def test_status_codes_without_touching_the_gpu(L):
     assert bw(d, ok11[:9] + [None, vp(0x1000)], vp(0x1000), 1 << 30) == 1
 
 
+def test_window_and_inverse_window_against_brute_force(L):
+    """A3 / B3 as the kernels compute them (csrc/common.cuh) against the definition by enumeration:
+    "centre the window on the query, then shift it inward until it fits" (PAPER.md:79 + reading R1),
+    and the inverse neighbourhood read off that enumeration (no formula)."""
+    for line in open(os.path.join(ROOT, "tests", "golden", "window_starts.txt")):      # hand-derived fixture
+        if line.startswith("#") or not line.strip():
+            continue
+        kn, st, cnt = (list(map(int, part.split())) for part in line.split("|"))
+        k, n = kn
+        assert [binding.strata_na3d_window_start(i, k, n) for i in range(n)] == st
+        inv = [binding.strata_na3d_inverse_window(j, k, n) for j in range(n)]
+        assert [h - l + 1 for l, h in inv] == cnt
+    for n in range(1, 41):
+        for k in range(1, n + 1):
+            starts = []
+            for i in range(n):
+                s = i - k // 2                      # centred ...
+                while s < 0:
+                    s += 1                          # ... shifted inward at the low border
+                while s + k > n:
+                    s -= 1                          # ... and at the high border
+                starts.append(s)
+                assert binding.strata_na3d_window_start(i, k, n) == s, (i, k, n)
+            for j in range(n):
+                attending = [i for i in range(n) if starts[i] <= j < starts[i] + k]
+                assert attending == list(range(attending[0], attending[-1] + 1))   # an interval
+                assert binding.strata_na3d_inverse_window(j, k, n) == (attending[0], attending[-1]), (j, k, n)
+    assert binding.strata_na3d_window_start(0, 5, 4) == -1 and binding.strata_na3d_inverse_window(4, 3, 4) is None
+    # hand-derived values of SURVEY.md §8(c): (k, n) = (3, 8) and (5, 8)
+    assert [binding.strata_na3d_window_start(i, 3, 8) for i in range(8)] == [0, 0, 1, 2, 3, 4, 5, 5]
+    assert [binding.strata_na3d_window_start(i, 5, 8) for i in range(8)] == [0, 0, 0, 1, 2, 3, 3, 3]
+    counts = lambda k, n: [h - l + 1 for l, h in (binding.strata_na3d_inverse_window(j, k, n) for j in range(n))]
+    assert counts(3, 8) == [2, 3, 4, 3, 3, 4, 3, 2] and counts(5, 8) == [3, 4, 5, 8, 8, 5, 4, 3]
+
+
 def test_no_cpu_fallback():
     import torch
     q = torch.zeros(1, 2, 2, 2, 1, 32)
