@@ -80,19 +80,85 @@ rope_table_kernel(uint2* __restrict__ table, const float* __restrict__ coords, c
   if (gid >= tokens * quarter) return;
   const long long t = gid / quarter;
   const int m = 2 * (int)(gid - t * quarter);
+  // The table is rounded to bf16 (2^-9): an fp32 angle (|phi| <~ 2e3 rad -> 1e-4 rad of rounding), a two-term
+  // Cody-Waite reduction to [-pi, pi] and the MUFU sin / cos (2^-21 abs on that range) are far inside that.
   float cs[2], sn[2];
 #pragma unroll
   for (int u = 0; u < 2; ++u) {
-    double phi = 0.0;
-    for (int a = 0; a < A; ++a) phi += (double)coords[t * A + a] * (double)freqs[a * half + m + u];
-    const double r = phi - 6.283185307179586477 * rint(phi * 0.15915494309189533577);
-    sincosf((float)r, &sn[u], &cs[u]);
+    float phi = 0.f;
+    for (int a = 0; a < A; ++a) phi = fmaf(coords[t * A + a], freqs[a * half + m + u], phi);
+    const float n = rintf(phi * 0.15915494309189535f);
+    const float r = fmaf(n, 1.7484555e-7f, fmaf(n, -6.2831854820251465f, phi));    // 2 pi = 6.2831854820251465 - 1.7484555e-7
+    __sincosf(r, &sn[u], &cs[u]);
   }
   const __nv_bfloat162 c2 = __floats2bfloat162_rn(cs[0], cs[1]), s2 = __floats2bfloat162_rn(sn[0], sn[1]);
   uint2 w;
   w.x = *reinterpret_cast<const uint32_t*>(&c2);
   w.y = *reinterpret_cast<const uint32_t*>(&s2);
   table[gid] = w;
+}
+
+// A1 + A2 for bf16 -> bf16 (the operands of the tensor-core kernels that take pre-rotated Q, K): 16-byte
+// accesses, one thread per (token, group of 8 channels) looping over the heads and both tensors with the
+// group's cos / sin in registers.  The result is rounded to bf16 (2^-9), so the angle is reduced and
+// evaluated in fp32 (two-term Cody-Waite, MUFU sin / cos: ~1e-4 abs at |phi| ~ 2e3 rad).
+// PAIR 0: group = channels [8g, 8g+8) = pairs 4g .. 4g+3.  PAIR 1: group = pairs 8g .. 8g+7, i.e. channels
+// [8g, 8g+8) and [D/2 + 8g, D/2 + 8g + 8).
+template <int PAIR>
+__global__ void __launch_bounds__(256)
+rope_rotate_bf16_kernel(const __nv_bfloat16* __restrict__ x0, const __nv_bfloat16* __restrict__ x1,
+                        __nv_bfloat16* __restrict__ y0, __nv_bfloat16* __restrict__ y1, const float* __restrict__ coords,
+                        const float* __restrict__ freqs, long long tokens, int H, int D, int A, float sign) {
+  constexpr int NP = PAIR ? 8 : 4;
+  const int half = D >> 1, groups = half / NP;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= tokens * groups) return;
+  const long long t = gid / groups;
+  const int g = (int)(gid - t * groups);
+  float cs[NP], sn[NP];
+#pragma unroll
+  for (int u = 0; u < NP; ++u) {
+    float phi = 0.f;
+    for (int a = 0; a < A; ++a) phi = fmaf(coords[t * A + a], freqs[a * half + NP * g + u], phi);
+    const float n = rintf(phi * 0.15915494309189535f);
+    const float r = fmaf(n, 1.7484555e-7f, fmaf(n, -6.2831854820251465f, phi));
+    __sincosf(r, &sn[u], &cs[u]);
+    sn[u] *= sign;
+  }
+  for (int h = 0; h < H; ++h) {
+    const long long base = (t * H + h) * (long long)D;
+#pragma unroll
+    for (int which = 0; which < 2; ++which) {
+      const __nv_bfloat16* x = which ? x1 : x0;
+      __nv_bfloat16* y = which ? y1 : y0;
+      if (x == nullptr) continue;
+      if (PAIR == 0) {
+        uint4 v = *reinterpret_cast<const uint4*>(x + base + 8 * g);
+        uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float2 ab = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&w[u]));
+          const __nv_bfloat162 r2 = __floats2bfloat162_rn(ab.x * cs[u] - ab.y * sn[u], ab.x * sn[u] + ab.y * cs[u]);
+          w[u] = *reinterpret_cast<const uint32_t*>(&r2);
+        }
+        *reinterpret_cast<uint4*>(y + base + 8 * g) = make_uint4(w[0], w[1], w[2], w[3]);
+      } else {
+        uint4 va = *reinterpret_cast<const uint4*>(x + base + 8 * g), vb = *reinterpret_cast<const uint4*>(x + base + half + 8 * g);
+        uint32_t wa[4] = {va.x, va.y, va.z, va.w}, wb[4] = {vb.x, vb.y, vb.z, vb.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[u]));
+          const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[u]));
+          const __nv_bfloat162 ra = __floats2bfloat162_rn(a2.x * cs[2 * u] - b2.x * sn[2 * u], a2.y * cs[2 * u + 1] - b2.y * sn[2 * u + 1]);
+          const __nv_bfloat162 rb = __floats2bfloat162_rn(a2.x * sn[2 * u] + b2.x * cs[2 * u], a2.y * sn[2 * u + 1] + b2.y * cs[2 * u + 1]);
+          wa[u] = *reinterpret_cast<const uint32_t*>(&ra);
+          wb[u] = *reinterpret_cast<const uint32_t*>(&rb);
+        }
+        *reinterpret_cast<uint4*>(y + base + 8 * g) = make_uint4(wa[0], wa[1], wa[2], wa[3]);
+        *reinterpret_cast<uint4*>(y + base + half + 8 * g) = make_uint4(wb[0], wb[1], wb[2], wb[3]);
+      }
+    }
+  }
 }
 
 // A1 as an fp32 table for the backward epilogues (B4): table[t][j] = (cos phi[t][j], sin phi[t][j]).
@@ -149,6 +215,19 @@ cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1,
   const long long grid = (threads + block - 1) / block;
   if (grid <= 0 || grid > 0x7fffffffLL) return cudaErrorInvalidValue;
   prof_begin(sign > 0 ? "rope_rotate" : "rope_unrotate", stream);
+  if (in_dtype == 1 && out_dtype == 1 && (p.D % 16) == 0) {       // vectorised bf16 -> bf16 path
+    const int np = p.pairing ? 8 : 4;
+    const long long vthreads = tokens * (p.D / 2 / np), vgrid = (vthreads + block - 1) / block;
+    if (p.pairing)
+      rope_rotate_bf16_kernel<1><<<(unsigned)vgrid, block, 0, stream>>>((const __nv_bfloat16*)x0, (const __nv_bfloat16*)x1,
+          (__nv_bfloat16*)y0, (__nv_bfloat16*)y1, coords, freqs, tokens, p.H, p.D, p.A, sign);
+    else
+      rope_rotate_bf16_kernel<0><<<(unsigned)vgrid, block, 0, stream>>>((const __nv_bfloat16*)x0, (const __nv_bfloat16*)x1,
+          (__nv_bfloat16*)y0, (__nv_bfloat16*)y1, coords, freqs, tokens, p.H, p.D, p.A, sign);
+    prof_end(stream);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+  }
 #define STRATA_ROPE(TI, TO)                                                                        \
   rope_rotate_kernel<TI, TO><<<(unsigned)grid, block, 0, stream>>>(                                \
       (const TI*)x0, (const TI*)x1, (TO*)y0, (TO*)y1, coords, freqs, tokens, p.H, p.D, p.A,        \
