@@ -70,7 +70,7 @@ struct FusedCfg {
   static constexpr int NQBUF = (D == 64) ? 2 : 1;                  // Q buffers per slot
   static constexpr int TMEM_SLOT = 256, TMEM_O = 0, TMEM_S = D;
   static constexpr int NBARS = 5 * NSTAGE + 2 * 14 + 1;
-  static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 512;
+  static constexpr int SMEM_BYTES = 1024 + (2 * NQBUF + 1) * Q_BYTES + 3 * NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 3 * 512;
   static constexpr bool FULLFOLD = (KX == HALF);                   // exactly one of the columns c, c + HALF is in the window
   static_assert(TL * TY * TX == 128 && (TY * TX) % 32 == 0 && TY == 2 * G, "128 queries per tile, one level per warp, two warps per level");
   static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1 && TX % 2 == 0 && KY >= 3, "odd windows only (HX even)");
@@ -88,6 +88,7 @@ struct FusedParams {
   long long N;
   float scale_log2e;
   int rope;       // 0: no rotation (rope_axes == 0)
+  int ncols;      // level columns = B * H * nty * ntx; CTA c owns columns c, c + gridDim.x, ... (persistent)
 #ifdef STRATA_TRACE
   unsigned long long* trace;   // debug: clock64 stamps of one CTA, [event][index]
   int trace_cta;
@@ -325,25 +326,35 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-  // ---- the level column of this CTA: head fastest (the H heads of a token are one contiguous
-  // H*D*2-byte run in HBM), then x, y, sample
-  int bid = blockIdx.x;
-  const int h = bid % p.H; bid /= p.H;
-  const int tx = bid % p.ntx; bid /= p.ntx;
-  const int ty = bid % p.nty;
-  const int b = bid / p.nty;
-  const int x0 = tx * C::TX, y0 = ty * C::TY;
-  const int yl = min(y0 + C::TY, p.Y) - 1;
-  const int hs_x = window_start(x0, C::KX, p.X), hs_y = window_start(y0, C::KY, p.Y);
-  const int hy = window_start(yl, C::KY, p.Y) + C::KY - hs_y;     // key rows of the halo, <= HY
-  const int nparts = hy > C::part_begin(2) ? 3 : hy > C::part_begin(1) ? 2 : 1;
-  const int nchunks = p.L * nparts;
+  // ---- geometry of one level column: head fastest (the H heads of a token are one contiguous
+  // H*D*2-byte run in HBM), then x, y, sample.  The CTA is persistent: it owns columns blockIdx.x,
+  // blockIdx.x + gridDim.x, ...; every pipeline counter (stage ring position, items, tiles, Q jobs)
+  // keeps running across columns, so the next column's loads, rotations and MMAs overlap the drain of
+  // the previous one.
+  struct Col {
+    int h, b, x0, y0, hs_x, hs_y, hy, nparts, nchunks, bl;
+  };
+  auto column = [&](int col) {
+    Col c;
+    int bid = col;
+    c.h = bid % p.H; bid /= p.H;
+    const int tx = bid % p.ntx; bid /= p.ntx;
+    const int ty = bid % p.nty;
+    c.b = bid / p.nty;
+    c.x0 = tx * C::TX; c.y0 = ty * C::TY;
+    const int yl = min(c.y0 + C::TY, p.Y) - 1;
+    c.hs_x = window_start(c.x0, C::KX, p.X); c.hs_y = window_start(c.y0, C::KY, p.Y);
+    c.hy = window_start(yl, C::KY, p.Y) + C::KY - c.hs_y;     // key rows of the halo, <= HY
+    c.nparts = c.hy > C::part_begin(2) ? 3 : c.hy > C::part_begin(1) ? 2 : 1;
+    c.nchunks = p.L * c.nparts;
+    c.bl = c.b * p.L;
+    return c;
+  };
   const int ntl = (p.L + C::TL - 1) / C::TL;
-  const int bl = b * p.L;
   const uint32_t op_tx = p.rope ? 2u : 1u;                        // operand + table bytes per barrier
-  // rows of part `part` that exist in this halo, and the rows its TMA box brings in
-  auto part_rows = [&](int part) { return min(C::part_begin(part + 1), hy) - C::part_begin(part); };
   auto box_rows = [&](int part) { return part == 1 ? C::RB : C::RA; };
+  // schedule tables, one per possible number of parts: sched_of(nparts)[plane * nparts + part]
+  auto sched_of = [&](int nparts) { return sched + kMaxChunks * (nparts - 1); };
 
   // ---- one-time setup
   if (warp == kWarpTma && lane == 0) {
@@ -367,20 +378,21 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     fence_barrier_init();
   }
   if (warp == kWarpTma) tmem_alloc(tmem_word, 512);
-  // schedule table: which slot needs part g, and whether it is the first / last part of its tile
-  for (int g = threadIdx.x; g < nchunks; g += kFusedThreads) {
-    const int plane = g / nparts, part = g - plane * nparts;
-    uint32_t e = 0;
-    for (int t = 0; t < ntl; ++t) {
-      const int lo = SlotWalk<C>::plo(t, p.L), hi = SlotWalk<C>::phi(t, p.L);
-      if (plane < lo || plane >= hi) continue;
-      uint32_t f = kNeeded;
-      if (plane == lo && part == 0) f |= kFirst;
-      if (plane == hi - 1 && part == nparts - 1) f |= kLast;
-      e |= f << (4 * (t & 1));
+  // schedule tables: which slot needs part g, and whether it is the first / last part of its tile
+  for (int np = 1; np <= C::NPARTS; ++np)
+    for (int g = threadIdx.x; g < p.L * np; g += kFusedThreads) {
+      const int plane = g / np, part = g - plane * np;
+      uint32_t e = 0;
+      for (int t = 0; t < ntl; ++t) {
+        const int lo = SlotWalk<C>::plo(t, p.L), hi = SlotWalk<C>::phi(t, p.L);
+        if (plane < lo || plane >= hi) continue;
+        uint32_t f = kNeeded;
+        if (plane == lo && part == 0) f |= kFirst;
+        if (plane == hi - 1 && part == np - 1) f |= kLast;
+        e |= f << (4 * (t & 1));
+      }
+      sched_of(np)[g] = (uint8_t)e;
     }
-    sched[g] = (uint8_t)e;
-  }
   // V stages start as zeros: rows of a stage that a (shorter) part does not overwrite are multiplied
   // by P = 0 in the PV MMA and must therefore hold finite numbers.
   for (uint32_t off = threadIdx.x * 16u; off < (uint32_t)(C::NSTAGE * C::STAGE_BYTES); off += kFusedThreads * 16u)
@@ -395,75 +407,86 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     reg_dec<56>();
     if (warp == kWarpTma) {
       // =========================== TMA producer ===========================
-      {
-        int nseq[2] = {0, 0};
-        int qjob = 0, part = 0, plane = 0;
-        for (int g = 0; g < nchunks; ++g) {
-          const uint32_t e = sched[g];
+      int nrun[2] = {0, 0};                                           // tiles of each slot so far (all columns)
+      int qjob = 0, gbase = 0;
+      for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
+        const Col c = column(col);
+        const uint8_t* sc = sched_of(c.nparts);
+        int nloc[2] = {0, 0};                                         // tiles of each slot in this column
+        int part = 0, plane = 0;
+        for (int g = 0; g < c.nchunks; ++g) {
+          const uint32_t e = sc[g];
 #pragma unroll
           for (int slot = 0; slot < 2; ++slot) {
             if (!((e >> (4 * slot)) & kFirst)) continue;
-            const int n = nseq[slot]++;                               // tiles of this slot so far
+            const int n = nrun[slot]++;
             const int buf = n % C::NQBUF, use = n / C::NQBUF;         // use-th tile in this Q buffer
             if (use >= 1) mbar_wait(bar_slot(slot, 4 + buf), (uint32_t)(use - 1) & 1u);   // its last QK^T is done
             if (p.rope && qjob >= 1) mbar_wait(bar_qtempty, (uint32_t)(qjob - 1) & 1u);
             const uint32_t bar = bar_slot(slot, buf);
             const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
-            const int l0 = bl + C::TL * (slot + 2 * n);
+            const int l0 = c.bl + C::TL * (slot + 2 * nloc[slot]++);
             if (elect_one()) {
               mbar_expect_tx(bar, op_tx * C::Q_BYTES);
 #pragma unroll
               for (int j = 0; j < C::DSUB; ++j) {
-                tma_load_5d(qb + j * C::SUB_Q, &tm_q, bar, 64 * j, h, x0, y0, l0);
-                if (p.rope) tma_load_5d(qt_smem + j * C::SUB_Q, &tm_tq, bar, 64 * j, 0, x0, y0, l0);
+                tma_load_5d(qb + j * C::SUB_Q, &tm_q, bar, 64 * j, c.h, c.x0, c.y0, l0);
+                if (p.rope) tma_load_5d(qt_smem + j * C::SUB_Q, &tm_tq, bar, 64 * j, 0, c.x0, c.y0, l0);
               }
             }
             __syncwarp();
             ++qjob;
           }
-          const int s = g % C::NSTAGE;
-          const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+          const int G = gbase + g;
+          const int s = G % C::NSTAGE;
+          const uint32_t ph = (uint32_t)(G / C::NSTAGE) & 1u;
           const bool mid = part == 1;
           const uint32_t bytes = (uint32_t)(box_rows(part) * C::HX * 128 * C::DSUB);
-          const int cy0 = hs_y + C::part_begin(part);
+          const int cy0 = c.hs_y + C::part_begin(part);
           mbar_wait(bar_kempty(s), ph ^ 1u);
-          if (lane == 0) TRACE(0, g);
+          if (lane == 0) TRACE(0, G);
           if (elect_one()) {
             mbar_expect_tx(bar_kfull(s), op_tx * bytes);
 #pragma unroll
             for (int j = 0; j < C::DSUB; ++j) {
-              tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_kb : &tm_ka, bar_kfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+              tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_kb : &tm_ka, bar_kfull(s), 64 * j, c.h, c.hs_x, cy0, c.bl + plane);
               if (p.rope)
-                tma_load_5d(t_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_tb : &tm_ta, bar_kfull(s), 64 * j, 0, hs_x, cy0, bl + plane);
+                tma_load_5d(t_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_tb : &tm_ta, bar_kfull(s), 64 * j, 0, c.hs_x, cy0, c.bl + plane);
             }
           }
           __syncwarp();
           mbar_wait(bar_vempty(s), ph ^ 1u);
-          if (lane == 0) TRACE(1, g);
+          if (lane == 0) TRACE(1, G);
           if (elect_one()) {
             mbar_expect_tx(bar_vfull(s), bytes);
 #pragma unroll
             for (int j = 0; j < C::DSUB; ++j)
-              tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_vb : &tm_va, bar_vfull(s), 64 * j, h, hs_x, cy0, bl + plane);
+              tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_vb : &tm_va, bar_vfull(s), 64 * j, c.h, c.hs_x, cy0, c.bl + plane);
           }
           __syncwarp();
-          if (++part == nparts) { part = 0; ++plane; }
+          if (++part == c.nparts) { part = 0; ++plane; }
         }
+        gbase += c.nchunks;
       }
     } else if (warp == kWarpQk) {
       // =========================== QK^T issuer (both slots) ===========================
       // The whole warp walks the schedule in uniform control flow (descriptors stay in uniform
       // registers); one elected lane issues the MMAs and commits.
       int it[2] = {0, 0}, nseq[2] = {-1, -1};
+      int gbase = 0;
+      for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
+      const Col c = column(col);
+      const uint8_t* sc = sched_of(c.nparts);
       int part = 0;
-      for (int g = 0; g < nchunks; ++g) {
-        const uint32_t e = sched[g];
-        const int s = g % C::NSTAGE;
-        const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+      for (int g = 0; g < c.nchunks; ++g) {
+        const uint32_t e = sc[g];
+        const int G = gbase + g;
+        const int s = G % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(G / C::NSTAGE) & 1u;
         const uint32_t idesc_qk = part == 1 ? instr_desc(C::M, C::NB, false) : instr_desc(C::M, C::NA, false);
-        if (++part == nparts) part = 0;
+        if (++part == c.nparts) part = 0;
         mbar_wait(bar_krot(s), ph);
-        if (lane == 0) TRACE(4, g);
+        if (lane == 0) TRACE(4, G);
         tc_fence_after();
 #pragma unroll
         for (int slot = 0; slot < 2; ++slot) {
@@ -490,23 +513,30 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             if (es & kLast) umma_commit(bar_slot(slot, 4 + buf));    // every QK^T of the tile is done: Q buffer free
           }
           __syncwarp();
-          if (lane == 0) TRACE(6 + slot, g);
+          if (lane == 0) TRACE(6 + slot, G);
         }
         if (elect_one()) umma_commit(bar_kempty(s));                 // both slots' QK^T of this part
         __syncwarp();
+      }
+      gbase += c.nchunks;
       }
     } else {
       // =========================== PV issuer of one slot ===========================
       const int slot = warp - kWarpPv;
       const uint32_t tm = tmem + slot * C::TMEM_SLOT;
       constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
-      int i = 0, part = 0;
-      for (int g = 0; g < nchunks; ++g) {
-        const uint32_t es = (sched[g] >> (4 * slot)) & 15u;
-        const int s = g % C::NSTAGE;
-        const uint32_t ph = (uint32_t)(g / C::NSTAGE) & 1u;
+      int i = 0, gbase = 0;
+      for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
+      const Col c = column(col);
+      const uint8_t* sc = sched_of(c.nparts);
+      int part = 0;
+      for (int g = 0; g < c.nchunks; ++g) {
+        const uint32_t es = (sc[g] >> (4 * slot)) & 15u;
+        const int G = gbase + g;
+        const int s = G % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(G / C::NSTAGE) & 1u;
         const int nk = (part == 1 ? C::NB : C::NA) / 16;
-        if (++part == nparts) part = 0;
+        if (++part == c.nparts) part = 0;
         if (!(es & kNeeded)) {        // this slot does not use the part: release it once it has landed
           mbar_wait(bar_vfull(s), ph);        // (one arrival per slot and phase, never ahead of the producer)
           if (elect_one()) mbar_arrive(bar_vempty(s));
@@ -514,7 +544,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           continue;
         }
         mbar_wait(bar_slot(slot, 8 + (i & 1)), (uint32_t)(i >> 1) & 1u);       // P of item i is in TMEM
-        if (lane == 0) TRACE(8 + slot, g);
+        if (lane == 0) TRACE(8 + slot, G);
         mbar_wait(bar_vfull(s), ph);
         tc_fence_after();
         const uint32_t a_tmem = tm + C::TMEM_S + (i & 1) * C::NMAX;
@@ -533,8 +563,10 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           mbar_arrive(bar_slot(slot, 12 + (i & 1)));
         }
         __syncwarp();
-        if (lane == 0) TRACE(10 + slot, g);
+        if (lane == 0) TRACE(10 + slot, G);
         ++i;
+      }
+      gbase += c.nchunks;
       }
     }
   } else if (warp >= kWarpRot) {
@@ -542,10 +574,15 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     reg_dec<88>();
     const int tid = threadIdx.x - 32 * kWarpRot;
     int nseq[2] = {0, 0};
+    int gbase = 0;
+    for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
+    const Col c = column(col);
+    const uint8_t* sc = sched_of(c.nparts);
     int part = 0;
-    for (int g = 0; g < nchunks; ++g) {
-      const uint32_t e = sched[g];
-      const int s = g % C::NSTAGE;
+    for (int g = 0; g < c.nchunks; ++g) {
+      const uint32_t e = sc[g];
+      const int G = gbase + g;
+      const int s = G % C::NSTAGE;
       // jobs of this step, all through ONE copy of the rotation code: the Q tile of a slot that
       // starts a tile here (job 0 / 1), then the K part (job 2)
 #pragma unroll 1
@@ -561,19 +598,21 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         } else {
           x_addr = k_smem + s * C::STAGE_BYTES; t_addr = t_smem + s * C::STAGE_BYTES; sub_stride = C::SUB_KV;
           rows = box_rows(part) * C::HX;
-          bar_in = bar_kfull(s); ph_in = (uint32_t)(g / C::NSTAGE) & 1u; bar_out = bar_krot(s);
+          bar_in = bar_kfull(s); ph_in = (uint32_t)(G / C::NSTAGE) & 1u; bar_out = bar_krot(s);
         }
         mbar_wait(bar_in, ph_in);                          // operand (+ table) landed
-        if (tid == 0 && job == 2) TRACE(2, g);
+        if (tid == 0 && job == 2) TRACE(2, G);
         if (p.rope) {
           rotate_inplace<C::DSUB, PAIR>(x_addr, t_addr, sub_stride, rows, tid);
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           if (job < 2) mbar_arrive(bar_qtempty);
         }
-        if (tid == 0 && job == 2) TRACE(3, g);
+        if (tid == 0 && job == 2) TRACE(3, G);
         mbar_arrive(bar_out);
       }
-      if (++part == nparts) part = 0;
+      if (++part == c.nparts) part = 0;
+    }
+    gbase += c.nchunks;
     }
   } else {
     // =========================== softmax + epilogue of one slot ===========================
@@ -583,12 +622,17 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int row = sp * 32 + lane;                // query row of the tile == TMEM lane
     const uint32_t tm = tmem + slot * C::TMEM_SLOT + ((uint32_t)(sp * 32) << 16);
     const int qx = row % C::TX, qy = (row / C::TX) % C::TY, ql = row / (C::TX * C::TY);
+    const float cs = p.scale_log2e;
+    int i = 0;
+    for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
+    const Col c = column(col);
+    const int x0 = c.x0, y0 = c.y0, hs_x = c.hs_x, hs_y = c.hs_y, hy = c.hy, nparts = c.nparts, h = c.h, b = c.b;
+    auto part_rows = [&](int part) { return min(C::part_begin(part + 1), hy) - C::part_begin(part); };
     const int ax = min(x0 + qx, p.X - 1), ay = min(y0 + qy, p.Y - 1);
     const bool active_xy = (x0 + qx < p.X) && (y0 + qy < p.Y);
     const int lo_x = window_start(ax, C::KX, p.X) - hs_x;
     const int lo_y = window_start(ay, C::KY, p.Y) - hs_y;
     const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
-    const float cs = p.scale_log2e;
     // x fold: of the halo columns c and c + HALF at most one lies in this query's window
     uint32_t m_lo[C::HALF];                        // all ones: column c is the one (else c + HALF, or neither)
     float xz[C::HALF];                             // 0 if one of the two is in the window, else -inf
@@ -613,7 +657,6 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       psel[j] = n0 | (n1 << 8);
     }
 
-    int i = 0;
     for (int tile = slot; tile < ntl; tile += 2) {
       const int al = min(C::TL * tile + ql, p.L - 1);
       const bool active = active_xy && (C::TL * tile + ql < p.L);
@@ -785,6 +828,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // the O reads above are complete before the next tile's first PV MMA overwrites O: that MMA
       // waits for this warpgroup's next p_full arrival, which follows these (waited-for) loads.
     }
+    }
   }
 
   // ---- teardown
@@ -840,8 +884,19 @@ cudaError_t launch_fused(const Problem& p, const void* q, const void* k, const v
     fp.trace_cta = c ? atoi(c) : 0;
   }
 #endif
-  const long long grid = (long long)p.B * p.H * fp.nty * fp.ntx;
-  if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+  const long long ncols = (long long)p.B * p.H * fp.nty * fp.ntx;
+  if (ncols > 0x7fffffffLL) return cudaErrorInvalidValue;
+  fp.ncols = (int)ncols;
+  static int sm_count = 0;
+  if (sm_count == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        sm_count <= 0) {
+      (void)cudaGetLastError();
+      sm_count = 148;
+    }
+  }
+  const long long grid = ncols < sm_count ? ncols : sm_count;      // persistent: one CTA per SM
   auto kernel = p.pairing ? na3d_fwd_fused_kernel<C, 1> : na3d_fwd_fused_kernel<C, 0>;
   static bool attr_set[2] = {false, false};
   if (!attr_set[p.pairing ? 1 : 0]) {
