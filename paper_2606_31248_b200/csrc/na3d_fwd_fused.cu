@@ -600,6 +600,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           rows = box_rows(part) * C::HX;
           bar_in = bar_kfull(s); ph_in = (uint32_t)(G / C::NSTAGE) & 1u; bar_out = bar_krot(s);
         }
+        if (tid == 0 && job == 2) TRACE(5, G);
         mbar_wait(bar_in, ph_in);                          // operand (+ table) landed
         if (tid == 0 && job == 2) TRACE(2, G);
         if (p.rope) {

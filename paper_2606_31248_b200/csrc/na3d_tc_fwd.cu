@@ -14,7 +14,7 @@
 // Pipelines (mbarriers): K/V stage full/empty (TMA <-> MMA), s_full (MMA1 -> softmax),
 // p_full (softmax -> MMA2), pv_done (MMA2 -> O rescale / epilogue).
 //
-// TMEM columns: O [0, D) fp32 | S [D, D+128) fp32 | P [D+128, D+192) bf16x2 (A operand of MMA2).
+// TMEM columns: O [0, D) fp32 | S [D, D+NKEY) fp32, overwritten by P (bf16x2, A operand of MMA2).
 #include "tc_common.cuh"
 
 namespace strata {
@@ -30,14 +30,15 @@ struct Cfg {
   static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
   static constexpr int TL = 2, TY = 8, TX = 8, M = 128;            // query tile
   static constexpr int HL = TL + KL - 1, HY = TY + KY - 1, HX = TX + KX - 1;   // halo box
-  static constexpr int CY = 8;                                     // key rows per chunk
+  static constexpr int CY = (D == 128) ? 4 : 8;                    // key rows per chunk (d = 128: small stages, two CTAs per SM)
   static constexpr int NKEY = CY * HX;                             // keys per chunk (UMMA N of S)
   static constexpr int DSUB = D / 64;                              // 128-byte sub-tiles per row
   static constexpr int SUB_Q = M * 128, SUB_KV = NKEY * 128;       // bytes of one sub-tile
   static constexpr int Q_BYTES = DSUB * SUB_Q, STAGE_BYTES = DSUB * SUB_KV;
   static constexpr int NSTAGE = (2 * 3 * STAGE_BYTES + Q_BYTES <= 110 * 1024) ? 3 : 2;
-  static constexpr int TMEM_O = 0, TMEM_S = D, TMEM_P = D + 128;
-  static constexpr int TMEM_COLS = (D + 192 <= 256) ? 256 : 512;
+  // P (bf16 pairs) overlays the front of S: every S column of a chunk is in registers before P is stored
+  static constexpr int TMEM_O = 0, TMEM_S = D, TMEM_P = D;
+  static constexpr int TMEM_COLS = (D + NKEY <= 256) ? 256 : 512;
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = 1024 + Q_BYTES + 2 * NSTAGE * STAGE_BYTES + BAR_BYTES;
   static constexpr int CTAS_PER_SM = (2 * SMEM_BYTES <= 227 * 1024 && TMEM_COLS == 256) ? 2 : 1;
