@@ -97,6 +97,19 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def measured_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu captures
+    (profiles/*traffic.csv: workload,kernel,dram_bytes_per_launch,capture); None if never captured."""
+    import csv
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*traffic.csv")), reverse=True):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == kernel:
+                    return float(row["dram_bytes_per_launch"])
+    return None
+
+
 def flops_of(w: wl.Workload) -> float:
     return w.useful_flops()
 
@@ -310,7 +323,7 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
     t_tc = flops / (peaks["bf16_tflops"] * 1e12)
     achieved = bytes_ / (dom_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "kernel_ms": dom_ms, "achieved": achieved, "peak": peaks["hbm_gbs"],
-                "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": None,
+                "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": measured_traffic(w.name, dom),
                 "peak_source": peaks["source"], "algorithmic_bytes": bytes_,
                 "roofline_ms": max(t_hbm, t_tc) * 1e3, "step_frac_of_roofline": max(t_hbm, t_tc) * 1e3 / ms,
                 "kernels_ms": per_kernel}
@@ -336,7 +349,7 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))

@@ -149,6 +149,13 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
+// One mbarrier arrival per WARP (barrier counts are in warps): every lane has made its own writes visible
+// (fence.proxy.async / tcgen05.wait::st + tcgen05.fence::before_thread_sync) before the warp barrier; the
+// arrival of lane 0 releases them cumulatively.  128 per-thread arrivals serialise in the barrier unit.
+__device__ __forceinline__ void warp_arrive(uint32_t bar) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
@@ -362,19 +369,19 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     tma_prefetch_desc(&tm_va); tma_prefetch_desc(&tm_vb);
     if (p.rope) { tma_prefetch_desc(&tm_tq); tma_prefetch_desc(&tm_ta); tma_prefetch_desc(&tm_tb); }
     for (int s = 0; s < C::NSTAGE; ++s) {
-      mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 128); mbar_init(bar_kempty(s), 1);
+      mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 4); mbar_init(bar_kempty(s), 1);
       mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 2);
     }
     for (int slot = 0; slot < 2; ++slot) {
       mbar_init(bar_slot(slot, 0), 1); mbar_init(bar_slot(slot, 1), 1);
-      mbar_init(bar_slot(slot, 2), 128); mbar_init(bar_slot(slot, 3), 128);
+      mbar_init(bar_slot(slot, 2), 4); mbar_init(bar_slot(slot, 3), 4);
       mbar_init(bar_slot(slot, 4), 1); mbar_init(bar_slot(slot, 5), 1);
       mbar_init(bar_slot(slot, 6), 1); mbar_init(bar_slot(slot, 7), 1);
-      mbar_init(bar_slot(slot, 8), 128); mbar_init(bar_slot(slot, 9), 128);
+      mbar_init(bar_slot(slot, 8), 4); mbar_init(bar_slot(slot, 9), 4);
       mbar_init(bar_slot(slot, 10), 1); mbar_init(bar_slot(slot, 11), 1);
       mbar_init(bar_slot(slot, 12), 1); mbar_init(bar_slot(slot, 13), 1);
     }
-    mbar_init(bar_qtempty, 128);
+    mbar_init(bar_qtempty, 4);
     fence_barrier_init();
   }
   if (warp == kWarpTma) tmem_alloc(tmem_word, 512);
@@ -606,10 +613,10 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         if (p.rope) {
           rotate_inplace<C::DSUB, PAIR>(x_addr, t_addr, sub_stride, rows, tid);
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          if (job < 2) mbar_arrive(bar_qtempty);
+          if (job < 2) warp_arrive(bar_qtempty);
         }
         if (tid == 0 && job == 2) TRACE(3, G);
-        mbar_arrive(bar_out);
+        warp_arrive(bar_out);
       }
       if (++part == c.nparts) part = 0;
     }
@@ -802,7 +809,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           tmem_wait_st();
           tc_fence_before();
           if (sp == 0 && lane == 0) TRACE(14 + slot, i);
-          mbar_arrive(bar_slot(slot, 8 + (i & 1)));
+          warp_arrive(bar_slot(slot, 8 + (i & 1)));
         }
       }
       // ---- tile epilogue: O / l -> bf16 -> global, LSE
