@@ -61,7 +61,7 @@ struct FusedCfg {
   __host__ __device__ static constexpr int part_begin(int p) { return p <= 0 ? 0 : p == 1 ? G : p == 2 ? G + KY - 1 : HY; }
   static constexpr int NA = (RA * HX + 15) / 16 * 16;              // UMMA N of parts 0 / 2 (whole TMA box)
   static constexpr int NB = (RB * HX + 15) / 16 * 16;              // UMMA N of part 1
-  static constexpr int NMAX = NA > NB ? NA : NB;                   // columns (= smem rows) of an S buffer / stage
+  static constexpr int NMAX = ((NA > NB ? NA : NB) + 31) / 32 * 32;  // columns (= smem rows) of an S buffer / stage: whole 32-row rotation groups
   static constexpr int NF = (HALF + 1) / 2;                        // packed folded P words per key row
   static constexpr int DSUB = D / 64;                              // 128-byte sub-rows per head row
   static constexpr int SUB_KV = NMAX * 128, SUB_Q = M * 128;       // bytes of one sub-tile
@@ -198,26 +198,26 @@ __device__ __forceinline__ void rot_interleaved(uint32_t& w0, uint32_t& w1, uint
 template <int DSUB, int PAIR>
 __device__ __forceinline__ void rotate_inplace(uint32_t x_smem, uint32_t t_smem, uint32_t sub_stride, int rows, int tid) {
   if constexpr (PAIR == 0) {
-    const int n = rows * 8;
+    // `rows` is a multiple of 32 (the callers round the job up to whole 32-row groups; the extra rows are
+    // pad rows of the stage that nothing reads): every thread owns exactly rows / 16 chunks per sub-tile,
+    // two per step, no predicates and no divergent reconvergence points in the loop.
+    const int nit = rows >> 5;
 #pragma unroll
     for (int sub = 0; sub < DSUB; ++sub) {
-      const uint32_t xb = x_smem + sub * sub_stride, tb = t_smem + sub * sub_stride;
-      for (int base = tid; base < n; base += 512) {       // four chunks per thread in flight
-        uint4 x[4], t[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int idx = base + 128 * u;
-          if (idx < n) { x[u] = lds128(xb + idx * 16); t[u] = lds128(tb + idx * 16); }
+      const uint32_t xb = x_smem + sub * sub_stride + tid * 16, tb = t_smem + sub * sub_stride + tid * 16;
+      uint4 x0 = lds128(xb), t0 = lds128(tb), x1 = lds128(xb + 2048), t1 = lds128(tb + 2048);
+#pragma unroll 1
+      for (int it = 0; it < nit; ++it) {
+        const uint32_t off = (uint32_t)it * 4096u;
+        uint4 nx0 = x0, nt0 = t0, nx1 = x1, nt1 = t1;
+        if (it + 1 < nit) {                                   // next step's chunks are in flight during the arithmetic
+          nx0 = lds128(xb + off + 4096); nt0 = lds128(tb + off + 4096);
+          nx1 = lds128(xb + off + 6144); nt1 = lds128(tb + off + 6144);
         }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int idx = base + 128 * u;
-          if (idx < n) {
-            rot_interleaved(x[u].x, x[u].y, t[u].x, t[u].y);
-            rot_interleaved(x[u].z, x[u].w, t[u].z, t[u].w);
-            sts128(xb + idx * 16, x[u]);
-          }
-        }
+        rot_interleaved(x0.x, x0.y, t0.x, t0.y); rot_interleaved(x0.z, x0.w, t0.z, t0.w);
+        rot_interleaved(x1.x, x1.y, t1.x, t1.y); rot_interleaved(x1.z, x1.w, t1.z, t1.w);
+        sts128(xb + off, x0); sts128(xb + off + 2048, x1);
+        x0 = nx0; t0 = nt0; x1 = nx1; t1 = nt1;
       }
     }
   } else {
@@ -605,6 +605,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         } else {
           x_addr = k_smem + s * C::STAGE_BYTES; t_addr = t_smem + s * C::STAGE_BYTES; sub_stride = C::SUB_KV;
           rows = box_rows(part) * C::HX;
+          if (PAIR == 0) rows = (rows + 31) & ~31;        // whole 32-row groups (pad rows of the stage: never read)
           bar_in = bar_kfull(s); ph_in = (uint32_t)(G / C::NSTAGE) & 1u; bar_out = bar_krot(s);
         }
         if (tid == 0 && job == 2) TRACE(5, G);
