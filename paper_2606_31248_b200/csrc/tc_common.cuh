@@ -39,6 +39,9 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity, uin
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
+#if defined(STRATA_WAIT_SLEEP_NS) && STRATA_WAIT_SLEEP_NS > 0
+    __nanosleep(STRATA_WAIT_SLEEP_NS);      // polling warps compete with the working warps for issue slots
+#endif
     if (++spins > 20000u) {
 #ifdef STRATA_DEBUG_SYNC
       printf("mbar timeout: block %d thread %d bar 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
