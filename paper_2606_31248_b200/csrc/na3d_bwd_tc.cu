@@ -262,16 +262,19 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
           mbar_wait(bar_sfull, (uint32_t)c & 1u);
           tc_fence_after();
           if (__any_sync(0xffffffffu, vm != 0ull)) {
+            // S' and dP' in batches of 32 columns: one wait per batch, branch-free arithmetic in between
+            auto batch = [&](auto h0c, auto nbc) {
+              constexpr int H0 = decltype(h0c)::value, NB = decltype(nbc)::value;
+              uint32_t svw[NB], dpw[NB];
+              tmem_ld_issue_n<NB>(tm + C::TMEM_S + H0, svw);
+              tmem_ld_issue_n<NB>(tm + C::TMEM_DP + H0, dpw);
+              asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+              reg_fence_n<NB>(svw);
+              reg_fence_n<NB>(dpw);
+              uint32_t pw[NB / 2], dw[NB / 2];
 #pragma unroll
-            for (int j0 = 0; j0 < C::N; j0 += 16) {
-              float sv[16], dp[16];
-              tmem_ld16(tm + C::TMEM_S + j0, sv);
-              tmem_ld16(tm + C::TMEM_DP + j0, dp);
-              tmem_wait_ld();
-              uint32_t pw[8], dw[8];
-#pragma unroll
-              for (int u = 0; u < 16; u += 2) {
-                const int col = j0 + u;                        // compile-time
+              for (int u = 0; u < NB; u += 2) {
+                const int col = H0 + u;                            // compile-time
                 if (col < C::NCOL) {
                   float l2a = my_l2, da = my_d, l2b = my_l2, db = my_d;
                   if (MODE == 1) {
@@ -281,17 +284,19 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
                                  : "=f"(st.x), "=f"(st.y), "=f"(st.z), "=f"(st.w) : "r"(stat_smem + (r * 32 + 2 * x) * 4));
                     l2a = st.x; da = st.y; l2b = st.z; db = st.w;
                   }
-                  const float ea = ex2(fmaf(sv[u], cs, -l2a)), eb = ex2(fmaf(sv[u + 1], cs, -l2b));
+                  const float ea = ex2(fmaf(__uint_as_float(svw[u]), cs, -l2a)), eb = ex2(fmaf(__uint_as_float(svw[u + 1]), cs, -l2b));
                   const float pa = ((vm >> col) & 1ull) ? ea : 0.f, pb = ((vm >> (col + 1)) & 1ull) ? eb : 0.f;
                   pw[u >> 1] = pack_bf16(pa, pb);
-                  dw[u >> 1] = pack_bf16(pa * (dp[u] - da), pb * (dp[u + 1] - db));
+                  dw[u >> 1] = pack_bf16(pa * (__uint_as_float(dpw[u]) - da), pb * (__uint_as_float(dpw[u + 1]) - db));
                 } else {
                   pw[u >> 1] = 0u; dw[u >> 1] = 0u;
                 }
               }
-              if (MODE == 1) tmem_st8(tm + C::TMEM_S + (j0 >> 1), pw);
-              tmem_st8(tm + C::TMEM_DP + (j0 >> 1), dw);
-            }
+              if (MODE == 1) tmem_st_n<NB / 2>(tm + C::TMEM_S + H0 / 2, pw);
+              tmem_st_n<NB / 2>(tm + C::TMEM_DP + H0 / 2, dw);
+            };
+            batch(std::integral_constant<int, 0>{}, std::integral_constant<int, (C::N < 32 ? C::N : 32)>{});
+            if constexpr (C::N > 32) batch(std::integral_constant<int, 32>{}, std::integral_constant<int, C::N - 32>{});
           } else {
             uint32_t z[8];
 #pragma unroll
