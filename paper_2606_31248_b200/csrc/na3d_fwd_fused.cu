@@ -680,6 +680,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       for (int plane = plo; plane < phi; ++plane) {
         const bool plane_needed = plane >= wl_lo && plane < wl_hi;
         const bool plane_ok = plane >= pw_lo && plane < pw_lo + C::KL;
+#pragma unroll 1
         for (int part = 0; part < nparts; ++part, ++i) {
           const int pb = C::part_begin(part);
           const int nrows = part_rows(part);
@@ -730,9 +731,37 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
             }
             float pr[R][C::HALF];                    // folded probabilities (times 2^-m_ref)
-            float rs;
+            float rs = 0.f;
+            int attempt = 0;
 #pragma unroll 1
-            for (int attempt = 0;; ++attempt) {
+            do {                                     // (rare block first: ONE copy of the exponential pass in the code)
+              if (attempt > 0) {
+                // ---- a logit far above the reference: move the reference to the true maximum and
+                // rescale what was accumulated so far (P of this part is not stored yet)
+                const bool mine = !(rs <= kBig);
+                float cso = cs;
+                asm volatile("mov.f32 %0, %0;" : "+f"(cso));
+                const float new_ref = mine ? fmaxf(m_ref, part_max(cso)) : m_ref;
+                const float alpha = new_ref != m_ref ? ex2(m_ref - new_ref) : 1.f;
+                if (!first_item) {
+                  // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
+                  mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
+                  tc_fence_after();
+#pragma unroll 1
+                  for (int j = 0; j < C::D; j += 16) {
+                    float ov[16];
+                    tmem_ld16(tm + C::TMEM_O + j, ov);
+                    tmem_wait_ld();
+                    uint32_t ow[16];
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
+                    tmem_st16(tm + C::TMEM_O + j, ow);
+                  }
+                  tmem_wait_st();
+                }
+                lsum *= alpha;
+                m_ref = new_ref;
+              }
               // ---- p = 2^(s * cs - m_ref), branch-free over the whole part
               float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
 #pragma unroll
@@ -754,33 +783,8 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                 }
               }
               rs = (e0 + e1) + (e2 + e3);
-              if (attempt > 0 || !__any_sync(0xffffffffu, !(rs <= kBig))) break;
-              // ---- a logit far above the reference: move the reference to the true maximum and
-              // rescale what was accumulated so far (P of this part is not stored yet)
-              const bool mine = !(rs <= kBig);
-              float cso = cs;
-              asm volatile("mov.f32 %0, %0;" : "+f"(cso));
-              const float new_ref = mine ? fmaxf(m_ref, part_max(cso)) : m_ref;
-              const float alpha = new_ref != m_ref ? ex2(m_ref - new_ref) : 1.f;
-              if (!first_item) {
-                // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
-                mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
-                tc_fence_after();
-#pragma unroll 1
-                for (int j = 0; j < C::D; j += 16) {
-                  float ov[16];
-                  tmem_ld16(tm + C::TMEM_O + j, ov);
-                  tmem_wait_ld();
-                  uint32_t ow[16];
-#pragma unroll
-                  for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
-                  tmem_st16(tm + C::TMEM_O + j, ow);
-                }
-                tmem_wait_st();
-              }
-              lsum *= alpha;
-              m_ref = new_ref;
-            }
+              ++attempt;
+            } while (attempt < 2 && __any_sync(0xffffffffu, !(rs <= kBig)));
             lsum += rs;
             // ---- pack folded pairs to bf16x2, un-fold with one byte permute per output word; P overlays
             // the front of S (every S column of the part is in registers by now)
