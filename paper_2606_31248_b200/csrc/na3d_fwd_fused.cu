@@ -19,7 +19,8 @@
 //
 // Warps (512 threads):
 //   0-3    softmax + epilogue of slot 0        4-7   softmax + epilogue of slot 1
-//   8-11   rotation warpgroup: rotates every K part and every Q tile IN PLACE in shared memory
+//   8-11   rotation warpgroup: rotates every K part IN PLACE in shared memory (the Q tile of a slot is
+//          rotated the same way by that slot's softmax warpgroup, between two tiles)
 //          (packed bf16x2 multiply-adds against the bf16 cos/sin table), then hands them to the MMA
 //          issuers.  For the interleaved pairing the two halves of a pair are first gathered into
 //          separate words and the rotated words are stored in that order: the same permutation of
@@ -583,45 +584,26 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     // =========================== rotation warpgroup ===========================
     reg_dec<88>();
     const int tid = threadIdx.x - 32 * kWarpRot;
-    int nseq[2] = {0, 0};
+    // K parts only: the Q tile of a slot is rotated by that slot's softmax warpgroup while it waits for the
+    // last PV MMA of its previous tile (see below).
     int gbase = 0;
     for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
     const Col c = column(col);
-    const uint8_t* sc = sched_of(c.nparts);
     int part = 0;
     for (int g = 0; g < c.nchunks; ++g) {
-      const uint32_t e = sc[g];
       const int G = gbase + g;
       const int s = G % C::NSTAGE;
-      // jobs of this step, all through ONE copy of the rotation code: the Q tile of a slot that
-      // starts a tile here (job 0 / 1), then the K part (job 2)
-#pragma unroll 1
-      for (int job = 0; job < 3; ++job) {
-        uint32_t x_addr, t_addr, sub_stride, bar_in, ph_in, bar_out;
-        int rows;
-        if (job < 2) {
-          if (!((e >> (4 * job)) & kFirst)) continue;
-          const int n = nseq[job]++;
-          const int buf = n % C::NQBUF, use = n / C::NQBUF;
-          x_addr = q_smem + (job * C::NQBUF + buf) * C::Q_BYTES; t_addr = qt_smem; sub_stride = C::SUB_Q; rows = C::M;
-          bar_in = bar_slot(job, buf); ph_in = (uint32_t)use & 1u; bar_out = bar_slot(job, 2 + buf);
-        } else {
-          x_addr = k_smem + s * C::STAGE_BYTES; t_addr = t_smem + s * C::STAGE_BYTES; sub_stride = C::SUB_KV;
-          rows = box_rows(part) * C::HX;
-          if (PAIR == 0) rows = (rows + 31) & ~31;        // whole 32-row groups (pad rows of the stage: never read)
-          bar_in = bar_kfull(s); ph_in = (uint32_t)(G / C::NSTAGE) & 1u; bar_out = bar_krot(s);
-        }
-        if (tid == 0 && job == 2) TRACE(5, G);
-        mbar_wait(bar_in, ph_in);                          // operand (+ table) landed
-        if (tid == 0 && job == 2) TRACE(2, G);
-        if (p.rope) {
-          rotate_inplace<C::DSUB, PAIR>(x_addr, t_addr, sub_stride, rows, tid);
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          if (job < 2) warp_arrive(bar_qtempty);
-        }
-        if (tid == 0 && job == 2) TRACE(3, G);
-        warp_arrive(bar_out);
+      int rows = box_rows(part) * C::HX;
+      if (PAIR == 0) rows = (rows + 31) & ~31;            // whole 32-row groups (pad rows of the stage: never read)
+      if (tid == 0) TRACE(5, G);
+      mbar_wait(bar_kfull(s), (uint32_t)(G / C::NSTAGE) & 1u);     // operand (+ table) landed
+      if (tid == 0) TRACE(2, G);
+      if (p.rope) {
+        rotate_inplace<C::DSUB, PAIR>(k_smem + s * C::STAGE_BYTES, t_smem + s * C::STAGE_BYTES, C::SUB_KV, rows, tid);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       }
+      if (tid == 0) TRACE(3, G);
+      warp_arrive(bar_krot(s));
       if (++part == c.nparts) part = 0;
     }
     gbase += c.nchunks;
@@ -635,6 +617,24 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const uint32_t tm = tmem + slot * C::TMEM_SLOT + ((uint32_t)(sp * 32) << 16);
     const int qx = row % C::TX, qy = (row / C::TX) % C::TY, ql = row / (C::TX * C::TY);
     const float cs = p.scale_log2e;
+    // A2 for Q: this warpgroup rotates its slot's Q tiles in place (same code as the K parts), the next tile's
+    // while the last PV MMA of the current tile is still running.
+    const int ncols_cta = (p.ncols - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int qtotal = ncols_cta * (ntl > slot ? (ntl - slot + 1) / 2 : 0);      // Q tiles of this slot, all columns
+    int nq = 0;
+    auto rotate_next_q = [&]() {
+      if (nq >= qtotal) return;
+      const int buf = nq % C::NQBUF, use = nq / C::NQBUF;
+      mbar_wait(bar_slot(slot, buf), (uint32_t)use & 1u);            // Q tile (+ its table rows) landed
+      if (p.rope) {
+        rotate_inplace<C::DSUB, PAIR>(q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES, qt_smem, C::SUB_Q, C::M, row);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        warp_arrive(bar_qtempty);
+      }
+      warp_arrive(bar_slot(slot, 2 + buf));
+      ++nq;
+    };
+    rotate_next_q();
     int i = 0;
     for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
     const Col c = column(col);
@@ -820,6 +820,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           warp_arrive(bar_slot(slot, 8 + (i & 1)));
         }
       }
+      rotate_next_q();
       // ---- tile epilogue: O / l -> bf16 -> global, LSE
       mbar_wait(bar_slot(slot, 10 + ((i - 1) & 1)), (uint32_t)((i - 1) >> 1) & 1u);
       tc_fence_after();
