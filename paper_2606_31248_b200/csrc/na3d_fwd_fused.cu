@@ -420,6 +420,23 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // =========================== TMA producer ===========================
       int nrun[2] = {0, 0};                                           // tiles of each slot so far (all columns)
       int qjob = 0, gbase = 0;
+      // a deferred V load: G < 0 = none; a = cy0 | hs_x << 16, b = plane (b * L + l), hm = h | mid << 16
+      int v0G = -1, v0a = 0, v0b = 0, v0hm = 0, v1G = -1, v1a = 0, v1b = 0, v1hm = 0;
+      auto issue_v = [&](int G, int a, int b, int hm) {
+        const int s = G % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(G / C::NSTAGE) & 1u;
+        const bool mid = (hm >> 16) != 0;
+        mbar_wait(bar_vempty(s), ph ^ 1u);
+        if (lane == 0) TRACE(1, G);
+        if (elect_one()) {
+          mbar_expect_tx(bar_vfull(s), (uint32_t)(box_rows(mid ? 1 : 0) * C::HX * 128 * C::DSUB));
+#pragma unroll
+          for (int jj = 0; jj < C::DSUB; ++jj)
+            tma_load_5d(v_smem + s * C::STAGE_BYTES + jj * C::SUB_KV, mid ? &tm_vb : &tm_va, bar_vfull(s), 64 * jj, hm & 0xffff,
+                        a >> 16, a & 0xffff, b);
+        }
+        __syncwarp();
+      };
       for (int col = blockIdx.x; col < p.ncols; col += gridDim.x) {
         const Col c = column(col);
         const uint8_t* sc = sched_of(c.nparts);
@@ -466,19 +483,17 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             }
           }
           __syncwarp();
-          mbar_wait(bar_vempty(s), ph ^ 1u);
-          if (lane == 0) TRACE(1, G);
-          if (elect_one()) {
-            mbar_expect_tx(bar_vfull(s), bytes);
-#pragma unroll
-            for (int j = 0; j < C::DSUB; ++j)
-              tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, mid ? &tm_vb : &tm_va, bar_vfull(s), 64 * j, c.h, c.hs_x, cy0, c.bl + plane);
-          }
-          __syncwarp();
+          // V of this part is loaded two steps later (see VJob): a V stage is released by the PV MMA, long
+          // after the K stage of the same part (QK^T); waiting for it here would hold back the next K loads
+          if (v0G >= 0) issue_v(v0G, v0a, v0b, v0hm);
+          v0G = v1G; v0a = v1a; v0b = v1b; v0hm = v1hm;
+          v1G = G; v1a = cy0 | (c.hs_x << 16); v1b = c.bl + plane; v1hm = c.h | ((mid ? 1 : 0) << 16);
           if (++part == c.nparts) { part = 0; ++plane; }
         }
         gbase += c.nchunks;
       }
+      if (v0G >= 0) issue_v(v0G, v0a, v0b, v0hm);
+      if (v1G >= 0) issue_v(v1G, v1a, v1b, v1hm);
     } else if (warp == kWarpQk) {
       // =========================== QK^T issuer (both slots) ===========================
       // The whole warp walks the schedule in uniform control flow (descriptors stay in uniform
