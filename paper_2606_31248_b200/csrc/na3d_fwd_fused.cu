@@ -577,12 +577,17 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const uint32_t vb = v_smem + s * C::STAGE_BYTES;
         const uint32_t acc0 = (es & kFirst) ? 0u : 1u;
         if (elect_one()) {
-          for (int ks = 0; ks < nk; ++ks) {
+          auto issue = [&](auto nkc) {               // fully unrolled: the descriptors are immediates off one base
 #pragma unroll
-            for (int j = 0; j < C::DSUB; ++j)
-              umma_ts(tm + C::TMEM_O + 64 * j, a_tmem + 8 * ks, smem_desc(vb + j * C::SUB_KV + ks * 16 * 128), idesc_pv,
-                      ks > 0 ? 1u : acc0);
-          }
+            for (int ks = 0; ks < decltype(nkc)::value; ++ks) {
+#pragma unroll
+              for (int j = 0; j < C::DSUB; ++j)
+                umma_ts(tm + C::TMEM_O + 64 * j, a_tmem + 8 * ks, smem_desc(vb + j * C::SUB_KV + ks * 16 * 128), idesc_pv,
+                        ks > 0 ? 1u : acc0);
+            }
+          };
+          if (nk == C::NB / 16) issue(std::integral_constant<int, C::NB / 16>{});
+          else issue(std::integral_constant<int, C::NA / 16>{});
           umma_commit(bar_vempty(s));
           umma_commit(bar_slot(slot, 10 + (i & 1)));
           tc_fence_before();
