@@ -127,7 +127,18 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       const int bl = b * p.L;
       mbar_expect_tx(bar_q, C::Q_BYTES);
       for (int j = 0; j < C::DSUB; ++j) tma_load_5d(q_smem + j * C::SUB_Q, &tm_q, bar_q, 64 * j, h, x0, y0, bl + l0);
-      int c = 0;
+      // K loads run one chunk ahead of the V loads: a K stage is released by the QK^T MMA, a V stage only by
+      // the PV MMA after the softmax; waiting for V first would hold back the next K chunk
+      auto load_v = [&](int c, int pl, int cy) {
+        const int s = c % C::NSTAGE;
+        const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
+        mbar_wait(bar_vempty(s), ph ^ 1u);
+        mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
+        for (int j = 0; j < C::DSUB; ++j)
+          tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_v, bar_vfull(s), 64 * j, h, hs_x,
+                      hs_y + cy * C::CY, bl + hs_l + pl);
+      };
+      int c = 0, ppl = -1, pcy = 0;
       for (int pl = 0; pl < hl; ++pl)
         for (int cy = 0; cy < ncy; ++cy, ++c) {
           const int s = c % C::NSTAGE;
@@ -137,12 +148,10 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
           for (int j = 0; j < C::DSUB; ++j)
             tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_k, bar_kfull(s), 64 * j, h, hs_x,
                         hs_y + cy * C::CY, bl + hs_l + pl);
-          mbar_wait(bar_vempty(s), ph ^ 1u);
-          mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
-          for (int j = 0; j < C::DSUB; ++j)
-            tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_v, bar_vfull(s), 64 * j, h, hs_x,
-                        hs_y + cy * C::CY, bl + hs_l + pl);
+          if (ppl >= 0) load_v(c - 1, ppl, pcy);
+          ppl = pl; pcy = cy;
         }
+      if (ppl >= 0) load_v(c - 1, ppl, pcy);
     }
   } else if (warp == 1) {
     // =========================== MMA issuer ===========================
