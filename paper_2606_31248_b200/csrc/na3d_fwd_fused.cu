@@ -511,7 +511,7 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const uint32_t ph = (uint32_t)(G / C::NSTAGE) & 1u;
         const uint32_t idesc_qk = part == 1 ? instr_desc(C::M, C::NB, false) : instr_desc(C::M, C::NA, false);
         if (++part == c.nparts) part = 0;
-        mbar_wait(bar_krot(s), ph);
+        mbar_wait<false>(bar_krot(s), ph);
         if (lane == 0) TRACE(4, G);
         tc_fence_after();
 #pragma unroll
@@ -520,10 +520,10 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           if (!(es & kNeeded)) continue;
           if (es & kFirst) ++nseq[slot];
           const int buf = nseq[slot] % C::NQBUF, use = nseq[slot] / C::NQBUF;
-          if (es & kFirst) mbar_wait(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);       // Q tile rotated
+          if (es & kFirst) mbar_wait<false>(bar_slot(slot, 2 + buf), (uint32_t)use & 1u);       // Q tile rotated
           const int i = it[slot]++;
           if (i >= 2) {     // S buffer (i & 1) may be overwritten by MMAs issued after the PV MMA of item i - 2
-            mbar_wait(bar_slot(slot, 12 + (i & 1)), (uint32_t)((i - 2) >> 1) & 1u);
+            mbar_wait<false>(bar_slot(slot, 12 + (i & 1)), (uint32_t)((i - 2) >> 1) & 1u);
             tc_fence_after();
           }
           const uint32_t qb = q_smem + (slot * C::NQBUF + buf) * C::Q_BYTES;
@@ -564,14 +564,14 @@ na3d_fwd_fused_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const int nk = (part == 1 ? C::NB : C::NA) / 16;
         if (++part == c.nparts) part = 0;
         if (!(es & kNeeded)) {        // this slot does not use the part: release it once it has landed
-          mbar_wait(bar_vfull(s), ph);        // (one arrival per slot and phase, never ahead of the producer)
+          mbar_wait<false>(bar_vfull(s), ph);        // (one arrival per slot and phase, never ahead of the producer)
           if (elect_one()) mbar_arrive(bar_vempty(s));
           __syncwarp();
           continue;
         }
-        mbar_wait(bar_slot(slot, 8 + (i & 1)), (uint32_t)(i >> 1) & 1u);       // P of item i is in TMEM
+        mbar_wait<false>(bar_slot(slot, 8 + (i & 1)), (uint32_t)(i >> 1) & 1u);       // P of item i is in TMEM
         if (lane == 0) TRACE(8 + slot, G);
-        mbar_wait(bar_vfull(s), ph);
+        mbar_wait<false>(bar_vfull(s), ph);
         tc_fence_after();
         const uint32_t a_tmem = tm + C::TMEM_S + (i & 1) * C::NMAX;
         const uint32_t vb = v_smem + s * C::STAGE_BYTES;

@@ -36,11 +36,14 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity, uin
   return ok != 0;
 }
 // Bounded wait: a protocol bug becomes a launch failure (trap) after ~2 s, not a hung GPU.
+// SLEEP = true: a short sleep between polls (STRATA_WAIT_SLEEP_NS, if the including file defines it) leaves
+// the issue slots to the working warps; latency-critical waiters (MMA issuers) pass SLEEP = false.
+template <bool SLEEP = true>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
 #if defined(STRATA_WAIT_SLEEP_NS) && STRATA_WAIT_SLEEP_NS > 0
-    __nanosleep(STRATA_WAIT_SLEEP_NS);      // polling warps compete with the working warps for issue slots
+    if (SLEEP) __nanosleep(STRATA_WAIT_SLEEP_NS);
 #endif
     if (++spins > 20000u) {
 #ifdef STRATA_DEBUG_SYNC
