@@ -27,6 +27,7 @@
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 = elementwise + epilogue.
 // TMEM (256 columns): acc1 [0,64) | acc2 [64,128) | S' -> P [128,192) | dP' -> dS [192,256).
 #include <cstdio>
+#include <cstdlib>
 #include <type_traits>
 
 #include "tc_common.cuh"
@@ -62,9 +63,42 @@ struct BwdParams {
   long long N;
   float scale, scale_log2e;
   int pairing;   // strata_rope_pairing_t of the fused un-rotation
+#ifdef STRATA_TRACE
+  unsigned long long* trace;   // debug: clock64 stamps of one CTA, [event][chunk]
+  int trace_cta;
+#endif
 };
+#ifdef STRATA_TRACE
+#define BTRACE(ev, idx) do { if (p.trace && (int)blockIdx.x == p.trace_cta && (idx) < 64) p.trace[(ev) * 64 + (idx)] = clock64(); } while (0)
+#else
+#define BTRACE(ev, idx) do {} while (0)
+#endif
 
 constexpr int kBwdThreads = 192;
+
+// packed fp32 pairs (one instruction for two columns)
+struct F2 { float x, y; };
+__device__ __forceinline__ F2 ffma2(F2 a, F2 b, F2 c) {
+  F2 d;
+  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+  return d;
+}
+__device__ __forceinline__ F2 fadd2(F2 a, F2 b) {
+  F2 d;
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+__device__ __forceinline__ F2 fmul2(F2 a, F2 b) {
+  F2 d;
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "mul.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
 
 // Streamed interval [lo, hi) of row index i on one axis: MODE 0 the window of query i (A3), MODE 1 the
 // inverse neighbourhood of key i (B3).
@@ -178,6 +212,7 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
         const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
         const uint32_t sb = st_smem + s * C::STAGE_BYTES;
         mbar_wait(bar_full(s), ph);
+        BTRACE(0, c);
         tc_fence_after();
         // ---- S' = A1 B1^T, dP' = A2 B2^T  (M = 128, N, K = 64 in steps of 16)
 #pragma unroll
@@ -188,8 +223,10 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
           umma_ss(tmem + C::TMEM_DP, smem_desc(a2_smem + ks * 32), smem_desc(sb + C::CHUNK_BYTES + ks * 32), idesc_s,
                   ks > 0 ? 1u : 0u);
         umma_commit(bar_sfull);
+        BTRACE(1, c);
         // ---- acc1 += dS B1, acc2 += P B2  (A from TMEM, K = N columns in steps of 16)
         mbar_wait(bar_pfull, (uint32_t)c & 1u);
+        BTRACE(2, c);
         tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < C::N / 16; ++ks) {
@@ -200,6 +237,7 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
                     (c > 0 || ks > 0) ? 1u : 0u);
         }
         umma_commit(bar_empty(s));
+        BTRACE(3, c);
         if (c == nchunks - 1) umma_commit(bar_done);
       }
     }
@@ -252,6 +290,20 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
             const int gy = cy * C::CY + r;
             if (plane_ok && gy >= iy0 && gy < iy1) vm |= (unsigned long long)xm << (r * C::HX);
           }
+          // the same mask as additive biases: nbr[r] = -lse (MODE 0) or 0 (MODE 1) for a valid chunk row, -inf else;
+          // xz2[x / 2] = 0 / -inf per column of the pair
+          float nbr[C::CY];
+          F2 xz2[C::HX / 2];
+#pragma unroll
+          for (int r = 0; r < C::CY; ++r) {
+            const int gy = cy * C::CY + r;
+            nbr[r] = (plane_ok && gy >= iy0 && gy < iy1) ? (MODE == 0 ? -my_l2 : 0.f) : -INFINITY;
+          }
+#pragma unroll
+          for (int x = 0; x < C::HX; x += 2) {
+            xz2[x >> 1].x = ((xm >> x) & 1u) ? 0.f : -INFINITY;
+            xz2[x >> 1].y = ((xm >> (x + 1)) & 1u) ? 0.f : -INFINITY;
+          }
           const uint32_t stat_smem = bars + 128 + (uint32_t)(c & 1) * C::STAT_BYTES;
           if (MODE == 1) {
             if (et < C::NCOL)
@@ -260,6 +312,7 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
             asm volatile("bar.sync 1, 128;" ::: "memory");
           }
           mbar_wait(bar_sfull, (uint32_t)c & 1u);
+          if (et == 0) BTRACE(4, c);
           tc_fence_after();
           if (__any_sync(0xffffffffu, vm != 0ull)) {
             // S' and dP' in batches of 32 columns: one wait per batch, branch-free arithmetic in between
@@ -276,18 +329,22 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
               for (int u = 0; u < NB; u += 2) {
                 const int col = H0 + u;                            // compile-time
                 if (col < C::NCOL) {
-                  float l2a = my_l2, da = my_d, l2b = my_l2, db = my_d;
+                  const int r = col / C::HX, x = col % C::HX;     // x even: (x, x + 1) are in the same row
+                  // window mask as an additive bias: 0 or -inf per chunk row (nbr) and per column pair (xz2)
+                  F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
                   if (MODE == 1) {
-                    const int r = col / C::HX, x = col % C::HX;   // x even: (x, x + 1) are in the same row
                     float4 st;
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                                  : "=f"(st.x), "=f"(st.y), "=f"(st.z), "=f"(st.w) : "r"(stat_smem + (r * 32 + 2 * x) * 4));
-                    l2a = st.x; da = st.y; l2b = st.z; db = st.w;
+                    nb = ffma2(F2{st.x, st.z}, F2{-1.f, -1.f}, nb);
+                    dd = F2{-st.y, -st.w};
                   }
-                  const float ea = ex2(fmaf(__uint_as_float(svw[u]), cs, -l2a)), eb = ex2(fmaf(__uint_as_float(svw[u + 1]), cs, -l2b));
-                  const float pa = ((vm >> col) & 1ull) ? ea : 0.f, pb = ((vm >> (col + 1)) & 1ull) ? eb : 0.f;
-                  pw[u >> 1] = pack_bf16(pa, pb);
-                  dw[u >> 1] = pack_bf16(pa * (__uint_as_float(dpw[u]) - da), pb * (__uint_as_float(dpw[u + 1]) - db));
+                  F2 t = ffma2(F2{__uint_as_float(svw[u]), __uint_as_float(svw[u + 1])}, F2{cs, cs}, nb);
+                  t = fadd2(t, xz2[x >> 1]);
+                  const F2 e = {ex2(t.x), ex2(t.y)};
+                  const F2 g = fmul2(e, fadd2(F2{__uint_as_float(dpw[u]), __uint_as_float(dpw[u + 1])}, dd));
+                  pw[u >> 1] = pack_bf16(e.x, e.y);
+                  dw[u >> 1] = pack_bf16(g.x, g.y);
                 } else {
                   pw[u >> 1] = 0u; dw[u >> 1] = 0u;
                 }
@@ -307,8 +364,10 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
               tmem_st8(tm + C::TMEM_DP + j0, z);
             }
           }
+          if (et == 0) BTRACE(5, c);
           tmem_wait_st();
           tc_fence_before();
+          if (et == 0) BTRACE(6, c);
           mbar_arrive(bar_pfull);
         }
     }
@@ -424,6 +483,14 @@ cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, con
   bp.B = p.B; bp.H = p.H; bp.L = p.L; bp.Y = p.Y; bp.X = p.X; bp.N = p.N;
   bp.ntl = (p.L + C::TL - 1) / C::TL; bp.nty = (p.Y + C::TY - 1) / C::TY; bp.ntx = (p.X + C::TX - 1) / C::TX;
   bp.scale = p.scale; bp.scale_log2e = p.scale * 1.4426950408889634f; bp.pairing = p.pairing;
+#ifdef STRATA_TRACE
+  {
+    const char* e = getenv("STRATA_TRACE_PTR");
+    bp.trace = e ? (unsigned long long*)strtoull(e, nullptr, 0) : nullptr;
+    const char* cc = getenv("STRATA_TRACE_CTA");
+    bp.trace_cta = cc ? atoi(cc) : 0;
+  }
+#endif
   const long long grid = (long long)p.B * p.H * bp.ntl * bp.nty * bp.ntx;
   const long long rows = p.rows(), sgrid = (rows * 8 + 255) / 256;
   if (grid > 0x7fffffffLL || sgrid > 0x7fffffffLL) return cudaErrorInvalidValue;
