@@ -31,6 +31,7 @@
 #include <type_traits>
 
 #include "tc_common.cuh"
+#include "bwd_common.cuh"
 
 namespace strata {
 namespace {
@@ -57,59 +58,7 @@ struct BwdCfg {
   static_assert(2 * SMEM_BYTES <= 227 * 1024, "two CTAs per SM");
 };
 
-struct BwdParams {
-  int B, H, L, Y, X;
-  int ntl, nty, ntx;
-  long long N;
-  float scale, scale_log2e;
-  int pairing;   // strata_rope_pairing_t of the fused un-rotation
-#ifdef STRATA_TRACE
-  unsigned long long* trace;   // debug: clock64 stamps of one CTA, [event][chunk]
-  int trace_cta;
-#endif
-};
-#ifdef STRATA_TRACE
-#define BTRACE(ev, idx) do { if (p.trace && (int)blockIdx.x == p.trace_cta && (idx) < 64) p.trace[(ev) * 64 + (idx)] = clock64(); } while (0)
-#else
-#define BTRACE(ev, idx) do {} while (0)
-#endif
-
 constexpr int kBwdThreads = 192;
-
-// packed fp32 pairs (one instruction for two columns)
-struct F2 { float x, y; };
-__device__ __forceinline__ F2 ffma2(F2 a, F2 b, F2 c) {
-  F2 d;
-  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
-      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
-      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
-  return d;
-}
-__device__ __forceinline__ F2 fadd2(F2 a, F2 b) {
-  F2 d;
-  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
-      "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
-      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
-  return d;
-}
-__device__ __forceinline__ F2 fmul2(F2 a, F2 b) {
-  F2 d;
-  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
-      "mul.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
-      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
-  return d;
-}
-
-// Streamed interval [lo, hi) of row index i on one axis: MODE 0 the window of query i (A3), MODE 1 the
-// inverse neighbourhood of key i (B3).
-template <int MODE>
-__device__ __forceinline__ void row_interval(int i, int k, int n, int& lo, int& hi) {
-  if (MODE == 0) {
-    lo = window_start(i, k, n); hi = lo + k;
-  } else {
-    inverse_window(i, k, n, lo, hi); hi += 1;
-  }
-}
 
 // ------------------------------------------------------------------------------------------------
 // Kernel
@@ -207,6 +156,7 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
       constexpr uint32_t idesc_acc = instr_desc(C::M, 64, true);
       mbar_wait(bar_a, 0);
       tc_fence_after();
+      const uint64_t da1 = smem_desc(a1_smem), da2 = smem_desc(a2_smem);
       for (int c = 0; c < nchunks; ++c) {
         const int s = c % C::NSTAGE;
         const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
@@ -214,14 +164,15 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
         mbar_wait(bar_full(s), ph);
         BTRACE(0, c);
         tc_fence_after();
-        // ---- S' = A1 B1^T, dP' = A2 B2^T  (M = 128, N, K = 64 in steps of 16)
+        // ---- S' = A1 B1^T, dP' = A2 B2^T  (M = 128, N, K = 64 in steps of 16).  The descriptors of the K steps
+        // differ by a constant in their address field: one base per operand, then additions.
+        const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks)
-          umma_ss(tmem + C::TMEM_S, smem_desc(a1_smem + ks * 32), smem_desc(sb + ks * 32), idesc_s, ks > 0 ? 1u : 0u);
+          umma_ss(tmem + C::TMEM_S, da1 + 2 * ks, db1 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks)
-          umma_ss(tmem + C::TMEM_DP, smem_desc(a2_smem + ks * 32), smem_desc(sb + C::CHUNK_BYTES + ks * 32), idesc_s,
-                  ks > 0 ? 1u : 0u);
+          umma_ss(tmem + C::TMEM_DP, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
         umma_commit(bar_sfull);
         BTRACE(1, c);
         // ---- acc1 += dS B1, acc2 += P B2  (A from TMEM, K = N columns in steps of 16)
@@ -230,11 +181,9 @@ na3d_bwd_tc_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_const
         tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < C::N / 16; ++ks) {
-          umma_ts(tmem + C::TMEM_ACC1, tmem + C::TMEM_DP + 8 * ks, smem_desc(sb + ks * 16 * 128), idesc_acc,
-                  (c > 0 || ks > 0) ? 1u : 0u);
+          umma_ts(tmem + C::TMEM_ACC1, tmem + C::TMEM_DP + 8 * ks, db1 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
           if (MODE == 1)
-            umma_ts(tmem + C::TMEM_ACC2, tmem + C::TMEM_S + 8 * ks, smem_desc(sb + C::CHUNK_BYTES + ks * 16 * 128), idesc_acc,
-                    (c > 0 || ks > 0) ? 1u : 0u);
+            umma_ts(tmem + C::TMEM_ACC2, tmem + C::TMEM_S + 8 * ks, db2 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
         }
         umma_commit(bar_empty(s));
         BTRACE(3, c);
@@ -469,6 +418,12 @@ bwd_stat_kernel(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __rest
   }
 }
 
+}  // namespace
+cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
+                                const void* stat, const void* rtab, void* dq, void* dk, void* dv,
+                                cudaStream_t stream, int* launches);
+namespace {
+
 template <class C>
 cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
                            const void* d_o, const float* lse, float2* stat, const void* rtab, void* dq, void* dk, void* dv,
@@ -512,6 +467,11 @@ cudaError_t launch_bwd_cfg(const Problem& p, const void* qr, const void* kr, con
   bwd_stat_kernel<<<(unsigned)sgrid, 256, 0, stream>>>((const __nv_bfloat16*)o, (const __nv_bfloat16*)d_o, lse, stat, rows, p.N, p.H);
   prof_end(stream);
   STRATA_DBG("stat");
+  static const bool use_v2 = getenv("STRATA_BWD2") ? atoi(getenv("STRATA_BWD2")) != 0 : true;
+  if (use_v2) {
+    if (launches) *launches += 1;
+    return launch_bwd_tc2_main(p, qr, kr, v, d_o, stat, rtab, dq, dk, dv, stream, launches);
+  }
   prof_begin("na3d_bwd_dq_tcgen05", stream);
   na3d_bwd_tc_kernel<C, 0><<<(unsigned)grid, kBwdThreads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, (const float4*)rtab, (__nv_bfloat16*)dq,
                                                                                   nullptr, bp);

@@ -1,0 +1,515 @@
+// na3d_bwd_tc2.cu -- persistent, double-buffered version of the tensor-core backward (na3d_bwd_tc.cu).
+//
+// Same mathematics, modes and per-chunk MMAs as na3d_bwd_tc.cu (read that header first: MODE 0 = dQ,
+// query-stationary; MODE 1 = dK / dV, key-stationary over the inverse neighbourhood; B4 fused in the
+// epilogue).  What differs is the schedule.  A trace of na3d_bwd_tc.cu (profiles/r1_bwd_cfg4_and_tile_cfg2.md)
+// shows a chunk costing ~3100 cycles in a strictly serial chain -- S'/dP' MMAs, elementwise pass, gradient
+// MMAs -- that two co-resident CTAs only half fill.  Here ONE persistent CTA per SM runs the chain as a
+// pipeline:
+//   * S' / dP' have three buffers in TMEM and TWO elementwise warpgroups take alternate chunks, so the
+//     MMAs of chunks c + 1, c + 2 run under the elementwise pass of chunk c;
+//   * the stationary operand tiles are double buffered in shared memory (and the dQ accumulator in TMEM) and the chunk stream runs on across tiles, so the epilogue of tile t
+//     (TMEM -> un-rotate -> HBM) and the operand loads of tile t + 1 overlap the MMAs of tile t + 1.
+// TMEM (512 columns): accumulators [0, 128) -- MODE 0: acc1 double buffered by tile parity, MODE 1: {acc1, acc2}
+// once -- | SD[buf] = {S' -> P, dP' -> dS} at 128 + 128 * buf, buf < 3 (chunk index mod 3).
+// Warps (352 threads): 0 TMA producer, 1 S'/dP' MMA issuer + TMEM owner, 2-5 elementwise group 0, 6-9 group 1,
+// 10 gradient-MMA issuer.
+// Group g takes the chunks of global index parity g; in the epilogue group 0 writes acc1 (dQ or dK,
+// un-rotated), group 1 writes acc2 (dV, MODE 1 only).
+#include <cstdio>
+#include <cstdlib>
+#include <type_traits>
+
+#include "tc_common.cuh"
+#include "bwd_common.cuh"
+
+namespace strata {
+namespace {
+
+using namespace tc;
+
+template <int KL_, int KY_, int KX_>
+struct Bwd2Cfg {
+  static constexpr int D = 64, KL = KL_, KY = KY_, KX = KX_;
+  static constexpr int TL = 2, TY = 8, TX = 8, M = 128;            // stationary tile (tokens)
+  static constexpr int HX = TX + KX - 1;                           // chunk width (columns of one row)
+  static constexpr int CY = 4;                                     // chunk rows
+  static constexpr int NCOL = CY * HX;                             // real columns of a chunk
+  static constexpr int N = (NCOL + 15) / 16 * 16;                  // UMMA N (pad columns are masked)
+  static constexpr int TILE_BYTES = M * 128, CHUNK_BYTES = N * 128;
+  static constexpr int STAGE_BYTES = 2 * CHUNK_BYTES;              // B1 | B2
+  static constexpr int NSTAGE = 4;
+  static constexpr int STAT_BYTES = CY * 128;                      // [CY][16 tokens] float2 (MODE 1)
+  static constexpr int NBUF = 3;                                   // S'/dP' buffers in TMEM
+  static constexpr int TMEM_ACC = 0, TMEM_SD = 128, TMEM_COLS = 512;
+  static constexpr int NBARS = 4 + 2 * NSTAGE + 3 * NBUF + 4;
+  static constexpr int SMEM_BYTES = 1024 + 4 * TILE_BYTES + NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 128 + 4 * STAT_BYTES;
+  static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1, "odd windows only");
+  static_assert(N <= 64 && HX <= 16 && HX % 2 == 0, "a chunk must fit 64 TMEM columns; column pairs share a row");
+  static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+};
+
+constexpr int kBwd2Threads = 352;
+
+// Geometry of one stationary tile and of its streamed box.
+struct Tile2 {
+  int b, h, x0, y0, l0;
+  int bx0, by0, bl0, bl1, ncx, ncy, nchunks;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Kernel
+// ------------------------------------------------------------------------------------------------
+template <class C, int MODE>
+__global__ void __launch_bounds__(kBwd2Threads, 1)
+na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_constant__ CUtensorMap tm_a2,
+                    const __grid_constant__ CUtensorMap tm_b1, const __grid_constant__ CUtensorMap tm_b2,
+                    const float2* __restrict__ stat, const float4* __restrict__ rtab,
+                    __nv_bfloat16* __restrict__ out1, __nv_bfloat16* __restrict__ out2, const BwdParams p,
+                    const int ntiles) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  auto a_smem = [&](int par, int which) { return base + (uint32_t)(2 * par + which) * C::TILE_BYTES; };
+  const uint32_t st_smem = base + 4 * C::TILE_BYTES;                       // stages
+  const uint32_t bars = st_smem + C::NSTAGE * C::STAGE_BYTES;
+  auto bar_afull = [&](int par) { return bars + 8u * par; };               // TMA -> MMA: operand tiles of a tile
+  auto bar_aempty = [&](int par) { return bars + 8u * (2 + par); };        // last S'/dP' MMA of the tile -> TMA
+  auto bar_full = [&](int s) { return bars + 8u * (4 + s); };
+  auto bar_empty = [&](int s) { return bars + 8u * (4 + C::NSTAGE + s); };
+  auto bar_sfull = [&](int b) { return bars + 8u * (4 + 2 * C::NSTAGE + b); };                  // MMA -> elementwise, buffer b
+  auto bar_pfull = [&](int b) { return bars + 8u * (4 + 2 * C::NSTAGE + C::NBUF + b); };        // elementwise -> MMA (4 warps)
+  auto bar_sdfree = [&](int b) { return bars + 8u * (4 + 2 * C::NSTAGE + 2 * C::NBUF + b); };   // gradient MMAs have read buffer b
+  auto bar_accdone = [&](int a) { return bars + 8u * (4 + 2 * C::NSTAGE + 3 * C::NBUF + a); };  // last gradient MMA of the tile
+  auto bar_accfree = [&](int a) { return bars + 8u * (6 + 2 * C::NSTAGE + 3 * C::NBUF + a); };  // epilogue has read acc[a]
+  // accumulators: MODE 0 needs acc1 only and double buffers it by tile parity; MODE 1 has {acc1, acc2} once
+  constexpr int NACC = MODE == 0 ? 2 : 1, ACC_STRIDE = 64;
+  const uint32_t tmem_slot = bars + 8u * C::NBARS;
+  const uint32_t stat_base = (tmem_slot + 16 + 127u) & ~127u;              // [group][2] x STAT_BYTES
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - raw));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  auto tile_of = [&](int t) {
+    Tile2 T;
+    int bid = t;
+    const int tx = bid % p.ntx; bid /= p.ntx;
+    const int ty = bid % p.nty; bid /= p.nty;
+    const int tl = bid % p.ntl; bid /= p.ntl;
+    T.h = bid % p.H;
+    T.b = bid / p.H;
+    T.x0 = tx * C::TX; T.y0 = ty * C::TY; T.l0 = tl * C::TL;
+    const int xl = min(T.x0 + C::TX, p.X) - 1, yl = min(T.y0 + C::TY, p.Y) - 1, ll = min(T.l0 + C::TL, p.L) - 1;
+    int bx1, by1, t0, t1;
+    row_interval<MODE>(T.x0, C::KX, p.X, T.bx0, t1); row_interval<MODE>(xl, C::KX, p.X, t0, bx1);
+    row_interval<MODE>(T.y0, C::KY, p.Y, T.by0, t1); row_interval<MODE>(yl, C::KY, p.Y, t0, by1);
+    row_interval<MODE>(T.l0, C::KL, p.L, T.bl0, t1); row_interval<MODE>(ll, C::KL, p.L, t0, T.bl1);
+    T.ncx = (bx1 - T.bx0 + C::HX - 1) / C::HX;
+    T.ncy = (by1 - T.by0 + C::CY - 1) / C::CY;
+    T.nchunks = (T.bl1 - T.bl0) * T.ncy * T.ncx;
+    return T;
+  };
+
+  // ---- one-time setup
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tm_a1); tma_prefetch_desc(&tm_a2); tma_prefetch_desc(&tm_b1); tma_prefetch_desc(&tm_b2);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(bar_afull(i), 1); mbar_init(bar_aempty(i), 1);
+      mbar_init(bar_accdone(i), 1); mbar_init(bar_accfree(i), MODE == 1 ? 8 : 4);
+    }
+    for (int i = 0; i < C::NBUF; ++i) { mbar_init(bar_sfull(i), 1); mbar_init(bar_pfull(i), 4); mbar_init(bar_sdfree(i), 1); }
+    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
+  // chunk rows the TMA box never writes (pad columns of the UMMA N) must hold finite numbers
+  if (C::N > C::NCOL) {
+    for (int s = 0; s < C::NSTAGE; ++s)
+      for (int u = threadIdx.x; u < 2 * (C::N - C::NCOL) * 8; u += kBwd2Threads) {
+        const int which = u / ((C::N - C::NCOL) * 8), off = u % ((C::N - C::NCOL) * 8);
+        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(st_smem + s * C::STAGE_BYTES + which * C::CHUNK_BYTES +
+                                                                     C::NCOL * 128 + off * 16), "r"(0u) : "memory");
+      }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // =========================== TMA producer ===========================
+    if (lane == 0) {
+      int Tn = 0, Cn = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
+        const Tile2 T = tile_of(t);
+        const int par = Tn & 1, bl = T.b * p.L;
+        mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
+        mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
+        tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        for (int pl = T.bl0; pl < T.bl1; ++pl)
+          for (int cy = 0; cy < T.ncy; ++cy)
+            for (int cx = 0; cx < T.ncx; ++cx, ++Cn) {
+              const int s = Cn % C::NSTAGE;
+              const uint32_t ph = (uint32_t)(Cn / C::NSTAGE) & 1u;
+              const uint32_t sb = st_smem + s * C::STAGE_BYTES;
+              const int gx = T.bx0 + cx * C::HX, gy = T.by0 + cy * C::CY;
+              mbar_wait(bar_empty(s), ph ^ 1u);
+              mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128);
+              tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
+            }
+      }
+    }
+  } else if (warp == 1) {
+    // =========================== S'/dP' issuer ===========================
+    // Issuing one tcgen05.mma costs its thread ~70 cycles whatever the shape (measured: 8 MMAs of 32 tensor-pipe
+    // cycles each take ~560 cycles to issue), so the two kinds of MMA have an issuer warp each.
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = instr_desc(C::M, C::N, false);
+      int Tn = 0, Cn = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
+        const int n = tile_of(t).nchunks;
+        const int par = Tn & 1;
+        mbar_wait<false>(bar_afull(par), (uint32_t)(Tn >> 1) & 1u);
+        const uint64_t da1 = smem_desc(a_smem(par, 0)), da2 = smem_desc(a_smem(par, 1));
+        for (int c = 0; c < n; ++c, ++Cn) {
+          const int s = Cn % C::NSTAGE, buf = Cn % C::NBUF;
+          mbar_wait<false>(bar_full(s), (uint32_t)(Cn / C::NSTAGE) & 1u);
+          mbar_wait<false>(bar_sdfree(buf), ((uint32_t)(Cn / C::NBUF) & 1u) ^ 1u);    // gradient MMAs of chunk Cn - NBUF are done
+          BTRACE(0, Cn);
+          tc_fence_after();
+          const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
+          const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) umma_ss(sd, da1 + 2 * ks, db1 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
+          umma_commit(bar_sfull(buf));
+          BTRACE(1, Cn);
+          if (c == n - 1) umma_commit(bar_aempty(par));           // the operand tiles are free after these MMAs
+        }
+      }
+    }
+  } else if (warp == 10) {
+    // =========================== gradient-MMA issuer ===========================
+    if (lane == 0) {
+      constexpr uint32_t idesc_acc = instr_desc(C::M, 64, true);
+      int Tn = 0, Cn = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
+        const int n = tile_of(t).nchunks;
+        const int ai = Tn % NACC, ak = Tn / NACC;
+        const uint32_t acc = tmem + C::TMEM_ACC + ACC_STRIDE * ai;
+        for (int c = 0; c < n; ++c, ++Cn) {
+          const int s = Cn % C::NSTAGE, buf = Cn % C::NBUF;
+          mbar_wait<false>(bar_pfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
+          if (c == 0) mbar_wait<false>(bar_accfree(ai), ((uint32_t)ak & 1u) ^ 1u);   // epilogue of the last tile on this accumulator
+          BTRACE(2, Cn);
+          tc_fence_after();
+          const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
+          const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
+#pragma unroll
+          for (int ks = 0; ks < C::N / 16; ++ks) {
+            umma_ts(acc, sd + 64 + 8 * ks, db1 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
+            if (MODE == 1) umma_ts(acc + 64, sd + 8 * ks, db2 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
+          }
+          umma_commit(bar_empty(s));
+          umma_commit(bar_sdfree(buf));
+          BTRACE(3, Cn);
+          if (c == n - 1) umma_commit(bar_accdone(ai));
+        }
+      }
+    }
+  } else {
+    // =========================== elementwise group g (one row per thread) + epilogue ===========================
+    const int g = (warp - 2) >> 2;                 // group: takes the chunks whose global index has parity g
+    const int sp = warp & 3;                       // TMEM subpartition of this warp
+    const int row = sp * 32 + lane;                // row of the stationary tile == TMEM lane
+    const int et = ((warp - 2) & 3) * 32 + lane;   // thread index inside the group (statistics fetch)
+    const uint32_t tm = tmem + ((uint32_t)(sp * 32) << 16);
+    const int rx = row & 7, ry = (row >> 3) & 7, rl = row >> 6;
+    const float cs = p.scale_log2e;
+    const int sr = et / C::HX, sx = et % C::HX;
+    // MODE 1: statistics of chunk `cc` of tile T (they belong to the chunk's columns)
+    auto fetch_stat = [&](const Tile2& T, int cc) -> float2 {
+      if (MODE != 1 || et >= C::NCOL) return make_float2(0.f, 0.f);
+      const int ccx = cc % T.ncx, t2 = cc / T.ncx, ccy = t2 % T.ncy, cpl = T.bl0 + t2 / T.ncy;
+      const int gy = T.by0 + ccy * C::CY + sr, gx = T.bx0 + ccx * C::HX + sx;
+      if (gy >= p.Y || gx >= p.X) return make_float2(0.f, 0.f);
+      return __ldg(&stat[((long long)T.b * p.H + T.h) * p.N + ((long long)cpl * p.Y + gy) * p.X + gx]);
+    };
+
+    int Tn = 0, Cn = 0, kg = 0;                    // kg: chunks this group has processed (statistics buffer parity)
+    int t = blockIdx.x;
+    Tile2 T = tile_of(t < ntiles ? t : 0);
+    // first chunk of this group in the stream: global index g (every tile has at least three chunks... not
+    // assumed: walk tiles until the group's chunk is found)
+    float2 next_stat = make_float2(0.f, 0.f);
+    {
+      int tt = t, c0 = g;
+      Tile2 TT = T;
+      while (tt < ntiles && c0 >= TT.nchunks) { c0 -= TT.nchunks; tt += gridDim.x; if (tt < ntiles) TT = tile_of(tt); }
+      if (tt < ntiles) next_stat = fetch_stat(TT, c0);
+    }
+    for (; t < ntiles; t += gridDim.x, ++Tn) {
+      const int par = Tn & 1;
+      const int tn = t + gridDim.x;
+      const Tile2 TNx = tile_of(tn < ntiles ? tn : t);
+      const int x0 = T.x0, y0 = T.y0, l0 = T.l0, b = T.b, h = T.h;
+      const bool active = (x0 + rx < p.X) && (y0 + ry < p.Y) && (l0 + rl < p.L);
+      const int ax = min(x0 + rx, p.X - 1), ay = min(y0 + ry, p.Y - 1), al = min(l0 + rl, p.L - 1);
+      const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
+      // streamed interval of this row on every axis, relative to the tile's box (planes: absolute)
+      int ix0, ix1, iy0, iy1, il0, il1;
+      row_interval<MODE>(ax, C::KX, p.X, ix0, ix1); ix0 -= T.bx0; ix1 -= T.bx0;
+      row_interval<MODE>(ay, C::KY, p.Y, iy0, iy1); iy0 -= T.by0; iy1 -= T.by0;
+      row_interval<MODE>(al, C::KL, p.L, il0, il1);
+      if (!active) { ix1 = ix0; iy1 = iy0; il1 = il0; }
+      float my_l2 = 0.f, my_d = 0.f;               // MODE 0: the statistics belong to the row
+      if (MODE == 0 && active) {
+        const float2 st = stat[((long long)b * p.H + h) * p.N + tok];
+        my_l2 = st.x; my_d = st.y;
+      }
+
+      int c = 0;
+      for (int pl = T.bl0; pl < T.bl1; ++pl) {
+        const bool plane_ok = pl >= il0 && pl < il1;
+        for (int cy = 0; cy < T.ncy; ++cy)
+          for (int cx = 0; cx < T.ncx; ++cx, ++c, ++Cn) {
+            if ((Cn & 1) != g) continue;
+            // validity of this row over the chunk's columns: bit mask (skip test) and additive biases
+            const int xa = max(ix0 - cx * C::HX, 0), xb = min(ix1 - cx * C::HX, C::HX);
+            const uint32_t xm = xb > xa ? ((1u << xb) - 1u) & ~((1u << xa) - 1u) : 0u;
+            bool anyrow = false;
+            float nbr[C::CY];
+#pragma unroll
+            for (int r = 0; r < C::CY; ++r) {
+              const int gy = cy * C::CY + r;
+              const bool ok = plane_ok && gy >= iy0 && gy < iy1;
+              anyrow |= ok;
+              nbr[r] = ok ? (MODE == 0 ? -my_l2 : 0.f) : -INFINITY;
+            }
+            F2 xz2[C::HX / 2];
+#pragma unroll
+            for (int x = 0; x < C::HX; x += 2) {
+              xz2[x >> 1].x = ((xm >> x) & 1u) ? 0.f : -INFINITY;
+              xz2[x >> 1].y = ((xm >> (x + 1)) & 1u) ? 0.f : -INFINITY;
+            }
+            const uint32_t stat_smem = stat_base + (uint32_t)(2 * g + (kg & 1)) * C::STAT_BYTES;
+            if (MODE == 1) {
+              if (et < C::NCOL)
+                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(stat_smem + (sr * 16 + sx) * 8), "f"(next_stat.x), "f"(next_stat.y) : "memory");
+              // this group's next chunk: two further in the stream, possibly in the next tile
+              if (c + 2 < T.nchunks) next_stat = fetch_stat(T, c + 2);
+              else if (tn < ntiles && c + 2 - T.nchunks < TNx.nchunks) next_stat = fetch_stat(TNx, c + 2 - T.nchunks);
+              asm volatile("bar.sync %0, 128;" ::"r"(1 + g) : "memory");
+            }
+            ++kg;
+            const int buf = Cn % C::NBUF;
+            const uint32_t sd = tm + C::TMEM_SD + 128 * buf;
+            mbar_wait(bar_sfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
+            if (et == 0) BTRACE(4 + 2 * g, Cn);
+            tc_fence_after();
+            if (__any_sync(0xffffffffu, anyrow && xm != 0u)) {
+              auto batch = [&](auto h0c, auto nbc) {
+                constexpr int H0 = decltype(h0c)::value, NB = decltype(nbc)::value;
+                uint32_t svw[NB], dpw[NB];
+                tmem_ld_issue_n<NB>(sd + H0, svw);
+                tmem_ld_issue_n<NB>(sd + 64 + H0, dpw);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                reg_fence_n<NB>(svw);
+                reg_fence_n<NB>(dpw);
+                uint32_t pw[NB / 2], dw[NB / 2];
+#pragma unroll
+                for (int u = 0; u < NB; u += 2) {
+                  const int col = H0 + u;                            // compile-time
+                  if (col < C::NCOL) {
+                    const int r = col / C::HX, x = col % C::HX;     // x even: (x, x + 1) are in the same row
+                    F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
+                    if (MODE == 1) {
+                      float4 st;
+                      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                   : "=f"(st.x), "=f"(st.y), "=f"(st.z), "=f"(st.w) : "r"(stat_smem + (r * 32 + 2 * x) * 4));
+                      nb = ffma2(F2{st.x, st.z}, F2{-1.f, -1.f}, nb);
+                      dd = F2{-st.y, -st.w};
+                    }
+                    F2 tt = ffma2(F2{__uint_as_float(svw[u]), __uint_as_float(svw[u + 1])}, F2{cs, cs}, nb);
+                    tt = fadd2(tt, xz2[x >> 1]);
+                    const F2 e = {ex2(tt.x), ex2(tt.y)};
+                    const F2 gq = fmul2(e, fadd2(F2{__uint_as_float(dpw[u]), __uint_as_float(dpw[u + 1])}, dd));
+                    pw[u >> 1] = pack_bf16(e.x, e.y);
+                    dw[u >> 1] = pack_bf16(gq.x, gq.y);
+                  } else {
+                    pw[u >> 1] = 0u; dw[u >> 1] = 0u;
+                  }
+                }
+                if (MODE == 1) tmem_st_n<NB / 2>(sd + H0 / 2, pw);
+                tmem_st_n<NB / 2>(sd + 64 + H0 / 2, dw);
+              };
+              batch(std::integral_constant<int, 0>{}, std::integral_constant<int, (C::N < 32 ? C::N : 32)>{});
+              if constexpr (C::N > 32) batch(std::integral_constant<int, 32>{}, std::integral_constant<int, C::N - 32>{});
+            } else {
+              uint32_t z[8];
+#pragma unroll
+              for (int u = 0; u < 8; ++u) z[u] = 0u;
+#pragma unroll
+              for (int j0 = 0; j0 < C::N / 2; j0 += 8) {
+                if (MODE == 1) tmem_st8(sd + j0, z);
+                tmem_st8(sd + 64 + j0, z);
+              }
+            }
+            tmem_wait_st();
+            tc_fence_before();
+            if (et == 0) BTRACE(5 + 2 * g, Cn);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_pfull(buf));
+          }
+      }
+      // ---- epilogue of this tile (overlaps the next tile's chunks, which the other warps are already on):
+      // group 0: dx = R(-phi) (scale * acc1) -> bf16 (B4 fused); group 1 (MODE 1): acc2 -> bf16 dV
+      if (g == 0 || MODE == 1) {
+        const int ai = Tn % NACC, ak = Tn / NACC;
+        mbar_wait(bar_accdone(ai), (uint32_t)ak & 1u);
+        tc_fence_after();
+        const uint32_t acc = tm + C::TMEM_ACC + ACC_STRIDE * ai;
+        if (g == 0) {
+          __nv_bfloat16* r1 = out1 + (((long long)b * p.N + tok) * p.H + h) * C::D;
+          const float4* trow = rtab ? rtab + ((long long)b * p.N + tok) * (C::D / 4) : nullptr;   // 2 pairs per float4
+          float av[C::D];
+#pragma unroll
+          for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + j, *reinterpret_cast<float(*)[16]>(&av[j]));
+          tmem_wait_ld();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_accfree(ai));            // acc1 is in registers
+#pragma unroll
+          for (int j = 0; j < C::D; ++j) av[j] *= p.scale;
+          if (active) {
+            if (trow) {
+              auto rot = [&](auto half_pairing) {
+                constexpr bool HP = decltype(half_pairing)::value;
+#pragma unroll
+                for (int m = 0; m < C::D / 2; m += 2) {               // pairs m, m + 1
+                  const float4 tq = __ldg(trow + (m >> 1));           // (cos m, sin m, cos m+1, sin m+1)
+                  const int a0 = HP ? m : 2 * m, b0 = HP ? m + C::D / 2 : 2 * m + 1;
+                  const int a1 = HP ? m + 1 : 2 * m + 2, b1 = HP ? m + 1 + C::D / 2 : 2 * m + 3;
+                  const float xa0 = av[a0], xb0 = av[b0], xa1 = av[a1], xb1 = av[b1];
+                  av[a0] = fmaf(xb0, tq.y, xa0 * tq.x); av[b0] = fmaf(-xa0, tq.y, xb0 * tq.x);
+                  av[a1] = fmaf(xb1, tq.w, xa1 * tq.z); av[b1] = fmaf(-xa1, tq.w, xb1 * tq.z);
+                }
+              };
+              if (p.pairing) rot(std::true_type{}); else rot(std::false_type{});
+            }
+#pragma unroll
+            for (int j = 0; j < C::D; j += 8) {
+              uint4 w;
+              w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
+              w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
+              reinterpret_cast<uint4*>(r1)[j >> 3] = w;
+            }
+          }
+        } else {
+          __nv_bfloat16* r2 = out2 + (((long long)b * p.N + tok) * p.H + h) * C::D;
+          float av[C::D];
+#pragma unroll
+          for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + 64 + j, *reinterpret_cast<float(*)[16]>(&av[j]));
+          tmem_wait_ld();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_accfree(ai));            // acc2 is in registers
+          if (active) {
+#pragma unroll
+            for (int j = 0; j < C::D; j += 8) {
+              uint4 w;
+              w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
+              w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
+              reinterpret_cast<uint4*>(r2)[j >> 3] = w;
+            }
+          }
+        }
+      }
+      T = TNx;
+    }
+  }
+
+  // ---- teardown
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem, C::TMEM_COLS);
+  }
+}
+
+template <class C>
+cudaError_t launch_bwd2_cfg(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
+                            const float2* stat, const void* rtab, void* dq, void* dk, void* dv,
+                            cudaStream_t stream, int* launches) {
+  CUtensorMap tq_t, tdo_t, tk_c, tv_c, tk_t, tv_t, tq_c, tdo_c;
+  if (!make_map(&tq_t, qr, p, C::TX, C::TY, C::TL) || !make_map(&tdo_t, d_o, p, C::TX, C::TY, C::TL) ||
+      !make_map(&tk_c, kr, p, C::HX, C::CY, 1) || !make_map(&tv_c, v, p, C::HX, C::CY, 1) ||
+      !make_map(&tk_t, kr, p, C::TX, C::TY, C::TL) || !make_map(&tv_t, v, p, C::TX, C::TY, C::TL) ||
+      !make_map(&tq_c, qr, p, C::HX, C::CY, 1) || !make_map(&tdo_c, d_o, p, C::HX, C::CY, 1))
+    return cudaErrorInvalidValue;
+  BwdParams bp;
+  bp.B = p.B; bp.H = p.H; bp.L = p.L; bp.Y = p.Y; bp.X = p.X; bp.N = p.N;
+  bp.ntl = (p.L + C::TL - 1) / C::TL; bp.nty = (p.Y + C::TY - 1) / C::TY; bp.ntx = (p.X + C::TX - 1) / C::TX;
+  bp.scale = p.scale; bp.scale_log2e = p.scale * 1.4426950408889634f; bp.pairing = p.pairing;
+#ifdef STRATA_TRACE
+  {
+    const char* e = getenv("STRATA_TRACE_PTR");
+    bp.trace = e ? (unsigned long long*)strtoull(e, nullptr, 0) : nullptr;
+    const char* cc = getenv("STRATA_TRACE_CTA");
+    bp.trace_cta = cc ? atoi(cc) : 0;
+  }
+#endif
+  const long long ntiles = (long long)p.B * p.H * bp.ntl * bp.nty * bp.ntx;
+  if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
+  static int sm_count = 0;
+  if (sm_count == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        sm_count <= 0) {
+      (void)cudaGetLastError();
+      sm_count = 148;
+    }
+  }
+  const unsigned grid = (unsigned)(ntiles < sm_count ? ntiles : sm_count);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(na3d_bwd_tc2_kernel<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(na3d_bwd_tc2_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  prof_begin("na3d_bwd_dq_tcgen05", stream);
+  na3d_bwd_tc2_kernel<C, 0><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, (const float4*)rtab,
+                                                                          (__nv_bfloat16*)dq, nullptr, bp, (int)ntiles);
+  prof_end(stream);
+  prof_begin("na3d_bwd_dkdv_tcgen05", stream);
+  na3d_bwd_tc2_kernel<C, 1><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tk_t, tv_t, tq_c, tdo_c, stat, (const float4*)rtab,
+                                                                          (__nv_bfloat16*)dk, (__nv_bfloat16*)dv, bp, (int)ntiles);
+  prof_end(stream);
+  if (launches) *launches += 2;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+// The two main kernels of the backward in their persistent form; false if the window is not instantiated.
+cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
+                                const void* stat, const void* rtab, void* dq, void* dk, void* dv,
+                                cudaStream_t stream, int* launches) {
+#define X(KL_, KY_, KX_)                                        \
+  if (p.kL == KL_ && p.kY == KY_ && p.kX == KX_)                \
+    return launch_bwd2_cfg<Bwd2Cfg<KL_, KY_, KX_>>(p, qr, kr, v, d_o, (const float2*)stat, rtab, dq, dk, dv, stream, launches);
+  X(3, 7, 7)
+  X(3, 5, 5)
+  X(3, 3, 3)
+#undef X
+  return cudaErrorNotSupported;
+}
+
+}  // namespace strata
