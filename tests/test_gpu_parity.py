@@ -222,3 +222,34 @@ def test_device_error_paths_and_stream():
     s.synchronize()
     assert torch.equal(o, o2) and torch.equal(lse, lse2)
     assert binding.strata_na3d_last_launch_count() >= 2
+
+
+def test_one_tile_backward_kernels_still_match(oracle_mod):
+    """The one-tile-per-CTA backward (na3d_bwd_tc.cu, STRATA_BWD2=0) is kept as a second implementation of
+    B1-B4; the switch is read once per process, so it runs in a child process and writes its gradients out."""
+    import os
+    import subprocess
+    import sys
+    import tempfile
+    w = wl.small(name="bwd_v1", dtype="bf16", value_scale="rsqrt_d", grid=(5, 13, 20), window=(3, 7, 7), heads=2,
+                 head_dim=64, batch=1)
+    inp = wl.make_inputs(w, with_do=True)
+    rq, rk, rv = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys, numpy as np, torch\n"
+        f"sys.path.insert(0, {root!r}); sys.path.insert(0, {os.path.join(root, 'tests')!r})\n"
+        "from paper_2606_31248_b200 import workloads as wl\n"
+        "import test_gpu_parity as T\n"
+        "w = wl.small(name='bwd_v1', dtype='bf16', value_scale='rsqrt_d', grid=(5, 13, 20), window=(3, 7, 7), heads=2, head_dim=64, batch=1)\n"
+        "inp = wl.make_inputs(w, with_do=True)\n"
+        "d, o, lse = T.run_fwd(w, inp)\n"
+        "g = T.run_bwd(w, inp, d, o, lse)\n"
+        "np.save(sys.argv[1], np.stack([x.float().cpu().numpy() for x in g]))\n")
+    with tempfile.TemporaryDirectory() as tmp:
+        out = os.path.join(tmp, "g.npy")
+        env = dict(os.environ, STRATA_BWD2="0")
+        subprocess.run([sys.executable, "-c", code, out], check=True, env=env, timeout=600)
+        g = np.load(out).astype(np.float64)
+    for got, ref, nm in zip(g, (rq, rk, rv), ("dQ", "dK", "dV")):
+        assert_parity(got, ref, "bf16", f"one-tile backward {nm}", rms_bound=2e-2)
