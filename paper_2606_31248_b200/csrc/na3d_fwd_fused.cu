@@ -4,7 +4,9 @@
 // pre-kernel): Q and K arrive un-rotated, are rotated in registers by a dedicated warpgroup and go
 // to the tensor cores from shared memory; the rotated copies never touch HBM.
 //
-// Work decomposition ("level sweep"): one CTA owns a level COLUMN of one (sample, head): the
+// Work decomposition ("level sweep"): persistent CTAs, one per SM; CTA c takes the level COLUMNS c,
+// c + gridDim.x, ... and every pipeline counter runs on across columns, so the loads, rotations and MMAs
+// of the next column start while the previous one drains.  A level column of one (sample, head) is the
 // TY x TX patch of every level, i.e. ceil(L / TL) query tiles of TL x TY x TX = 128 queries.  The
 // key / value planes of the column's halo ((TY+kY-1) x (TX+kX-1) keys per level) stream through
 // shared memory ONCE, level by level, in three parts of key rows ([0, G), [G, G+kY-1), [G+kY-1, HY)
@@ -25,11 +27,13 @@
 //          issuers.  For the interleaved pairing the two halves of a pair are first gathered into
 //          separate words and the rotated words are stored in that order: the same permutation of
 //          the 8 channels of every 16-byte chunk is applied to Q and K, which leaves Q K^T unchanged.
-//   12     TMA producer: K + rotary-table + V parts into a stage ring; Q tiles + their table rows;
-//          TMEM owner
+//   12     TMA producer: K + rotary-table + V parts into a stage ring (the K loads run two parts ahead
+//          of the V loads: a V stage is released by the PV MMA, long after the K stage of the same
+//          part); Q tiles + their table rows; TMEM owner
 //   13     QK^T issuer of both slots          14, 15   PV issuer of slot 0 / 1
 //          (whole warp in uniform control flow, one elected lane issues; the QK^T issuer re-uses
-//          an S buffer once the PV MMA that read its P has completed)
+//          an S buffer once the PV MMA that reads its P has been ISSUED: the tensor pipe executes in
+//          issue order)
 // Register budget via setmaxnreg: 184 / 184 / 88 / 56 per thread for the four warpgroups.
 //
 // Softmax: a thread (= query row) takes the whole S part (R key rows x HX columns) into registers with
