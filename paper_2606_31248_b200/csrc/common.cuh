@@ -65,6 +65,12 @@ bool fused_fwd_supported(const Problem& p);
 cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
                              void* o, float* lse, cudaStream_t stream, int* launches);
 
+// na3d_fwd_sweep.cu: tcgen05 forward, everything (A1-A6) in one kernel: un-rotated bf16 operands, coordinates and
+// frequencies in, O and LSE out; no workspace.
+bool sweep_fwd_supported(const Problem& p);
+cudaError_t launch_fwd_sweep2(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
+                              const float* freqs, void* o, float* lse, cudaStream_t stream, int* launches);
+
 // na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
 cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             void* o, float* lse, cudaStream_t stream, int* launches);

@@ -25,33 +25,37 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// try_wait suspends the thread in hardware until the phase completes or `hint_ns` elapses.
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity, uint32_t hint_ns = 100000u) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok) : "r"(bar), "r"(parity), "r"(hint_ns) : "memory");
-  return ok != 0;
-}
-// Bounded wait: a protocol bug becomes a launch failure (trap) after ~2 s, not a hung GPU.
-// SLEEP = true: a short sleep between polls (STRATA_WAIT_SLEEP_NS, if the including file defines it) leaves
-// the issue slots to the working warps; latency-critical waiters (MMA issuers) pass SLEEP = false.
+// try_wait blocks in hardware for a short, system-dependent time (about 40 cycles on B200) and returns false if
+// the phase has not completed by then.  The wait loop is kept to two instructions (try_wait, branch): up to
+// sixteen warps of a CTA sit in such loops, and every extra instruction per poll is taken from the issue slots
+// of the working warps (a suspend-time hint, a nanosleep or a poll counter cost more than they save: the sleeps
+// return after a few nanoseconds while other warps signal barriers).
+// STRATA_DEBUG_SYNC: bounded wait, a protocol bug becomes a trap after ~1 s instead of a hung GPU.
 template <bool SLEEP = true>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-#if defined(STRATA_WAIT_SLEEP_NS) && STRATA_WAIT_SLEEP_NS > 0
-    if (SLEEP) __nanosleep(STRATA_WAIT_SLEEP_NS);
-#endif
-    if (++spins > 20000u) {
 #ifdef STRATA_DEBUG_SYNC
+  uint32_t spins = 0;
+  for (;;) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) break;
+    if (++spins > 20000000u) {
       printf("mbar timeout: block %d thread %d bar 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
-#endif
       __trap();
     }
   }
+#else
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@!p bra WAIT_LOOP;\n\t}"
+      :: "r"(bar), "r"(parity) : "memory");
+#endif
 }
 // One lane of a converged warp (all 32 lanes must execute this).
 __device__ __forceinline__ bool elect_one() {
