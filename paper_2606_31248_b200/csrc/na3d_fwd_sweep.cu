@@ -206,6 +206,12 @@ __device__ __forceinline__ void sincos_reduced(float phi, float& sn, float& cs) 
   const float r = fmaf(n, 1.7484555e-7f, fmaf(n, -6.2831854820251465f, phi));    // 2 pi = 6.2831854820251465 - 1.7484555e-7
   __sincosf(r, &sn, &cs);
 }
+// Pins a value in a register: the compiler can no longer re-derive it from its inputs at every use (it does that
+// for TMEM and barrier addresses, at the cost of ten instructions per use).
+__device__ __forceinline__ uint32_t pinned(uint32_t x) {
+  asm volatile("mov.u32 %0, %0;" : "+r"(x));
+  return x;
+}
 // (a & m) | (b & ~m)
 __device__ __forceinline__ uint32_t bitsel(uint32_t m, uint32_t a, uint32_t b) {
   uint32_t d;
@@ -253,7 +259,8 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   uint8_t* need = smem_raw + (tmem_word + 16 - raw);                   // [L] bit s: slot s has a tile that reaches the plane
   float4* cc = reinterpret_cast<float4*>(smem_raw + (cc_smem - raw));
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // (the shuffle makes the warp index provably warp-uniform for the compiler: role state then lives in uniform registers)
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
   // ---- geometry of one level column: head fastest (the H heads of a token are one contiguous H*D*2-byte run
   // in HBM), then x, y, sample.
@@ -741,11 +748,11 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int slot = warp >> 2;
     const int sp = warp & 3;                       // TMEM subpartition
     const int row = sp * 32 + lane;                // query row of the tile == TMEM lane
-    const uint32_t tm = tmem + slot * C::T_SLOT + ((uint32_t)(sp * 32) << 16);
+    const uint32_t tm = pinned(tmem + slot * C::T_SLOT + ((uint32_t)(sp * 32) << 16));
     const int qx = row % C::TX, qy = (row / C::TX) % C::TY, ql = row / (C::TX * C::TY);
     const float cs = p.scale_log2e;
-    const uint32_t bar_sfull = bar_slot(slot, 0), bar_sfree = bar_slot(slot, 1), bar_pfull = bar_slot(slot, 2),
-                   bar_pvdone = bar_slot(slot, 3);
+    const uint32_t bar_sfull = pinned(bar_slot(slot, 0)), bar_sfree = pinned(bar_slot(slot, 1)), bar_pfull = pinned(bar_slot(slot, 2)),
+                   bar_pvdone = pinned(bar_slot(slot, 3));
     // pad keys of a part: P = 0 for good (nothing else writes these columns)
     if constexpr (C::NPART / 2 > C::RH * C::PW) {
       uint32_t z[C::NPART / 2 - C::RH * C::PW];
