@@ -4,49 +4,53 @@
 // table are the only inputs; the rotary angles (A1), the rotation of Q and K (A2), the clamped windows (A3),
 // logits, softmax + LSE and the output (A4-A6) all happen here; nothing rotated ever touches HBM.
 //
-// Work decomposition ("level sweep"): persistent CTAs, one per SM; CTA c takes the level COLUMNS c,
-// c + gridDim.x, ...  A level column of one (sample, head) is the TY x TX patch of every level, i.e.
-// ceil(L / TL) query tiles of TL x TY x TX = 128 queries.  The key / value planes of the column's halo
-// ((TY+kY-1) x (TX+kX-1) keys per level) stream through shared memory ONCE, level by level, each plane in two
-// PARTS of RH = HY/2 key rows; every part is multiplied against the (at most two) query tiles whose clamped
-// level windows (R1) reach its plane.  Two independent tile pipelines ("slots") run
-// inside the CTA: slot s owns tiles s, s+2, ... (their plane ranges are disjoint and increasing, checked on
-// the host).  One (tile, part) pair is an ITEM of its slot.
+// Work decomposition ("level sweep"): persistent CTAs, one per SM; CTA c takes the UNITS c, c + gridDim.x, ...
+// A unit is hg consecutive heads of one (sample, y tile, x tile); one head of it is a level COLUMN: the TY x TX
+// patch of every level, i.e. ceil(L / TL) query tiles of TL x TY x TX = 128 queries.  The key / value planes of
+// the column's halo ((TY+kY-1) x (TX+kX-1) keys per level) stream through shared memory ONCE, level by level,
+// each plane in three PARTS of key rows ([0, G), [G, G+kY-1), [G+kY-1, HY) with G = 32 / TX query rows per softmax
+// warp: away from the grid border a warp needs either every row of a part or none); every part is multiplied
+// against the (at most two) query tiles whose clamped level windows (R1) reach its plane.
+// Two independent tile pipelines ("slots") run inside the CTA: slot s owns tiles s, s+2, ... (their plane
+// ranges are disjoint and increasing, checked on the host).  One (tile, part) pair is an ITEM of its slot.
 //
-// Per slot, 256 TMEM columns: O [0, 64) fp32 | S [64, 64+NPART) fp32 | P [.., +NPART/2) packed bf16.
-// Item pipeline of a slot (i = item counter; every barrier below completes exactly one phase per item):
-//   issuer : QK^T(i) -> S            commit s_full
-//   softmax: wait s_full, S -> registers, arrive s_free   (the issuer may now issue QK^T(i+1) over S)
-//            exp2 against a lazy reference maximum, row sum, P (bf16) in registers
-//            wait pv_done(i-1) (P columns free, O complete up to item i-1) [+ epilogue of the previous tile]
-//            P -> TMEM, arrive p_full
-//   issuer : wait p_full, O += P V   commit pv_done
-// so S(i+1) is ready long before the softmax of item i ends and the softmax warps never wait for the MMAs in
-// steady state; the tensor pipe is fed by two such chains.
+// Per slot, 256 TMEM columns: O [0, 64) fp32 | S0 | S1 (S is double buffered; P (bf16) is written over the front of
+// the S buffer it came from, row by row, and is the TMEM A-operand of the PV MMA).  Item pipeline of a slot:
+//   issuer : QK^T(i) -> S[i & 1]                 commit s_full[i & 1]      (two items ahead of the PV MMAs)
+//   softmax: wait s_full, row by row: S row -> registers, exp2 against a lazy reference maximum, P row -> TMEM;
+//            arrive p_full[i & 1]
+//   issuer : wait p_full, O += P V, then QK^T(i + 2) into the same buffer (the tensor pipe executes in issue order)
+// so S(i+1) is ready when the softmax of item i ends.
+//
+// THE INSTRUCTION CACHE IS THE DESIGN CONSTRAINT.  Measured on B200 (one warp per scheduler, straight-line FFMA):
+// a loop body of <= 512 instructions runs at 1.2 cycles / instruction out of the L0 cache of its scheduler, 1K - 2K
+// instructions at 3.1, anything larger at 5.7.  A warp-specialised kernel keeps four different instruction streams
+// on every scheduler, so each role's steady-state loop here is a small ROLLED loop: the softmax walks the key rows
+// of a part one at a time (S row from TMEM, ~50 instructions), the rotation walks 16-byte chunks four at a time,
+// the issuer prepares its descriptors with adds.  (Round 1's kernel unrolled whole parts: 600-instruction bodies
+// that streamed from L2 at every item.)
 //
 // Warps (512 threads):
 //   0-3    softmax + epilogue of slot 0 (one query row per thread = one TMEM lane)      4-7   the same, slot 1
-//   8-11   rotation warpgroup.  Per column: loads the halo's coordinates, checks that they are the same on
+//   8-11   rotation warpgroup.  Per unit: loads the halo's coordinates, checks that they are the same on
 //          every level (the paper's A = 2 case: (x, y) of a column do not depend on the level),
 //          builds the (cos, sin) table of the halo in shared memory (A1: fp32 fma chain, two-term Cody-Waite
-//          reduction, MUFU sin / cos, rounded to bf16) -- once per column when level invariant, else per level
+//          reduction, MUFU sin / cos, rounded to bf16) -- once per unit when level invariant, else per level
 //          -- and rotates every Q tile and every K part IN PLACE in shared memory with packed bf16x2
 //          multiply-adds (A2), then hands them to the MMA issuers.  For the interleaved pairing the two halves
 //          of a pair are gathered into separate words and left in that order: the same permutation of the 8
 //          channels of every 16-byte chunk is applied to Q and K, which leaves Q K^T unchanged.
 //   12     TMA producer of Q tiles and K parts; TMEM owner          13   TMA producer of V parts
-//   14,15  MMA issuer of slot 0 / 1: QK^T(i+1) then PV(i), one elected lane
+//   14,15  MMA issuer of slot 0 / 1, one elected lane
 // Register budget via setmaxnreg: 168 / 168 / 120 / 56.
 //
-// Softmax of an item: the thread's S row (R key rows x HX columns) comes into registers with one batch of
-// tcgen05.ld; everything up to the P store is branch-free.  A warp owns 4 query rows (y) of one level: it
-// needs kY + 3 of the HY halo rows, i.e. all RH rows of one part and a few of the other -- the second goes
-// through a short variant (RP rows), a part of a plane outside the warp's level window stores zeros.
-// exp2 with a LAZY reference maximum: the row maximum is computed only for the first part that holds a valid
-// key of the row and when the part's sum overflows 2^40 (checked once per part, before P is stored).
-// The x window of a query covers kX of the HX halo columns; with kX <= HX/2 at most one of the columns c and
-// c + HX/2 is inside it, so the two halves of every key row are FOLDED with a per-thread bit select before the
-// exponential (half the MUFU work); P is packed to bf16 folded and un-folded by one byte permute per word.
+// Softmax of a row: exp2 with a LAZY reference maximum: the row maximum is computed only for the first part
+// that holds a valid key of the query and when a key row's sum overflows 2^40; the reference then moves up by a
+// whole number of octaves, so everything accumulated so far (O, the row sum, the P rows already stored) is
+// rescaled by an exact power of two.  The x window of a query covers kX of the HX halo columns; with kX <= HX/2 at
+// most one of the columns c and c + HX/2 is inside it, so the two halves of every key row are FOLDED with a
+// per-thread bit select before the exponential (half the MUFU work); P is packed to bf16 folded and un-folded by
+// one byte permute per output word (a masked slot replicates the zero sign bit).
 #include <cstdlib>
 #include <mutex>
 #include <type_traits>
@@ -59,32 +63,37 @@ namespace {
 
 using namespace tc;
 
+
 template <int D_, int KL_, int KY_, int KX_, int NS_>
 struct SweepCfg {
   static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
   static constexpr int TL = 2, TY = 8, TX = 8, M = 128;
   static constexpr int HY = TY + KY - 1, HX = TX + KX - 1, HALF = HX / 2;
-  static constexpr int RH = HY / 2;                                  // key rows of a part (half a halo plane)
-  static constexpr int NKEY = RH * HX;                               // keys of a part
-  static constexpr int NPART = (NKEY + 15) / 16 * 16;                // UMMA N (QK^T) and K extent (PV) of a part
+  static constexpr int G = 32 / TX;                                  // query rows (y) per softmax warp
+  static constexpr int NPARTS = 3;                                   // key-row parts of a halo plane
+  static constexpr int RA = G, RB = KY - 1;                          // key rows of parts 0 / 2 and of part 1
+  __host__ __device__ static constexpr int part_begin(int p) { return p <= 0 ? 0 : p == 1 ? G : p == 2 ? G + KY - 1 : HY; }
+  __host__ __device__ static constexpr int part_rows(int p) { return p == 1 ? RB : RA; }
+  static constexpr int NA = (RA * HX + 15) / 16 * 16;                // UMMA N (QK^T) / K extent (PV) of parts 0 / 2
+  static constexpr int NB = (RB * HX + 15) / 16 * 16;                // ... of part 1
+  static constexpr int NMAX = NA > NB ? NA : NB;                     // columns of an S buffer, rows of a stage
   static constexpr int PW = HX / 2;                                  // packed P words per key row
   static constexpr int NF = (HALF + 1) / 2;                          // packed folded P words per key row
-  static constexpr int RA = (RH + 1) / 2, RB = RH - RA;              // the two row groups of the softmax of a part
   static constexpr bool FULLFOLD = (KX == HALF);                     // exactly one of the columns c, c + HALF is in the window
   static constexpr int NS = NS_, NQ = 4;                             // K / V stages, Q buffers
-  static constexpr int STAGE = NPART * 128, QB = M * 128;            // bytes of a K / V / table part, of a Q tile
-  static constexpr int T_O = 0, T_S = D, T_P = D + NPART, T_SLOT = 256;
-  static constexpr int LA = 2;                                       // a Q tile is loaded / rotated LA parts before its first use
-  static constexpr int NBARS = 5 * NS + 3 * NQ + 8;
-  static constexpr int CC_BYTES = 2 * NKEY * 16;                     // coordinate cache: float4 per halo token
-  static constexpr int SMEM_BYTES = 1024 + NQ * QB + 2 * NS * STAGE + 2 * STAGE + CC_BYTES + 8 * NBARS + 16 + 256;
+  static constexpr int STAGE = NMAX * 128, QB = M * 128;             // bytes of a K / V / table part, of a Q tile
+  static constexpr int T_O = 0, T_S = D, T_SLOT = 256;               // S buffer b of a slot: T_S + b * NMAX
+  static constexpr int LA = 3;                                       // a Q tile is loaded / rotated LA parts before its first use
+  static constexpr int NBARS = 5 * NS + 3 * NQ + 12;
+  static constexpr int NTOK = HY * HX;                               // halo tokens of a plane
+  static constexpr int CC_BYTES = NTOK * 16;                         // coordinate cache: float4 per halo token
+  static constexpr int SMEM_BYTES = 1024 + NQ * QB + 2 * NS * STAGE + NPARTS * STAGE + CC_BYTES + 8 * NBARS + 16 + 256;
   static_assert(D == 64, "head_dim 64");
   static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1 && KY >= 3, "odd windows only (HX, HY even)");
   static_assert(KX <= HALF, "the x fold needs kX <= HX / 2");
   static_assert(TL >= KL - 1, "tiles t and t+2 must reach disjoint planes");
-  static_assert(HX <= 16 && 2 * NKEY <= 256, "halo of at most 256 keys per plane");
-  static_assert(RB >= 1, "two row groups");
-  static_assert(D + NPART + NPART / 2 <= T_SLOT, "TMEM columns of a slot");
+  static_assert(HX <= 16 && NTOK <= 256, "halo of at most 256 keys per plane");
+  static_assert(D + 2 * NMAX <= T_SLOT, "TMEM columns of a slot");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
@@ -226,13 +235,22 @@ template <class C> __device__ __host__ __forceinline__ int tile_phi(int t, int L
   return window_start(last < L - 1 ? last : L - 1, C::KL, L) + C::KL;
 }
 
+
+// Shared-memory matrix descriptor from its low word (start address >> 4 | leading offset); the high word is the
+// same for every operand here: 8-row groups 1024 bytes apart, version 1, 128-byte swizzle.  A k-step adds an
+// immediate to the low word.
+__device__ __forceinline__ uint32_t desc_lo(uint32_t addr) { return ((addr >> 4) & 0x3FFFu) | (1u << 16); }
+__device__ __forceinline__ uint64_t desc_from_lo(uint32_t lo) { return ((uint64_t)0x40004040u << 32) | lo; }
+
+
 // ------------------------------------------------------------------------------------------------
 // Kernel
 // ------------------------------------------------------------------------------------------------
 template <class C, int PAIR>   // PAIR: strata_rope_pairing_t of the rotation
 __global__ void __launch_bounds__(kSweepThreads, 1)
-na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                      const __grid_constant__ CUtensorMap tm_v, const float* __restrict__ coords,
+na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_ka,
+                      const __grid_constant__ CUtensorMap tm_kb, const __grid_constant__ CUtensorMap tm_va,
+                      const __grid_constant__ CUtensorMap tm_vb, const float* __restrict__ coords,
                       const float* __restrict__ freqs, __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                       const SweepParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -241,8 +259,8 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   const uint32_t q_smem = base;                                        // [NQ] Q tiles
   const uint32_t k_smem = q_smem + C::NQ * C::QB;                      // [NS] K parts
   const uint32_t v_smem = k_smem + C::NS * C::STAGE;                   // [NS] V parts
-  const uint32_t t_smem = v_smem + C::NS * C::STAGE;                   // (cos, sin) table of the halo, [2 parts]
-  const uint32_t cc_smem = t_smem + 2 * C::STAGE;                      // coordinates of the halo tokens, float4 each
+  const uint32_t t_smem = v_smem + C::NS * C::STAGE;                   // (cos, sin) table of the halo, [NPARTS] in K-part geometry
+  const uint32_t cc_smem = t_smem + C::NPARTS * C::STAGE;              // coordinates of the halo tokens, float4 each
   const uint32_t bars = cc_smem + C::CC_BYTES;
   auto bar_kfull = [&](int s) { return bars + 8u * s; };                          // TMA -> rotation
   auto bar_krot = [&](int s) { return bars + 8u * (C::NS + s); };                 // rotation (4 warps) -> issuers
@@ -252,8 +270,11 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   auto bar_qfull = [&](int b) { return bars + 8u * (5 * C::NS + b); };            // TMA -> rotation
   auto bar_qrot = [&](int b) { return bars + 8u * (5 * C::NS + C::NQ + b); };     // rotation -> issuer
   auto bar_qfree = [&](int b) { return bars + 8u * (5 * C::NS + 2 * C::NQ + b); };   // issuer commit -> TMA
-  // per slot: 0 s_full (issuer commit)  1 s_free (4 softmax warps)  2 p_full (4 softmax warps)  3 pv_done (issuer commit)
-  auto bar_slot = [&](int slot, int which) { return bars + 8u * (5 * C::NS + 3 * C::NQ + 4 * slot + which); };
+  // per slot: 0, 1 s_full[buf] (issuer commit)   2, 3 p_full[buf] (4 softmax warps)   4, 5 pv_done[buf] (issuer commit)
+  // (pv_done is waited for only now and then, so it is split by item parity: a parity test can tell a phase from
+  // the one before it, not from the one two back; when S(i) is there, PV(i - 2) is complete -- the tensor pipe
+  // executes in issue order -- so pv_done[(i - 1) & 1] is in the phase of PV(i - 1) or the next)
+  auto bar_slot = [&](int slot, int which) { return bars + 8u * (5 * C::NS + 3 * C::NQ + 6 * slot + which); };
   const uint32_t tmem_word = bars + 8u * C::NBARS;
   uint32_t* tmem_word_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_word - raw));
   uint8_t* need = smem_raw + (tmem_word + 16 - raw);                   // [L] bit s: slot s has a tile that reaches the plane
@@ -278,7 +299,7 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int yl = min(c.y0 + C::TY, p.Y) - 1;
     c.hs_x = window_start(c.x0, C::KX, p.X); c.hs_y = window_start(c.y0, C::KY, p.Y);
     c.hy = window_start(yl, C::KY, p.Y) + C::KY - c.hs_y;     // key rows of the halo, <= HY
-    c.np = c.hy > C::RH ? 2 : 1;
+    c.np = c.hy > C::part_begin(2) ? 3 : c.hy > C::part_begin(1) ? 2 : 1;
     c.nchunks = p.L * c.np;
     c.bl = c.b * p.L;
     return c;
@@ -286,24 +307,37 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   const int ntl = (p.L + C::TL - 1) / C::TL;
   // part index (within the column) before which Q tile t is loaded and rotated
   auto qpos = [&](int t, int np) { return max(tile_plo<C>(t, p.L) * np - C::LA, 0); };
-  // the cl-th column of this CTA (-1: none): unit blockIdx.x + (cl / hg) * gridDim.x, head cl % hg of the unit
-  auto col_of = [&](int cl) {
-    const long long u = (long long)blockIdx.x + (long long)(cl / p.hg) * gridDim.x;
-    const long long col = u * p.hg + cl % p.hg;
-    return col < p.ncols ? (int)col : -1;
+  // Walk over the columns of this CTA.  The columns of a unit differ in the head only, so the geometry (divisions,
+  // window clamps) is worked out once per unit: the code of `column` is off the steady-state path of every role.
+  struct ColIter {
+    Col c;
+    int cl, hh;          // columns so far, head within the unit
+    long long u;         // unit
+  };
+  auto col_begin = [&](ColIter& it) { it.cl = -1; it.hh = 0; it.u = 0; };
+  auto col_advance = [&](ColIter& it) -> bool {
+    ++it.cl;
+    if (it.cl > 0 && ++it.hh < p.hg) { ++it.c.h; return true; }
+    it.hh = 0;
+    it.u = it.cl == 0 ? (long long)blockIdx.x : it.u + gridDim.x;
+    if (it.u * p.hg >= p.ncols) return false;
+    it.c = column((int)(it.u * p.hg));
+    return true;
   };
 
   // ---- one-time setup
   if (warp == kWarpLoadK && lane == 0) {
-    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_v);
+    tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_ka); tma_prefetch_desc(&tm_kb);
+    tma_prefetch_desc(&tm_va); tma_prefetch_desc(&tm_vb);
     for (int s = 0; s < C::NS; ++s) {
       mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 4); mbar_init(bar_kempty(s), 2);
       mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 2);
     }
     for (int b = 0; b < C::NQ; ++b) { mbar_init(bar_qfull(b), 1); mbar_init(bar_qrot(b), 4); mbar_init(bar_qfree(b), 1); }
     for (int slot = 0; slot < 2; ++slot) {
-      mbar_init(bar_slot(slot, 0), 1); mbar_init(bar_slot(slot, 1), 4);
-      mbar_init(bar_slot(slot, 2), 4); mbar_init(bar_slot(slot, 3), 1);
+      mbar_init(bar_slot(slot, 0), 1); mbar_init(bar_slot(slot, 1), 1);
+      mbar_init(bar_slot(slot, 2), 4); mbar_init(bar_slot(slot, 3), 4);
+      mbar_init(bar_slot(slot, 4), 1); mbar_init(bar_slot(slot, 5), 1);
     }
     fence_barrier_init();
   }
@@ -314,15 +348,10 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (l >= tile_plo<C>(t, p.L) && l < tile_phi<C>(t, p.L)) e |= 1u << (t & 1);
     need[l] = (uint8_t)e;
   }
-  // The pad rows of the V stages (keys NKEY .. NPART of a part) are multiplied by P = 0 in the PV MMA and must
-  // therefore hold finite numbers: zeros, never overwritten by the TMA boxes.
-  if constexpr (C::NPART > C::NKEY) {
-    constexpr uint32_t pad = (uint32_t)(C::NPART - C::NKEY) * 128u;
-    for (uint32_t off = threadIdx.x * 16u; off < (uint32_t)C::NS * pad; off += kSweepThreads * 16u) {
-      const uint32_t s = off / pad, r = off - s * pad;
-      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(v_smem + s * C::STAGE + C::NKEY * 128 + r), "r"(0u) : "memory");
-    }
-  }
+  // K and V stages start as zeros: the rows of a stage a (shorter) part does not overwrite are keys outside every
+  // window (P = 0 there), which must hold finite numbers.
+  for (uint32_t off = threadIdx.x * 16u; off < 2u * C::NS * C::STAGE; off += kSweepThreads * 16u)
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(k_smem + off), "r"(0u) : "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   tc_fence_before();
   __syncthreads();
@@ -334,12 +363,14 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     if (warp == kWarpLoadK) {
       // =========================== TMA producer: Q tiles and K parts ===========================
       int gbase = 0;
-      for (int cl = 0, col; (col = col_of(cl)) >= 0; ++cl) {
-        const Col c = column(col);
-        int tq = 0;
+      ColIter it;
+      col_begin(it);
+      while (col_advance(it)) {
+        const Col& c = it.c;
+        int tq = 0, plane = 0, part = 0;
         for (int g = 0; g < c.nchunks; ++g) {
           while (tq < ntl && qpos(tq, c.np) == g) {
-            const int n = cl * ntl + tq, buf = n % C::NQ, use = n / C::NQ;
+            const int n = it.cl * ntl + tq, buf = n % C::NQ, use = n / C::NQ;
             if (use >= 1) mbar_wait(bar_qfree(buf), (uint32_t)(use - 1) & 1u);      // every QK^T of its previous tile is done
             if (elect_one()) {
               mbar_expect_tx(bar_qfull(buf), C::QB);
@@ -350,37 +381,42 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
           const int G = gbase + g, s = G % C::NS;
           const uint32_t ph = (uint32_t)(G / C::NS) & 1u;
-          const int plane = g / c.np, part = g - plane * c.np;
           mbar_wait(bar_kempty(s), ph ^ 1u);
           if (lane == 0) TRACE(0, G);
           if (elect_one()) {
-            mbar_expect_tx(bar_kfull(s), C::NKEY * 128);
-            tma_load_5d(k_smem + s * C::STAGE, &tm_k, bar_kfull(s), 0, c.h, c.hs_x, c.hs_y + C::RH * part, c.bl + plane);
+            mbar_expect_tx(bar_kfull(s), (uint32_t)(C::part_rows(part) * C::HX * 128));
+            tma_load_5d(k_smem + s * C::STAGE, part == 1 ? &tm_kb : &tm_ka, bar_kfull(s), 0, c.h, c.hs_x,
+                        c.hs_y + C::part_begin(part), c.bl + plane);
           }
           __syncwarp();
+          if (++part == c.np) { part = 0; ++plane; }
         }
         gbase += c.nchunks;
       }
     } else if (warp == kWarpLoadV) {
       // =========================== TMA producer: V parts ===========================
       int gbase = 0;
-      for (int cl = 0, col; (col = col_of(cl)) >= 0; ++cl) {
-        const Col c = column(col);
+      ColIter it;
+      col_begin(it);
+      while (col_advance(it)) {
+        const Col& c = it.c;
+        int plane = 0, part = 0;
         for (int g = 0; g < c.nchunks; ++g) {
           const int G = gbase + g, s = G % C::NS;
           const uint32_t ph = (uint32_t)(G / C::NS) & 1u;
-          const int plane = g / c.np, part = g - plane * c.np;
           mbar_wait(bar_vempty(s), ph ^ 1u);
           if (lane == 0) TRACE(1, G);
           if (elect_one()) {
-            mbar_expect_tx(bar_vfull(s), C::NKEY * 128);
-            tma_load_5d(v_smem + s * C::STAGE, &tm_v, bar_vfull(s), 0, c.h, c.hs_x, c.hs_y + C::RH * part, c.bl + plane);
+            mbar_expect_tx(bar_vfull(s), (uint32_t)(C::part_rows(part) * C::HX * 128));
+            tma_load_5d(v_smem + s * C::STAGE, part == 1 ? &tm_vb : &tm_va, bar_vfull(s), 0, c.h, c.hs_x,
+                        c.hs_y + C::part_begin(part), c.bl + plane);
             // a slot whose tiles do not reach this plane never releases the stage: arrive for it
             const uint32_t nd = need[plane];
             if (!(nd & 1u)) mbar_arrive(bar_vempty(s));
             if (!(nd & 2u)) mbar_arrive(bar_vempty(s));
           }
           __syncwarp();
+          if (++part == c.np) { part = 0; ++plane; }
         }
         gbase += c.nchunks;
       }
@@ -389,20 +425,26 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // The whole warp walks the item sequence in uniform control flow; one elected lane issues and commits.
       const int slot = warp - kWarpMma;
       const uint32_t tm = tmem + slot * C::T_SLOT;
-      constexpr uint32_t idesc_qk = instr_desc(C::M, C::NPART, false);
-      constexpr uint32_t idesc_pv = instr_desc(C::M, C::D, true);
       // position of an item in the part stream
       struct Cur {
-        int col, cl, gbase, np, nchunks, h, t, plane, part, plo, phi;
+        int col, cl, hh, gbase, np, nchunks, t, plane, part, plo, phi;
         bool valid;
       };
       auto enter_tile = [&](Cur& w) { w.plo = tile_plo<C>(w.t, p.L); w.phi = tile_phi<C>(w.t, p.L); w.plane = w.plo; w.part = 0; };
+      // parts per plane of the cursor's unit (one call site: the divisions stay out of the item path)
+      auto unit_parts = [&](Cur& w) {
+        const int ty = (w.col / (p.H * p.ntx)) % p.nty;
+        const int y0 = ty * C::TY, yl = min(y0 + C::TY, p.Y) - 1;
+        const int hy = window_start(yl, C::KY, p.Y) + C::KY - window_start(y0, C::KY, p.Y);
+        w.np = hy > C::part_begin(2) ? 3 : hy > C::part_begin(1) ? 2 : 1;
+        w.nchunks = p.L * w.np;
+      };
       auto cur_init = [&](Cur& w) {
-        w.cl = 0; w.col = col_of(0); w.gbase = 0; w.t = slot;
+        w.cl = 0; w.hh = 0; w.gbase = 0; w.t = slot; w.np = 1; w.nchunks = 0;
+        w.col = (long long)blockIdx.x * p.hg < p.ncols ? (int)(blockIdx.x * p.hg) : -1;
         w.valid = w.col >= 0 && slot < ntl;
         if (!w.valid) return;
-        const Col c = column(w.col);
-        w.np = c.np; w.nchunks = c.nchunks;
+        unit_parts(w);
         enter_tile(w);
       };
       auto cur_next = [&](Cur& w) {
@@ -411,10 +453,15 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         if (++w.plane < w.phi) return;
         w.t += 2;
         if (w.t >= ntl) {
-          w.gbase += w.nchunks; ++w.cl; w.col = col_of(w.cl); w.t = slot;
-          if (w.col < 0) { w.valid = false; return; }
-          const Col c = column(w.col);
-          w.np = c.np; w.nchunks = c.nchunks;
+          w.gbase += w.nchunks; ++w.cl; w.t = slot;
+          if (++w.hh < p.hg) { ++w.col; }
+          else {                                  // next unit: the parts per plane may change
+            w.hh = 0;
+            const long long col = ((long long)blockIdx.x + (long long)(w.cl / p.hg) * gridDim.x) * p.hg;
+            if (col >= p.ncols) { w.valid = false; return; }
+            w.col = (int)col;
+            unit_parts(w);
+          }
         }
         enter_tile(w);
       };
@@ -422,22 +469,24 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       cur_init(wq); cur_init(wp);
       int iq = 0, ip = 0;
 
+      // QK^T of the next item of the QK cursor -> S[iq & 1].  The buffer is free: the PV MMA that read its P (item
+      // iq - 2) was issued before this call and the tensor pipe executes in issue order.
       auto issue_qk = [&]() {
         const int G = wq.gbase + wq.plane * wq.np + wq.part, s = G % C::NS;
         const uint32_t ph = (uint32_t)(G / C::NS) & 1u;
         const bool first = wq.plane == wq.plo && wq.part == 0;
         const bool last = wq.plane == wq.phi - 1 && wq.part == wq.np - 1;
         const int n = wq.cl * ntl + wq.t, buf = n % C::NQ;
+        const uint32_t idesc = wq.part == 1 ? instr_desc(C::M, C::NB, false) : instr_desc(C::M, C::NA, false);
+        const uint32_t lo_q = desc_lo(q_smem + buf * C::QB), lo_k = desc_lo(k_smem + s * C::STAGE);
         if (first) mbar_wait<false>(bar_qrot(buf), (uint32_t)(n / C::NQ) & 1u);          // Q tile rotated
         mbar_wait<false>(bar_krot(s), ph);                                                // K part rotated
-        if (iq >= 1) mbar_wait<false>(bar_slot(slot, 1), (uint32_t)(iq - 1) & 1u);        // S(iq - 1) is in registers
         tc_fence_after();
-        const uint32_t qb = q_smem + buf * C::QB, kb = k_smem + s * C::STAGE;
         if (elect_one()) {
 #pragma unroll
           for (int ks = 0; ks < C::D / 16; ++ks)
-            umma_ss(tm + C::T_S, smem_desc(qb + 32u * ks), smem_desc(kb + 32u * ks), idesc_qk, ks > 0 ? 1u : 0u);
-          umma_commit(bar_slot(slot, 0));
+            umma_ss(tm + C::T_S + (iq & 1) * C::NMAX, desc_from_lo(lo_q + 2u * ks), desc_from_lo(lo_k + 2u * ks), idesc, ks > 0 ? 1u : 0u);
+          umma_commit(bar_slot(slot, iq & 1));
           umma_commit(bar_kempty(s));
           if (last) umma_commit(bar_qfree(buf));
         }
@@ -446,22 +495,27 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         ++iq;
         cur_next(wq);
       };
+      // O (+)= P V of the next item of the PV cursor
       auto issue_pv = [&]() {
         const int G = wp.gbase + wp.plane * wp.np + wp.part, s = G % C::NS;
         const uint32_t ph = (uint32_t)(G / C::NS) & 1u;
         const bool first = wp.plane == wp.plo && wp.part == 0;
-        mbar_wait<false>(bar_slot(slot, 2), (uint32_t)ip & 1u);                           // P(ip) is in TMEM
+        const uint32_t lo_v = desc_lo(v_smem + s * C::STAGE);
+        const uint32_t a_tmem = tm + C::T_S + (ip & 1) * C::NMAX;
+        const bool mid = wp.part == 1;
+        mbar_wait<false>(bar_slot(slot, 2 + (ip & 1)), (uint32_t)(ip >> 1) & 1u);         // P(ip) is in TMEM
         if (lane == 0) TRACE(6 + slot, ip);
         mbar_wait<false>(bar_vfull(s), ph);
         tc_fence_after();
-        const uint32_t vb = v_smem + s * C::STAGE;
         const uint32_t acc0 = first ? 0u : 1u;
         if (elect_one()) {
+          constexpr uint32_t idesc_pv = instr_desc(C::M, C::D, true);
 #pragma unroll
-          for (int ks = 0; ks < C::NPART / 16; ++ks)
-            umma_ts(tm + C::T_O, tm + C::T_P + 8u * ks, smem_desc(vb + 2048u * ks), idesc_pv, ks > 0 ? 1u : acc0);
+          for (int ks = 0; ks < C::NB / 16; ++ks)
+            if (ks < C::NA / 16 || mid)
+              umma_ts(tm + C::T_O, a_tmem + 8u * ks, desc_from_lo(lo_v + 128u * ks), idesc_pv, ks > 0 ? 1u : acc0);
           umma_commit(bar_vempty(s));
-          umma_commit(bar_slot(slot, 3));
+          umma_commit(bar_slot(slot, 4 + (ip & 1)));
         }
         __syncwarp();
         if (lane == 0) TRACE(8 + slot, ip);
@@ -469,14 +523,15 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         cur_next(wp);
       };
       if (wq.valid) issue_qk();
+      if (wq.valid) issue_qk();
       while (wp.valid) {
-        if (wq.valid) issue_qk();
         issue_pv();
+        if (wq.valid) issue_qk();
       }
     }
   } else if (warp >= kWarpRot) {
     // =========================== rotation warpgroup ===========================
-    reg_dec<104>();
+    reg_dec<120>();
     const int tid = threadIdx.x - 32 * kWarpRot;
     const bool rope = p.A > 0;
     constexpr int NPF = PAIR ? 8 : 4;                                  // rotary pairs per table work item
@@ -491,43 +546,40 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     int gbase = 0;
     int tab_level = 0;
     bool invariant = true;
-    for (int cl = 0, col; (col = col_of(cl)) >= 0; ++cl) {
-      const Col c = column(col);
+    long long cidx[2] = {0, 0};          // halo tokens of this thread, tok = tid, tid + 128 (row-major over the halo): index at level 0
+    const long long lstride = (long long)p.Y * p.X;
+    ColIter it;
+    col_begin(it);
+    while (col_advance(it)) {
+      const Col& c = it.c;
       const int oy = c.y0 - c.hs_y, ox = c.x0 - c.hs_x;               // the Q tile inside the halo
-      // halo tokens of this thread: tok = tid, tid + 128 (part-major, then key row, then x)
-      long long cidx[2];
-      bool ctok[2];
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const int tok = tid + 128 * j;
-        ctok[j] = tok < 2 * C::NKEY;
-        const int pt = tok >= C::NKEY ? 1 : 0, r = tok - C::NKEY * pt;
-        const int hy = C::RH * pt + r / C::HX, hx = r % C::HX;
-        const int y = min(c.hs_y + hy, p.Y - 1), x = min(c.hs_x + hx, p.X - 1);
-        cidx[j] = (((long long)c.b * p.L) * p.Y + y) * p.X + x;         // level 0
-      }
-      const long long lstride = (long long)p.Y * p.X;
-      auto load_coords = [&](int level) {                               // coordinates of `level` -> cache
+      auto load_coords = [&](int level) {                               // coordinates of `level` -> cache; true: they differ from the cache
+        bool diff = false;
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-          if (!ctok[j]) continue;
+          const int tok = tid + 128 * j;
+          if (tok >= C::NTOK) continue;
           const float* src = coords + (cidx[j] + level * lstride) * p.A;
           float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
           v.x = src[0];
           if (p.A > 1) v.y = src[1];
           if (p.A > 2) v.z = src[2];
-          cc[tid + 128 * j] = v;
+          const float4 old = cc[tok];
+          diff |= __float_as_uint(old.x) != __float_as_uint(v.x) || __float_as_uint(old.y) != __float_as_uint(v.y) ||
+                  __float_as_uint(old.z) != __float_as_uint(v.z);
+          if (level == 0 || !invariant) cc[tok] = v;
         }
+        return diff;
       };
-      // A1: (cos, sin) of every halo token and rotary pair -> table, in the layout of a K part
+      // A1: (cos, sin) of every halo token and rotary pair -> table, in the layout of the K parts
       auto build_table = [&]() {
-#pragma unroll
-        for (int pt = 0; pt < 2; ++pt) {
+#pragma unroll 1
+        for (int pt = 0; pt < C::NPARTS; ++pt) {
+          const int nrow = C::part_rows(pt) * C::HX, tok0 = C::part_begin(pt) * C::HX;
           if constexpr (PAIR == 0) {
-            constexpr int NCH = C::NKEY * 8;
-#pragma unroll 2
-            for (int q = tid; q < NCH; q += 128) {
-              const float4 xyz = cc[pt * C::NKEY + (q >> 3)];
+#pragma unroll 1
+            for (int q = tid; q < nrow * 8; q += 128) {
+              const float4 xyz = cc[tok0 + (q >> 3)];
               float cs[4], sn[4];
 #pragma unroll
               for (int u = 0; u < 4; ++u) {
@@ -542,11 +594,10 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               sts128(t_smem + pt * C::STAGE + q * 16, w);
             }
           } else {
-            constexpr int NIT = C::NKEY * 4;
 #pragma unroll 1
-            for (int q = tid; q < NIT; q += 128) {
+            for (int q = tid; q < nrow * 4; q += 128) {
               const int row = q >> 2;
-              const float4 xyz = cc[pt * C::NKEY + row];
+              const float4 xyz = cc[tok0 + row];
               float cs[8], sn[8];
 #pragma unroll
               for (int u = 0; u < 8; ++u) {
@@ -565,62 +616,42 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
         }
       };
-      if (rope && cl % p.hg == 0) {
-        // First column of a unit (the others have the same tokens).  Level 0 -> cache; are the coordinates of
-        // the other levels the same bits?  (4 levels of loads in flight per pass.)
-        bool diff = false;
-        uint32_t c0[2][3];
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-#pragma unroll
-          for (int a = 0; a < 3; ++a) c0[j][a] = (ctok[j] && a < p.A) ? __float_as_uint(coords[cidx[j] * p.A + a]) : 0u;
-          if (ctok[j]) cc[tid + 128 * j] = make_float4(__uint_as_float(c0[j][0]), __uint_as_float(c0[j][1]), __uint_as_float(c0[j][2]), 0.f);
-        }
-#pragma unroll 1
-        for (int l0 = 1; l0 < p.L; l0 += 4) {
-          uint32_t cl_[4][2][3];
-#pragma unroll
-          for (int dl = 0; dl < 4; ++dl)
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const bool on = ctok[j] && l0 + dl < p.L;
-              const float* src = coords + (cidx[j] + (l0 + dl) * lstride) * p.A;
-              if (p.A == 2) {
-                float2 v = on ? *reinterpret_cast<const float2*>(src) : make_float2(__uint_as_float(c0[j][0]), __uint_as_float(c0[j][1]));
-                cl_[dl][j][0] = __float_as_uint(v.x); cl_[dl][j][1] = __float_as_uint(v.y); cl_[dl][j][2] = c0[j][2];
-              } else {
-#pragma unroll
-                for (int a = 0; a < 3; ++a) cl_[dl][j][a] = (on && a < p.A) ? __float_as_uint(src[a]) : c0[j][a];
-              }
-            }
-#pragma unroll
-          for (int dl = 0; dl < 4; ++dl)
-#pragma unroll
-            for (int j = 0; j < 2; ++j)
-#pragma unroll
-              for (int a = 0; a < 3; ++a) diff |= cl_[dl][j][a] != c0[j][a];
-        }
-        invariant = !rot_sync_or(diff);         // (also: every thread has left the previous unit's table, the cache is written)
-        build_table();
-        rot_sync();
-        tab_level = 0;
-      }
-      // the table of `level` must be in shared memory (a no-op when the coordinates are level invariant)
+      // The table of `level` must be in shared memory.  level < 0: new unit (level 0 is loaded and the other
+      // levels are compared with it).  ONE copy of the table code in the kernel.
       auto ensure_table = [&](int level) {
-        if (invariant || level == tab_level) return;
-        rot_sync();                               // everyone is done with the current table and cache
-        load_coords(level);
-        rot_sync();
+        if (!rope) return;
+        if (level >= 0 && (invariant || level == tab_level)) return;
+        rot_sync();                                 // everyone is done with the current table and cache
+        if (level < 0) {
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const int tok = tid + 128 * j;
+            const int hyr = tok / C::HX, hx = tok - hyr * C::HX;
+            const int y = min(c.hs_y + hyr, p.Y - 1), x = min(c.hs_x + hx, p.X - 1);
+            cidx[j] = (((long long)c.b * p.L) * p.Y + y) * p.X + x;
+          }
+          invariant = true;
+          load_coords(0);
+          bool diff = false;
+#pragma unroll 1
+          for (int l = 1; l < p.L; ++l) diff |= load_coords(l);     // (compares only: `invariant` is still set)
+          invariant = !rot_sync_or(diff);
+          level = 0;
+        } else {
+          load_coords(level);
+          rot_sync();
+        }
         build_table();
         rot_sync();
         tab_level = level;
       };
+      if (it.hh == 0) ensure_table(-1);
 
-      int tq = 0;
+      int tq = 0, plane = 0, part = 0;
       for (int g = 0; g < c.nchunks; ++g) {
         // ---- Q tiles due before this part
         while (tq < ntl && qpos(tq, c.np) == g) {
-          const int n = cl * ntl + tq, buf = n % C::NQ;
+          const int n = it.cl * ntl + tq, buf = n % C::NQ;
           mbar_wait(bar_qfull(buf), (uint32_t)(n / C::NQ) & 1u);
           if (rope) {
 #pragma unroll 1
@@ -633,8 +664,9 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                   const int q = tid + 128 * k, rr = q >> 3;                        // row of the level, physical chunk q & 7
-                  const int hy = (rr >> 3) + oy, pt = hy >= C::RH ? 1 : 0;
-                  const int tr = (hy - C::RH * pt) * C::HX + (rr & 7) + ox;        // table row of the query's token
+                  const int hyr = (rr >> 3) + oy;
+                  const int pt = hyr >= C::part_begin(2) ? 2 : hyr >= C::part_begin(1) ? 1 : 0;
+                  const int tr = (hyr - C::part_begin(pt)) * C::HX + (rr & 7) + ox;      // table row of the query's token
                   const uint32_t cl16 = (uint32_t)((q & 7) ^ (rr & 7));            // logical chunk
                   xa[k] = qb + q * 16;
                   x[k] = lds128(xa[k]);
@@ -650,8 +682,9 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
                 for (int k = 0; k < 2; ++k) {
                   const int q = tid + 128 * k, rr = q >> 2;                        // row of the level, logical chunk cch
-                  const int hy = (rr >> 3) + oy, pt = hy >= C::RH ? 1 : 0;
-                  const int tr = (hy - C::RH * pt) * C::HX + (rr & 7) + ox;
+                  const int hyr = (rr >> 3) + oy;
+                  const int pt = hyr >= C::part_begin(2) ? 2 : hyr >= C::part_begin(1) ? 1 : 0;
+                  const int tr = (hyr - C::part_begin(pt)) * C::HX + (rr & 7) + ox;
                   const uint32_t xr = qb + rr * 128, sw = (uint32_t)(rr & 7);
                   const uint32_t trb = t_smem + pt * C::STAGE + tr * 128, tsw = (uint32_t)(tr & 7);
                   aa[k] = xr + (((uint32_t)cch ^ sw) << 4); ba[k] = xr + (((uint32_t)(cch + 4) ^ sw) << 4);
@@ -671,61 +704,50 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         }
         // ---- K part g
         const int G = gbase + g, s = G % C::NS;
-        const int plane = g / c.np, part = g - plane * c.np;
         if (tid == 0) TRACE(2, G);
         mbar_wait(bar_kfull(s), (uint32_t)(G / C::NS) & 1u);
         if (tid == 0) TRACE(3, G);
         if (rope) {
           ensure_table(plane);
           const uint32_t kb = k_smem + s * C::STAGE, tb = t_smem + part * C::STAGE;
+          const int nrow = C::part_rows(part) * C::HX;
           if constexpr (PAIR == 0) {
-            // The table part has the K part's geometry, so the loop is linear over physical 16-byte chunks.
-            constexpr int NCH = C::NKEY * 8, NIT = (NCH + 127) / 128;
-#pragma unroll
-            for (int k0 = 0; k0 < NIT; k0 += 4) {
+            // The table part has the K part's geometry, so the loop is linear over physical 16-byte chunks;
+            // four chunks per thread in flight.
+            const int nch = nrow * 8;
+#pragma unroll 1
+            for (int q0 = tid; q0 < nch; q0 += 512) {
               uint4 x[4], t[4];
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                const int k = k0 + j;
-                if (k < NIT && ((k + 1) * 128 <= NCH || tid + 128 * k < NCH)) {
-                  x[j] = lds128(kb + (tid + 128 * k) * 16);
-                  t[j] = lds128(tb + (tid + 128 * k) * 16);
-                }
-              }
+              for (int j = 0; j < 4; ++j)
+                if (q0 + 128 * j < nch) { x[j] = lds128(kb + (q0 + 128 * j) * 16); t[j] = lds128(tb + (q0 + 128 * j) * 16); }
+#pragma unroll
+              for (int j = 0; j < 4; ++j) rot_chunk(x[j], t[j]);
 #pragma unroll
               for (int j = 0; j < 4; ++j)
-                if (k0 + j < NIT) rot_chunk(x[j], t[j]);
-#pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                const int k = k0 + j;
-                if (k < NIT && ((k + 1) * 128 <= NCH || tid + 128 * k < NCH)) sts128(kb + (tid + 128 * k) * 16, x[j]);
-              }
+                if (q0 + 128 * j < nch) sts128(kb + (q0 + 128 * j) * 16, x[j]);
             }
           } else {
-            constexpr int NITM = C::NKEY * 4, NIT = (NITM + 127) / 128;
-#pragma unroll
-            for (int k0 = 0; k0 < NIT; k0 += 2) {
+            const int nit = nrow * 4;
+#pragma unroll 1
+            for (int q0 = tid; q0 < nit; q0 += 256) {
               uint4 a[2], b[2], tc_[2], ts_[2];
               uint32_t ao[2], bo[2];
 #pragma unroll
               for (int j = 0; j < 2; ++j) {
-                const int k = k0 + j;
-                if (k < NIT && ((k + 1) * 128 <= NITM || tid + 128 * k < NITM)) {
-                  const int row = (tid + 128 * k) >> 2;
-                  const uint32_t sw = (uint32_t)(row & 7);
-                  ao[j] = row * 128 + (((uint32_t)cch ^ sw) << 4); bo[j] = row * 128 + (((uint32_t)(cch + 4) ^ sw) << 4);
+                const int row = (q0 + 128 * j) >> 2;
+                const uint32_t sw = (uint32_t)(row & 7);
+                ao[j] = row * 128 + (((uint32_t)cch ^ sw) << 4); bo[j] = row * 128 + (((uint32_t)(cch + 4) ^ sw) << 4);
+                if (q0 + 128 * j < nit) {
                   a[j] = lds128(kb + ao[j]); b[j] = lds128(kb + bo[j]);
                   tc_[j] = lds128(tb + ao[j]); ts_[j] = lds128(tb + bo[j]);
                 }
               }
 #pragma unroll
-              for (int j = 0; j < 2; ++j)
-                if (k0 + j < NIT) rot_chunks_half(a[j], b[j], tc_[j], ts_[j]);
+              for (int j = 0; j < 2; ++j) rot_chunks_half(a[j], b[j], tc_[j], ts_[j]);
 #pragma unroll
-              for (int j = 0; j < 2; ++j) {
-                const int k = k0 + j;
-                if (k < NIT && ((k + 1) * 128 <= NITM || tid + 128 * k < NITM)) { sts128(kb + ao[j], a[j]); sts128(kb + bo[j], b[j]); }
-              }
+              for (int j = 0; j < 2; ++j)
+                if (q0 + 128 * j < nit) { sts128(kb + ao[j], a[j]); sts128(kb + bo[j], b[j]); }
             }
           }
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -739,36 +761,30 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           if (!(nd & 1u)) mbar_arrive(bar_kempty(s));
           if (!(nd & 2u)) mbar_arrive(bar_kempty(s));
         }
+        if (++part == c.np) { part = 0; ++plane; }
       }
       gbase += c.nchunks;
     }
   } else {
     // =========================== softmax + epilogue of one slot ===========================
-    reg_inc<176>();
+    reg_inc<168>();
     const int slot = warp >> 2;
     const int sp = warp & 3;                       // TMEM subpartition
     const int row = sp * 32 + lane;                // query row of the tile == TMEM lane
     const uint32_t tm = pinned(tmem + slot * C::T_SLOT + ((uint32_t)(sp * 32) << 16));
     const int qx = row % C::TX, qy = (row / C::TX) % C::TY, ql = row / (C::TX * C::TY);
     const float cs = p.scale_log2e;
-    const uint32_t bar_sfull = pinned(bar_slot(slot, 0)), bar_sfree = pinned(bar_slot(slot, 1)), bar_pfull = pinned(bar_slot(slot, 2)),
-                   bar_pvdone = pinned(bar_slot(slot, 3));
-    // pad keys of a part: P = 0 for good (nothing else writes these columns)
-    if constexpr (C::NPART / 2 > C::RH * C::PW) {
-      uint32_t z[C::NPART / 2 - C::RH * C::PW];
-#pragma unroll
-      for (int u = 0; u < C::NPART / 2 - C::RH * C::PW; ++u) z[u] = 0u;
-      tmem_st_n<C::NPART / 2 - C::RH * C::PW>(tm + C::T_P + C::RH * C::PW, z);
-      tmem_wait_st();
-    }
+    const uint32_t bar_s0 = pinned(bar_slot(slot, 0)), bar_p0 = pinned(bar_slot(slot, 2)), bar_pv0 = pinned(bar_slot(slot, 4));
     int i = 0;                                      // item counter of the slot
-    // epilogue of the previous tile, run inside the first item of the next one (see do_tail)
+    // epilogue of the previous tile, run inside the first item of the next one
     bool ep = false, ep_active = false;
     float ep_inv = 0.f, ep_lse = 0.f;
     __nv_bfloat16* ep_orow = nullptr;
     float* ep_lrow = nullptr;
     auto epilogue = [&]() {
-      // O / l -> bf16 -> global, LSE.  Every PV MMA of the tile is complete (pv_done of its last item).
+      // O / l -> bf16 -> global, LSE.  Every PV MMA of the tile must be complete: pv_done of its last item.
+      mbar_wait(bar_pv0 + 8u * ((i - 1) & 1), (uint32_t)((i - 1) >> 1) & 1u);
+      tc_fence_after();
 #pragma unroll 1
       for (int j = 0; j < C::D; j += 16) {
         float ov[16];
@@ -787,56 +803,45 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (ep_active) *ep_lrow = ep_lse;
       ep = false;
     };
-    // Before P(i) may be stored: the PV MMA of item i - 1 has read the P columns (it was issued when item i - 1
-    // ended, a whole S load and fold ago); O then holds every item up to i - 1, so a finished tile is written out
-    // here, overlapped with the MMAs of the other slot.
-    auto do_tail_begin = [&]() {
-      if (sp == 0 && lane == 0) TRACE(13 + 5 * slot, i);
-      if (i >= 1) {
-        mbar_wait(bar_pvdone, (uint32_t)(i - 1) & 1u);
-        tc_fence_after();
-      }
-      if (sp == 0 && lane == 0) TRACE(14 + 5 * slot, i);
-      if (ep) epilogue();
-    };
-    auto do_tail_end = [&]() {
-      tmem_wait_st();
-      tc_fence_before();
-      if (sp == 0 && lane == 0) TRACE(15 + 5 * slot, i);
-      warp_arrive(bar_pfull);
-      ++i;
-    };
 
-    for (int cl = 0, col; (col = col_of(cl)) >= 0; ++cl) {
-      const Col c = column(col);
-      const int ax = min(c.x0 + qx, p.X - 1), ay = min(c.y0 + qy, p.Y - 1);
-      const bool active_xy = (c.x0 + qx < p.X) && (c.y0 + qy < p.Y);
-      const int lo_x = window_start(ax, C::KX, p.X) - c.hs_x;
-      const int lo_y = window_start(ay, C::KY, p.Y) - c.hs_y;
-      const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
-      const uint32_t rowbits = ((1u << C::KY) - 1u) << lo_y;       // halo rows inside this query's window
-      // x fold: of the halo columns c and c + HALF at most one lies in this query's window
-      uint32_t m_lo[C::HALF];                        // all ones: column c is the one (else c + HALF, or neither)
-      float xz[C::HALF];                             // 0 if one of the two is in the window, else -inf
+    // per-unit constants of this query row (the columns of a unit share the tile, hence the windows)
+    int ax = 0, ay = 0, wy_lo = 0, wy_hi = 0;
+    bool active_xy = false;
+    uint32_t rowbits = 0;                           // halo rows inside this query's window
+    uint32_t m_lo[C::HALF];                         // x fold: all ones: column c is in the window (else c + HALF, or neither)
+    float xz[C::HALF];                              // 0 if one of the two is in the window, else -inf
+    uint32_t psel[C::PW];                           // un-fold selectors, see below
+    ColIter it;
+    col_begin(it);
+    while (col_advance(it)) {
+      const Col& c = it.c;
+      if (it.hh == 0) {
+        ax = min(c.x0 + qx, p.X - 1); ay = min(c.y0 + qy, p.Y - 1);
+        active_xy = (c.x0 + qx < p.X) && (c.y0 + qy < p.Y);
+        const int lo_x = window_start(ax, C::KX, p.X) - c.hs_x;
+        const int lo_y = window_start(ay, C::KY, p.Y) - c.hs_y;
+        wy_lo = __reduce_min_sync(0xffffffffu, lo_y); wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
+        rowbits = ((1u << C::KY) - 1u) << lo_y;
+        // x fold: of the halo columns c and c + HALF at most one lies in this query's window
 #pragma unroll
-      for (int cc_ = 0; cc_ < C::HALF; ++cc_) {
-        const bool in_lo = cc_ >= lo_x && cc_ < lo_x + C::KX, in_hi = cc_ + C::HALF >= lo_x && cc_ + C::HALF < lo_x + C::KX;
-        m_lo[cc_] = in_lo ? 0xffffffffu : 0u;
-        xz[cc_] = (in_lo || in_hi) ? 0.f : -INFINITY;
-      }
-      // un-fold: P word j holds the halo columns (2j, 2j+1).  Column col comes from the folded value
-      // fc = col mod HALF, which sits in half (fc & 1) of the packed word F[fc / 2]; psel[j] is the byte
-      // selector of prmt(F[fc(2j) / 2], F[fc(2j+1) / 2]).  A column outside the window selects "sign of a
-      // high byte", which is 0x00 because every P value is >= +0.
-      uint32_t psel[C::PW];
+        for (int cc_ = 0; cc_ < C::HALF; ++cc_) {
+          const bool in_lo = cc_ >= lo_x && cc_ < lo_x + C::KX, in_hi = cc_ + C::HALF >= lo_x && cc_ + C::HALF < lo_x + C::KX;
+          m_lo[cc_] = in_lo ? 0xffffffffu : 0u;
+          xz[cc_] = (in_lo || in_hi) ? 0.f : -INFINITY;
+        }
+        // un-fold: P word j holds the halo columns (2j, 2j+1).  Column col comes from the folded value
+        // fc = col mod HALF, which sits in half (fc & 1) of the packed word F[fc / 2]; psel[j] is the byte
+        // selector of prmt(F[fc(2j) / 2], F[fc(2j+1) / 2]).  A column outside the window selects "sign of a
+        // high byte", which is 0x00 because every P value is >= +0.
 #pragma unroll
-      for (int j = 0; j < C::PW; ++j) {
-        const int c0 = 2 * j, c1 = 2 * j + 1;
-        const int f0 = c0 % C::HALF, f1 = c1 % C::HALF;
-        const bool v0 = c0 >= lo_x && c0 < lo_x + C::KX, v1 = c1 >= lo_x && c1 < lo_x + C::KX;
-        const uint32_t n0 = v0 ? (uint32_t)(2 * (f0 & 1)) | ((uint32_t)(2 * (f0 & 1) + 1) << 4) : 0x99u;
-        const uint32_t n1 = v1 ? (uint32_t)(4 + 2 * (f1 & 1)) | ((uint32_t)(5 + 2 * (f1 & 1)) << 4) : 0xDDu;
-        psel[j] = n0 | (n1 << 8);
+        for (int j = 0; j < C::PW; ++j) {
+          const int c0 = 2 * j, c1 = 2 * j + 1;
+          const int f0 = c0 % C::HALF, f1 = c1 % C::HALF;
+          const bool v0 = c0 >= lo_x && c0 < lo_x + C::KX, v1 = c1 >= lo_x && c1 < lo_x + C::KX;
+          const uint32_t n0 = v0 ? (uint32_t)(2 * (f0 & 1)) | ((uint32_t)(2 * (f0 & 1) + 1) << 4) : 0x99u;
+          const uint32_t n1 = v1 ? (uint32_t)(4 + 2 * (f1 & 1)) | ((uint32_t)(5 + 2 * (f1 & 1)) << 4) : 0xDDu;
+          psel[j] = n0 | (n1 << 8);
+        }
       }
 
       for (int tile = slot; tile < ntl; tile += 2) {
@@ -849,159 +854,139 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         for (int plane = plo; plane < phi; ++plane) {
           const bool plane_ok = plane >= pw_lo && plane < pw_lo + C::KL;
 #pragma unroll 1
-          for (int part = 0; part < c.np; ++part) {
+          for (int part = 0; part < c.np; ++part, ++i) {
             const bool first_item = (plane == plo && part == 0);
-            // Key rows of this part some query of the warp attends: [ra, rb) (warp-uniform).  The part's RH rows
-            // are covered by two row groups, A = rows [0, RA) and B = RB rows starting at row r0b; a warp that
-            // needs only the part's first or last RB rows runs group B alone.
-            const int ra = max(wy_lo - C::RH * part, 0), rb = min(wy_hi - C::RH * part, C::RH);
-            bool do_a = true, do_b = true;
-            int r0b = C::RA;
-            if (!plane_ok || ra >= rb) { do_a = false; do_b = false; }
-            else if (rb <= C::RB) { do_a = false; r0b = 0; }
-            else if (ra >= C::RA) { do_a = false; }
-            const uint32_t pbits = rowbits >> (C::RH * part);          // this query's rows of the part
-            const uint32_t bits_a = do_a ? (pbits & ((1u << C::RA) - 1u)) : 0u;
-            const uint32_t bits_b = do_b ? ((pbits >> r0b) & ((1u << C::RB) - 1u)) : 0u;
+            const int pb = C::part_begin(part), nrows = C::part_rows(part);
+            // key rows of this part some query of the warp attends: [ra, rb) (warp-uniform)
+            const int ra = plane_ok ? max(wy_lo - pb, 0) : 0, rb = plane_ok ? min(wy_hi - pb, nrows) : 0;
+            const uint32_t pbits = plane_ok ? (rowbits >> pb) & ((1u << nrows) - 1u) : 0u;       // this query's rows of the part
+            const uint32_t s_tm = tm + C::T_S + (i & 1) * C::NMAX;   // S of the item; P goes over its front
             if (sp == 0 && lane == 0) TRACE(11 + 5 * slot, i);
-            mbar_wait(bar_sfull, (uint32_t)i & 1u);
+            mbar_wait(bar_s0 + 8u * (i & 1), (uint32_t)(i >> 1) & 1u);
             if (sp == 0 && lane == 0) TRACE(12 + 5 * slot, i);
             tc_fence_after();
-            // ---- S -> registers, folded, one row group after the other (the whole TMA box: rows past the halo are
-            // zero keys, outside every window); then S may be overwritten by the next QK^T
-            float va[C::RA][C::HALF], vb[C::RB][C::HALF];       // folded logits
-            auto load_fold = [&](auto& v, auto rc, const int r0) {
-              constexpr int R = decltype(rc)::value;
-              uint32_t sv[R * C::HX];
-              tmem_ld_n<R * C::HX>(tm + C::T_S + r0 * C::HX, sv);
-#pragma unroll
-              for (int r = 0; r < R; ++r)
-#pragma unroll
-                for (int cc_ = 0; cc_ < C::HALF; ++cc_)
-                  v[r][cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[r * C::HX + cc_], sv[r * C::HX + cc_ + C::HALF]));
-            };
-            if (do_a) load_fold(va, std::integral_constant<int, C::RA>{}, 0);
-            if (do_b) load_fold(vb, std::integral_constant<int, C::RB>{}, r0b);
-            if (slot == 0 && sp == 0 && lane == 0) TRACE(21, i);
-            tc_fence_before();
-            warp_arrive(bar_sfree);
+            if (ep) epilogue();                       // (the O of the previous tile: before this item's p_full lets the first PV MMA of the new tile go)
 
-            // One row group: p = 2^(s * cs - m_ref), row sum, packed bf16 P in registers.  Branch-free over the rows; the
-            // exponentials (MUFU) of a row overlap the pack / un-fold arithmetic of its neighbours.  `prev` / NPREV: the
-            // P words of the item's other group, already computed against the current reference.
-            auto row_group = [&](auto& v, auto rc, const uint32_t bits, uint32_t* pw, uint32_t* prev, auto nprev, const bool has_prev) {
-              constexpr int R = decltype(rc)::value, NPREV = decltype(nprev)::value;
-              // maximum of this query's valid logits of the group (log2 units)
-              // (the scale goes through an opaque register, so that the compiler cannot hoist this rarely needed
-              // computation out of its branches)
-              auto group_max = [&]() {
-                float csm = cs;
-                asm volatile("mov.f32 %0, %0;" : "+f"(csm));
-                float cmax = -INFINITY;
+            // one key row of S -> registers, folded (the whole TMA box: rows past the halo are zero keys, outside
+            // every window)
+            auto load_row = [&](int r, float (&v)[C::HALF]) {
+              uint32_t sv[C::HX];
+              tmem_ld_n<C::HX>(s_tm + r * C::HX, sv);
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                  float rmax = -INFINITY;
+              for (int cc_ = 0; cc_ < C::HALF; ++cc_) v[cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[cc_], sv[cc_ + C::HALF]));
+            };
+            auto row_max = [&](const float (&v)[C::HALF]) {
+              float rmax = -INFINITY;
 #pragma unroll
-                  for (int cc_ = 0; cc_ < C::HALF; ++cc_) rmax = fmaxf(rmax, C::FULLFOLD ? v[r][cc_] * csm : fmaf(v[r][cc_], csm, xz[cc_]));
-                  if ((bits >> r) & 1u) cmax = fmaxf(cmax, rmax);
-                }
-                return cmax;
-              };
-              if (__any_sync(0xffffffffu, bits != 0u && !inited)) {
-                // ---- first valid keys of some query: its reference is the true maximum of this group
-                const float cmax = group_max();
-                if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
+              for (int cc_ = 0; cc_ < C::HALF; ++cc_) rmax = fmaxf(rmax, C::FULLFOLD ? v[cc_] * cs : fmaf(v[cc_], cs, xz[cc_]));
+              return rmax;
+            };
+            // ---- queries that see their first valid keys: their reference is the true maximum of this part
+            if (__any_sync(0xffffffffu, pbits != 0u && !inited)) {
+              float cmax = -INFINITY;
+#pragma unroll 1
+              for (int r = ra; r < rb; ++r) {
+                float v[C::HALF];
+                load_row(r, v);
+                const float rmax = row_max(v);
+                if ((pbits >> r) & 1u) cmax = fmaxf(cmax, rmax);
               }
-              float rs = 0.f;
-              int attempt = 0;
+              if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
+            }
+            // ---- the key rows of the part, one at a time: P row r overwrites S columns [PW r, PW r + PW), all of
+            // them read (rows <= r / 2) before
 #pragma unroll 1
-              do {                                     // (rare block first: ONE copy of the pass in the code)
-                if (attempt > 0) {
-                  // ---- a logit far above the reference: raise the reference by a whole number of octaves (every
-                  // factor below is then an exact power of two) and rescale what was accumulated so far
-                  const bool mine = !(rs <= kBig);
-                  float k = mine ? ceilf(group_max() - m_ref) : 0.f;
-                  if (!(k > 0.f)) k = 0.f;
-                  const float alpha = ex2(-k);
-                  if (!first_item) {
-                    // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
-                    mbar_wait(bar_pvdone, (uint32_t)(i - 1) & 1u);
-                    tc_fence_after();
+            for (int r = 0; r < nrows; ++r) {
+              uint32_t pw[C::PW];
+              if (r >= ra && r < rb) {
+                float v[C::HALF];
+                load_row(r, v);
+                float rs;
+                float pr[C::HALF + 1];               // folded probabilities (times 2^-m_ref)
+                pr[C::HALF] = 0.f;
+                int attempt = 0;
 #pragma unroll 1
-                    for (int j = 0; j < C::D; j += 16) {
-                      float ov[16];
-                      tmem_ld16(tm + C::T_O + j, ov);
-                      tmem_wait_ld();
-                      uint32_t ow[16];
+                do {                                 // (rare block first: ONE copy of the exponentials in the code)
+                  if (attempt > 0) {
+                    // ---- a logit far above the reference: raise the reference by a whole number of octaves (every
+                    // factor below is an exact power of two) and rescale what was accumulated so far
+                    float k = !(rs <= kBig) ? ceilf(row_max(v) - m_ref) : 0.f;
+                    if (!(k > 0.f)) k = 0.f;
+                    const float alpha = ex2(-k);
+                    if (!first_item) {
+                      // O holds earlier parts of this tile: all its PV MMAs are complete after pv_done(i - 1)
+                      mbar_wait(bar_pv0 + 8u * ((i - 1) & 1), (uint32_t)((i - 1) >> 1) & 1u);
+                      tc_fence_after();
+#pragma unroll 1
+                      for (int j = 0; j < C::D; j += 16) {
+                        float ov[16];
+                        tmem_ld16(tm + C::T_O + j, ov);
+                        tmem_wait_ld();
+                        uint32_t ow[16];
 #pragma unroll
-                      for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
-                      tmem_st16(tm + C::T_O + j, ow);
+                        for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
+                        tmem_st16(tm + C::T_O + j, ow);
+                      }
+                    }
+                    // the P rows of this item stored so far
+                    tmem_wait_st();
+                    const uint32_t a2 = pack_bf16(alpha, alpha);
+#pragma unroll 1
+                    for (int j = ra * C::PW; j < r * C::PW; ++j) {
+                      uint32_t w;
+                      tmem_ld_x1(s_tm + j, &w);
+                      tmem_wait_ld();
+                      w = bmul2(w, a2);
+                      tmem_st_x1(s_tm + j, &w);
                     }
                     tmem_wait_st();
+                    lsum *= alpha;
+                    m_ref += k;
                   }
-                  if (NPREV > 0 && has_prev) {
-                    const uint32_t a2 = pack_bf16(alpha, alpha);
-#pragma unroll
-                    for (int j = 0; j < NPREV; ++j) prev[j] = bmul2(prev[j], a2);
-                  }
-                  lsum *= alpha;
-                  m_ref += k;
-                }
-                float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                  const float br = ((bits >> r) & 1u) ? -m_ref : -INFINITY;
-                  float pr[C::HALF + 1];               // folded probabilities (times 2^-m_ref)
-                  pr[C::HALF] = 0.f;
+                  const float br = ((pbits >> r) & 1u) ? -m_ref : -INFINITY;
+                  float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
 #pragma unroll
                   for (int cc_ = 0; cc_ < C::HALF; cc_ += 2) {
                     if (cc_ + 1 < C::HALF) {
                       float t0, t1;
-                      if (C::FULLFOLD) ffma2(t0, t1, v[r][cc_], v[r][cc_ + 1], cs, br, br);
-                      else ffma2(t0, t1, v[r][cc_], v[r][cc_ + 1], cs, br + xz[cc_], br + xz[cc_ + 1]);
+                      if (C::FULLFOLD) ffma2(t0, t1, v[cc_], v[cc_ + 1], cs, br, br);
+                      else ffma2(t0, t1, v[cc_], v[cc_ + 1], cs, br + xz[cc_], br + xz[cc_ + 1]);
                       pr[cc_] = ex2(t0); pr[cc_ + 1] = ex2(t1);
                       if ((cc_ >> 1) & 1) fadd2(e2, e3, e2, e3, pr[cc_], pr[cc_ + 1]);
                       else fadd2(e0, e1, e0, e1, pr[cc_], pr[cc_ + 1]);
                     } else {
-                      pr[cc_] = ex2(fmaf(v[r][cc_], cs, C::FULLFOLD ? br : br + xz[cc_]));
+                      pr[cc_] = ex2(fmaf(v[cc_], cs, C::FULLFOLD ? br : br + xz[cc_]));
                       e0 += pr[cc_];
                     }
                   }
-                  // pack folded pairs to bf16x2, un-fold with one byte permute per output word
-                  uint32_t f[C::NF];
+                  rs = (e0 + e1) + (e2 + e3);
+                  ++attempt;
+                } while (attempt < 2 && __any_sync(0xffffffffu, !(rs <= kBig)));
+                lsum += rs;
+                // pack folded pairs to bf16x2, un-fold with one byte permute per output word
+                uint32_t f[C::NF];
 #pragma unroll
-                  for (int m = 0; m < C::NF; ++m) f[m] = pack_bf16(pr[2 * m], pr[2 * m + 1]);
+                for (int m = 0; m < C::NF; ++m) f[m] = pack_bf16(pr[2 * m], pr[2 * m + 1]);
 #pragma unroll
-                  for (int j = 0; j < C::PW; ++j)
-                    pw[r * C::PW + j] = prmt(f[((2 * j) % C::HALF) / 2], f[((2 * j + 1) % C::HALF) / 2], psel[j]);
-                }
-                rs = (e0 + e1) + (e2 + e3);
-                ++attempt;
-              } while (attempt < 2 && __any_sync(0xffffffffu, !(rs <= kBig)));
-              lsum += rs;
-            };
-            uint32_t pa[C::RA * C::PW], pb[C::RB * C::PW];
-            if (do_a) row_group(va, std::integral_constant<int, C::RA>{}, bits_a, pa, pa, std::integral_constant<int, 0>{}, false);
-            if (do_b) row_group(vb, std::integral_constant<int, C::RB>{}, bits_b, pb, pa, std::integral_constant<int, C::RA * C::PW>{}, do_a);
-            if (slot == 0 && sp == 0 && lane == 0) TRACE(23, i);
-            // ---- P -> TMEM once the PV MMA of the previous item has read the P columns
-            do_tail_begin();
-            if (do_a) tmem_st_n<C::RA * C::PW>(tm + C::T_P, pa);
-            if (do_b) tmem_st_n<C::RB * C::PW>(tm + C::T_P + r0b * C::PW, pb);
-            // ---- the rows of the part no query of the warp attends: P = 0
-            if (!do_a) {
-              uint32_t z[C::RA * C::PW];
+                for (int j = 0; j < C::PW; ++j) pw[j] = prmt(f[((2 * j) % C::HALF) / 2], f[((2 * j + 1) % C::HALF) / 2], psel[j]);
+              } else {
 #pragma unroll
-              for (int u = 0; u < C::RA * C::PW; ++u) z[u] = 0u;
-              tmem_st_n<C::RA * C::PW>(tm + C::T_P + (r0b == 0 ? C::RB * C::PW : 0), z);
+                for (int j = 0; j < C::PW; ++j) pw[j] = 0u;   // a key row no query of the warp attends
+              }
+              tmem_st_n<C::PW>(s_tm + r * C::PW, pw);
             }
-            if (!do_b) {
-              uint32_t z[C::RB * C::PW];
+            // pad keys of the part (stale rows of the K / V stage): P = 0
+            {
+              uint32_t z[8];
 #pragma unroll
-              for (int u = 0; u < C::RB * C::PW; ++u) z[u] = 0u;
-              tmem_st_n<C::RB * C::PW>(tm + C::T_P + C::RA * C::PW, z);
+              for (int u = 0; u < 8; ++u) z[u] = 0u;
+              if (part == 1) { if constexpr (C::NB / 2 > C::RB * C::PW) tmem_st_n<C::NB / 2 - C::RB * C::PW>(s_tm + C::RB * C::PW, z); }
+              else { if constexpr (C::NA / 2 > C::RA * C::PW) tmem_st_n<C::NA / 2 - C::RA * C::PW>(s_tm + C::RA * C::PW, z); }
             }
-            do_tail_end();
+            tmem_wait_st();
+            tc_fence_before();
+            if (sp == 0 && lane == 0) TRACE(15 + 5 * slot, i);
+            warp_arrive(bar_p0 + 8u * (i & 1));
           }
         }
         // ---- the tile is written out inside the next item of this slot (or after the loop)
@@ -1013,11 +998,7 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         ep_lrow = lse + ((long long)c.b * p.H + c.h) * p.N + tok;
       }
     }
-    if (ep) {
-      mbar_wait(bar_pvdone, (uint32_t)(i - 1) & 1u);
-      tc_fence_after();
-      epilogue();
-    }
+    if (ep) epilogue();
   }
 
   // ---- teardown
@@ -1066,8 +1047,9 @@ DeviceState* device_state() {
 template <class C>
 cudaError_t launch_sweep(const Problem& p, int cfg_index, const void* q, const void* k, const void* v, const float* coords,
                          const float* freqs, void* o, float* lse, cudaStream_t stream, int* launches) {
-  CUtensorMap tq, tk, tv;
-  if (!make_map(&tq, q, p, C::TX, C::TY, C::TL) || !make_map(&tk, k, p, C::HX, C::RH, 1) || !make_map(&tv, v, p, C::HX, C::RH, 1))
+  CUtensorMap tq, tka, tkb, tva, tvb;
+  if (!make_map(&tq, q, p, C::TX, C::TY, C::TL) || !make_map(&tka, k, p, C::HX, C::RA, 1) || !make_map(&tkb, k, p, C::HX, C::RB, 1) ||
+      !make_map(&tva, v, p, C::HX, C::RA, 1) || !make_map(&tvb, v, p, C::HX, C::RB, 1))
     return cudaErrorInvalidValue;
   SweepParams sp;
   sp.B = p.B; sp.H = p.H; sp.L = p.L; sp.Y = p.Y; sp.X = p.X; sp.N = p.N;
@@ -1106,7 +1088,7 @@ cudaError_t launch_sweep(const Problem& p, int cfg_index, const void* q, const v
     ds->attr[ai] = true;
   }
   prof_begin("na3d_fwd_sweep", stream);
-  kernel<<<(unsigned)grid, kSweepThreads, C::SMEM_BYTES, stream>>>(tq, tk, tv, coords, freqs, (__nv_bfloat16*)o, lse, sp);
+  kernel<<<(unsigned)grid, kSweepThreads, C::SMEM_BYTES, stream>>>(tq, tka, tkb, tva, tvb, coords, freqs, (__nv_bfloat16*)o, lse, sp);
   prof_end(stream);
   if (launches) ++*launches;
   return cudaGetLastError();
