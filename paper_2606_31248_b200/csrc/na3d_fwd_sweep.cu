@@ -94,6 +94,7 @@ struct SweepCfg {
   static_assert(TL >= KL - 1, "tiles t and t+2 must reach disjoint planes");
   static_assert(HX <= 16 && NTOK <= 256, "halo of at most 256 keys per plane");
   static_assert(D + 2 * NMAX <= T_SLOT, "TMEM columns of a slot");
+  static_assert(RA % 2 == 0 && RB % 2 == 0, "key rows in pairs");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
@@ -875,10 +876,14 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
               for (int cc_ = 0; cc_ < C::HALF; ++cc_) v[cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[cc_], sv[cc_ + C::HALF]));
             };
+            // (the scale goes through an opaque register, so that the compiler cannot hoist this rarely needed
+            // computation out of its branches into the exponential pass)
             auto row_max = [&](const float (&v)[C::HALF]) {
+              float csm = cs;
+              asm volatile("mov.f32 %0, %0;" : "+f"(csm));
               float rmax = -INFINITY;
 #pragma unroll
-              for (int cc_ = 0; cc_ < C::HALF; ++cc_) rmax = fmaxf(rmax, C::FULLFOLD ? v[cc_] * cs : fmaf(v[cc_], cs, xz[cc_]));
+              for (int cc_ = 0; cc_ < C::HALF; ++cc_) rmax = fmaxf(rmax, C::FULLFOLD ? v[cc_] * csm : fmaf(v[cc_], csm, xz[cc_]));
               return rmax;
             };
             // ---- queries that see their first valid keys: their reference is the true maximum of this part
@@ -893,24 +898,35 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               }
               if (!inited && cmax > -INFINITY) { m_ref = cmax; inited = true; }
             }
-            // ---- the key rows of the part, one at a time: P row r overwrites S columns [PW r, PW r + PW), all of
-            // them read (rows <= r / 2) before
+            // ---- the key rows of the part, two at a time: the P rows (2j, 2j + 1) overwrite S columns
+            // [HX j, HX j + HX) = S row j, read before (or in this very step).  Away from the grid border a warp
+            // needs every row of a part or none (that is what the part boundaries are for); a row outside a
+            // query's window gives P = 0 through the -inf bias.
+            if (ra < rb) {
 #pragma unroll 1
-            for (int r = 0; r < nrows; ++r) {
-              uint32_t pw[C::PW];
-              if (r >= ra && r < rb) {
-                float v[C::HALF];
-                load_row(r, v);
+              for (int j = 0; j < nrows / 2; ++j) {
+                uint32_t sv[2 * C::HX];
+                tmem_ld_n<2 * C::HX>(s_tm + j * (2 * C::HX), sv);
+                float v[2][C::HALF];
+#pragma unroll
+                for (int q = 0; q < 2; ++q)
+#pragma unroll
+                  for (int cc_ = 0; cc_ < C::HALF; ++cc_)
+                    v[q][cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[q * C::HX + cc_], sv[q * C::HX + cc_ + C::HALF]));
+                const uint32_t bits2 = pbits >> (2 * j);
                 float rs;
-                float pr[C::HALF + 1];               // folded probabilities (times 2^-m_ref)
-                pr[C::HALF] = 0.f;
+                float pr[2][C::HALF + 1];            // folded probabilities (times 2^-m_ref)
+                pr[0][C::HALF] = 0.f; pr[1][C::HALF] = 0.f;
                 int attempt = 0;
 #pragma unroll 1
                 do {                                 // (rare block first: ONE copy of the exponentials in the code)
                   if (attempt > 0) {
                     // ---- a logit far above the reference: raise the reference by a whole number of octaves (every
                     // factor below is an exact power of two) and rescale what was accumulated so far
-                    float k = !(rs <= kBig) ? ceilf(row_max(v) - m_ref) : 0.f;
+                    float gm = -INFINITY;
+                    if (bits2 & 1u) gm = row_max(v[0]);
+                    if (bits2 & 2u) gm = fmaxf(gm, row_max(v[1]));
+                    float k = !(rs <= kBig) ? ceilf(gm - m_ref) : 0.f;
                     if (!(k > 0.f)) k = 0.f;
                     const float alpha = ex2(-k);
                     if (!first_item) {
@@ -918,45 +934,48 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                       mbar_wait(bar_pv0 + 8u * ((i - 1) & 1), (uint32_t)((i - 1) >> 1) & 1u);
                       tc_fence_after();
 #pragma unroll 1
-                      for (int j = 0; j < C::D; j += 16) {
+                      for (int jj = 0; jj < C::D; jj += 16) {
                         float ov[16];
-                        tmem_ld16(tm + C::T_O + j, ov);
+                        tmem_ld16(tm + C::T_O + jj, ov);
                         tmem_wait_ld();
                         uint32_t ow[16];
 #pragma unroll
                         for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
-                        tmem_st16(tm + C::T_O + j, ow);
+                        tmem_st16(tm + C::T_O + jj, ow);
                       }
                     }
                     // the P rows of this item stored so far
                     tmem_wait_st();
                     const uint32_t a2 = pack_bf16(alpha, alpha);
 #pragma unroll 1
-                    for (int j = ra * C::PW; j < r * C::PW; ++j) {
+                    for (int jj = 0; jj < j * 2 * C::PW; ++jj) {
                       uint32_t w;
-                      tmem_ld_x1(s_tm + j, &w);
+                      tmem_ld_x1(s_tm + jj, &w);
                       tmem_wait_ld();
                       w = bmul2(w, a2);
-                      tmem_st_x1(s_tm + j, &w);
+                      tmem_st_x1(s_tm + jj, &w);
                     }
                     tmem_wait_st();
                     lsum *= alpha;
                     m_ref += k;
                   }
-                  const float br = ((pbits >> r) & 1u) ? -m_ref : -INFINITY;
                   float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
 #pragma unroll
-                  for (int cc_ = 0; cc_ < C::HALF; cc_ += 2) {
-                    if (cc_ + 1 < C::HALF) {
-                      float t0, t1;
-                      if (C::FULLFOLD) ffma2(t0, t1, v[cc_], v[cc_ + 1], cs, br, br);
-                      else ffma2(t0, t1, v[cc_], v[cc_ + 1], cs, br + xz[cc_], br + xz[cc_ + 1]);
-                      pr[cc_] = ex2(t0); pr[cc_ + 1] = ex2(t1);
-                      if ((cc_ >> 1) & 1) fadd2(e2, e3, e2, e3, pr[cc_], pr[cc_ + 1]);
-                      else fadd2(e0, e1, e0, e1, pr[cc_], pr[cc_ + 1]);
-                    } else {
-                      pr[cc_] = ex2(fmaf(v[cc_], cs, C::FULLFOLD ? br : br + xz[cc_]));
-                      e0 += pr[cc_];
+                  for (int q = 0; q < 2; ++q) {
+                    const float br = ((bits2 >> q) & 1u) ? -m_ref : -INFINITY;
+#pragma unroll
+                    for (int cc_ = 0; cc_ < C::HALF; cc_ += 2) {
+                      if (cc_ + 1 < C::HALF) {
+                        float t0, t1;
+                        if (C::FULLFOLD) ffma2(t0, t1, v[q][cc_], v[q][cc_ + 1], cs, br, br);
+                        else ffma2(t0, t1, v[q][cc_], v[q][cc_ + 1], cs, br + xz[cc_], br + xz[cc_ + 1]);
+                        pr[q][cc_] = ex2(t0); pr[q][cc_ + 1] = ex2(t1);
+                        if (q) fadd2(e2, e3, e2, e3, pr[q][cc_], pr[q][cc_ + 1]);
+                        else fadd2(e0, e1, e0, e1, pr[q][cc_], pr[q][cc_ + 1]);
+                      } else {
+                        pr[q][cc_] = ex2(fmaf(v[q][cc_], cs, C::FULLFOLD ? br : br + xz[cc_]));
+                        if (q) e2 += pr[q][cc_]; else e0 += pr[q][cc_];
+                      }
                     }
                   }
                   rs = (e0 + e1) + (e2 + e3);
@@ -964,24 +983,32 @@ na3d_fwd_sweep_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                 } while (attempt < 2 && __any_sync(0xffffffffu, !(rs <= kBig)));
                 lsum += rs;
                 // pack folded pairs to bf16x2, un-fold with one byte permute per output word
-                uint32_t f[C::NF];
+                uint32_t pw[2 * C::PW];
 #pragma unroll
-                for (int m = 0; m < C::NF; ++m) f[m] = pack_bf16(pr[2 * m], pr[2 * m + 1]);
+                for (int q = 0; q < 2; ++q) {
+                  uint32_t f[C::NF];
 #pragma unroll
-                for (int j = 0; j < C::PW; ++j) pw[j] = prmt(f[((2 * j) % C::HALF) / 2], f[((2 * j + 1) % C::HALF) / 2], psel[j]);
-              } else {
+                  for (int m = 0; m < C::NF; ++m) f[m] = pack_bf16(pr[q][2 * m], pr[q][2 * m + 1]);
 #pragma unroll
-                for (int j = 0; j < C::PW; ++j) pw[j] = 0u;   // a key row no query of the warp attends
+                  for (int jj = 0; jj < C::PW; ++jj)
+                    pw[q * C::PW + jj] = prmt(f[((2 * jj) % C::HALF) / 2], f[((2 * jj + 1) % C::HALF) / 2], psel[jj]);
+                }
+                tmem_st_n<2 * C::PW>(s_tm + j * (2 * C::PW), pw);
               }
-              tmem_st_n<C::PW>(s_tm + r * C::PW, pw);
-            }
-            // pad keys of the part (stale rows of the K / V stage): P = 0
-            {
+              // pad keys of the part (stale rows of the K / V stage): P = 0
               uint32_t z[8];
 #pragma unroll
               for (int u = 0; u < 8; ++u) z[u] = 0u;
               if (part == 1) { if constexpr (C::NB / 2 > C::RB * C::PW) tmem_st_n<C::NB / 2 - C::RB * C::PW>(s_tm + C::RB * C::PW, z); }
               else { if constexpr (C::NA / 2 > C::RA * C::PW) tmem_st_n<C::NA / 2 - C::RA * C::PW>(s_tm + C::RA * C::PW, z); }
+            } else {
+              // no query of this warp attends a key of this part: P = 0
+              constexpr int NZ = (C::NA > C::NB ? C::NA : C::NB) / 2;
+              uint32_t z[NZ];
+#pragma unroll
+              for (int u = 0; u < NZ; ++u) z[u] = 0u;
+              if (part == 1) tmem_st_n<C::NB / 2>(s_tm, z);
+              else tmem_st_n<C::NA / 2>(s_tm, z);
             }
             tmem_wait_st();
             tc_fence_before();
