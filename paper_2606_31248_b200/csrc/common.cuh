@@ -71,6 +71,13 @@ bool sweep_fwd_supported(const Problem& p);
 cudaError_t launch_fwd_sweep2(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
                               const float* freqs, void* o, float* lse, cudaStream_t stream, int* launches);
 
+// na3d_fwd_plane.cu: tcgen05 forward (head_dim 64, k_L = 3), everything (A1-A6) in one kernel; whole key planes per
+// softmax hand-off, Q~ in TMEM.  `fix` is plane_fwd_workspace_bytes() of device scratch (rows for the fix-up kernel).
+bool plane_fwd_supported(const Problem& p);
+size_t plane_fwd_workspace_bytes();
+cudaError_t launch_fwd_plane(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
+                             const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches);
+
 // na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
 cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             void* o, float* lse, cudaStream_t stream, int* launches);
