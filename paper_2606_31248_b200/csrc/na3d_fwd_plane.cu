@@ -97,7 +97,7 @@ struct PlaneParams {
   int A;          // rotary axes (0: no rotation)
   int ncols;      // level columns = B * H * nty * ntx
   int hg;         // heads per work unit
-  unsigned long long* fix;   // [0] number of listed rows, [1 ...] the rows ((b * H + h) * N + token)
+  unsigned long long* fix;   // [0] number of listed rows, [1] != 0: every row, [2 ...] the rows ((b * H + h) * N + token)
   unsigned int fix_cap;
 };
 
@@ -149,14 +149,6 @@ template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setma
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ bool aux_sync_or(bool pred) {
-  uint32_t r;
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, %2, 128, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(r) : "r"((uint32_t)pred), "n"(kBarAux) : "memory");
-  return r != 0;
-}
-
 // ---- A2 in packed bf16x2 arithmetic.  Table words: C = (cos m, cos m+1), S = (sin m, sin m+1).
 __device__ __forceinline__ uint32_t bmul2(uint32_t a, uint32_t b) {
   uint32_t d;
@@ -175,7 +167,8 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 }
 // (a, b) -> (a cos - b sin, a sin + b cos) on two pairs at once: A = (a_m, a_m+1), B = (b_m, b_m+1).
 __device__ __forceinline__ void rot2(uint32_t& A, uint32_t& B, uint32_t C, uint32_t S) {
-  const uint32_t nB = B ^ 0x80008000u;
+  uint32_t nB;
+  asm("neg.bf16x2 %0, %1;" : "=r"(nB) : "r"(B));
   const uint32_t ra = bfma2(nB, S, bmul2(A, C));
   const uint32_t rb = bfma2(A, S, bmul2(B, C));
   A = ra; B = rb;
@@ -436,12 +429,12 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     // logical 16-byte chunk this thread owns in the plane-linear loops below
     const int cch = PAIR ? (tid & 3) : ((tid & 7) ^ ((tid >> 3) & 7));
 
-    int tab_level = 0;
-    bool invariant = true;
-
-    // coordinates of `level` of the halo of column c -> cache (this thread: halo tokens tid, tid + 128, row-major);
-    // true: they differ from the cache
-    auto load_coords = [&](const Col& c, int level) {
+    // A1, once per unit: coordinates of the halo of column c (this thread: halo tokens tid, tid + 128, row-major)
+    // -> (cos, sin) of every halo token and rotary pair -> table, in the layout of a K plane.  The coordinates of
+    // a column must not depend on the level (they are a function of the token's (lat, lon)); if
+    // they do, every row of the problem is handed to the fix-up kernel, which takes each token's own coordinates.
+    auto build_table = [&](const Col& c) {
+      bar_sync(kBarAux, 128);                       // everyone is done with the current table and cache
       bool diff = false;
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
@@ -449,23 +442,22 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
         if (tok >= C::NTOK) continue;
         const int hyr = tok / C::HX, hx = tok - hyr * C::HX;
         const int y = min(c.hs_y + hyr, p.Y - 1), x = min(c.hs_x + hx, p.X - 1);
-        const float* src = coords + ((((long long)c.b * p.L + level) * p.Y + y) * p.X + x) * p.A;
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        v.x = src[0];
-        if (p.A > 1) v.y = src[1];
-        if (p.A > 2) v.z = src[2];
-        const float4 old = cc[tok];
-        diff |= __float_as_uint(old.x) != __float_as_uint(v.x) || __float_as_uint(old.y) != __float_as_uint(v.y) ||
-                __float_as_uint(old.z) != __float_as_uint(v.z);
-        if (level == 0 || !invariant) cc[tok] = v;
+        const float* src = coords + ((((long long)c.b * p.L) * p.Y + y) * p.X + x) * p.A;
+        const long long lstride = (long long)p.Y * p.X * p.A;
+        float4 v = make_float4(src[0], p.A > 1 ? src[1] : 0.f, 0.f, 0.f);
+#pragma unroll 1
+        for (int l = 1; l < p.L; ++l) {
+          const float* sl = src + l * lstride;
+          diff |= __float_as_uint(sl[0]) != __float_as_uint(v.x);
+          if (p.A > 1) diff |= __float_as_uint(sl[1]) != __float_as_uint(v.y);
+        }
+        cc[tok] = v;
       }
-      return diff;
-    };
-    // A1: (cos, sin) of every halo token and rotary pair -> table, in the layout of a K plane
-    auto build_table = [&]() {
-      float fr[3][NPF];
+      if (diff) p.fix[1] = 1ull;                    // (any thread: the whole problem goes to the fix-up kernel)
+      bar_sync(kBarAux, 128);
+      float fr[2][NPF];
 #pragma unroll
-      for (int a = 0; a < 3; ++a)
+      for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int u = 0; u < NPF; ++u) fr[a][u] = (a < p.A) ? __ldg(freqs + a * (C::D / 2) + NPF * cch + u) : 0.f;
       if constexpr (PAIR == 0) {
@@ -474,12 +466,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
           const float4 xyz = cc[qi >> 3];
           float cs[4], sn[4];
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            float phi = xyz.x * fr[0][u];
-            phi = fmaf(xyz.y, fr[1][u], phi);
-            phi = fmaf(xyz.z, fr[2][u], phi);
-            sincos_reduced(phi, sn[u], cs[u]);
-          }
+          for (int u = 0; u < 4; ++u) sincos_reduced(fmaf(xyz.y, fr[1][u], xyz.x * fr[0][u]), sn[u], cs[u]);
           uint4 w;
           w.x = pack_bf16(cs[0], cs[1]); w.y = pack_bf16(sn[0], sn[1]);
           w.z = pack_bf16(cs[2], cs[3]); w.w = pack_bf16(sn[2], sn[3]);
@@ -492,12 +479,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
           const float4 xyz = cc[r];
           float cs[8], sn[8];
 #pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            float phi = xyz.x * fr[0][u];
-            phi = fmaf(xyz.y, fr[1][u], phi);
-            phi = fmaf(xyz.z, fr[2][u], phi);
-            sincos_reduced(phi, sn[u], cs[u]);
-          }
+          for (int u = 0; u < 8; ++u) sincos_reduced(fmaf(xyz.y, fr[1][u], xyz.x * fr[0][u]), sn[u], cs[u]);
           uint4 wc, ws;
           wc.x = pack_bf16(cs[0], cs[1]); wc.y = pack_bf16(cs[2], cs[3]); wc.z = pack_bf16(cs[4], cs[5]); wc.w = pack_bf16(cs[6], cs[7]);
           ws.x = pack_bf16(sn[0], sn[1]); ws.y = pack_bf16(sn[2], sn[3]); ws.z = pack_bf16(sn[4], sn[5]); ws.w = pack_bf16(sn[6], sn[7]);
@@ -506,35 +488,9 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
           sts128(rb + (((uint32_t)(cch + 4) ^ sw) << 4), ws);
         }
       }
-    };
-    // The table of `level` of the unit of column c must be in shared memory.  fresh: new unit (level 0 is loaded and
-    // the other levels are compared with it; a table that depends on the level is then rebuilt for `level`).
-    // ONE copy of the table code in the kernel.
-    auto ensure_table = [&](const Col& c, bool fresh, int level) {
-#pragma unroll 1
-      for (int pass = 0; pass < 2; ++pass) {
-        if (!fresh && (invariant || level == tab_level)) return;
-        bar_sync(kBarAux, 128);                       // everyone is done with the current table and cache
-        int lv = level;
-        if (fresh) {
-          invariant = true;
-          bool diff = false;
-#pragma unroll 1
-          for (int l = 0; l < p.L; ++l) diff |= load_coords(c, l) && l > 0;   // (levels > 0 are compared only: `invariant` is still set)
-          invariant = !aux_sync_or(diff);
-          lv = 0;
-        } else {
-          load_coords(c, lv);
-          bar_sync(kBarAux, 128);
-        }
-        build_table();
-        bar_sync(kBarAux, 128);
-        tab_level = lv;
-        fresh = false;
-      }
+      bar_sync(kBarAux, 128);
     };
 
-    // ---- the query row of a tile: global -> registers (the rows were prefetched into L2 a tile earlier)
     __nv_bfloat16 *ep_orow = nullptr, *pv_orow = nullptr;     // output row / LSE of the tile whose Q~ was stored last, of the one before
     float *ep_lrow = nullptr, *pv_lrow = nullptr;
     bool ep_active = false, pv_active = false;
@@ -543,26 +499,31 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       const long long tok = ((long long)lv * p.Y + y) * p.X + x;
       return q + (((long long)c.b * p.N + tok) * p.H + c.h) * C::D;
     };
-    // A2 for the query row in registers (the table of the row's level is in shared memory)
-    auto q_rotate = [&](const Col& c, uint4 (&qr)[8]) {
-      const int tr = (qy + c.y0 - c.hs_y) * C::HX + qx + c.x0 - c.hs_x;       // table row of the query's token
-      const uint32_t trb = t_smem + tr * 128, tsw = (uint32_t)(tr & 7);
-      if constexpr (PAIR == 0) {
+    // The query row of tile t (prefetched into L2 a tile earlier): global -> registers -> rotated (A2) -> TMEM (bf16
+    // pairs, K-major: the A operand of Q K^T).  T: running number of the tile.
+    auto q_task = [&](const Col& c, int t, int T) {
+      uint4 qr[8];
+      const uint4* src = reinterpret_cast<const uint4*>(q_row(c, t));
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const uint4 tb = lds128(trb + (((uint32_t)j ^ tsw) << 4));
-          rot_chunk(qr[j], tb);
-        }
-      } else {
+      for (int j = 0; j < 8; ++j) qr[j] = __ldg(src + j);
+      if (rope) {
+        const int tr = (qy + c.y0 - c.hs_y) * C::HX + qx + c.x0 - c.hs_x;       // table row of the query's token
+        const uint32_t trb = t_smem + tr * 128, tsw = (uint32_t)(tr & 7);
+        if constexpr (PAIR == 0) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint4 tc_ = lds128(trb + (((uint32_t)j ^ tsw) << 4)), ts_ = lds128(trb + (((uint32_t)(j + 4) ^ tsw) << 4));
-          rot_chunks_half(qr[j], qr[j + 4], tc_, ts_);
+          for (int j = 0; j < 8; ++j) {
+            const uint4 tb = lds128(trb + (((uint32_t)j ^ tsw) << 4));
+            rot_chunk(qr[j], tb);
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint4 tc_ = lds128(trb + (((uint32_t)j ^ tsw) << 4)), ts_ = lds128(trb + (((uint32_t)(j + 4) ^ tsw) << 4));
+            rot_chunks_half(qr[j], qr[j + 4], tc_, ts_);
+          }
         }
       }
-    };
-    // Q~ -> TMEM (bf16 pairs, K-major: the A operand of Q K^T); the output row of the tile for its epilogue
-    auto q_store = [&](const Col& c, int t, const uint4 (&qr)[8]) {
+      if (T > 0) { mbar_wait(bar_qfree, (uint32_t)(T - 1) & 1u); tc_fence_after(); }   // every Q K^T of the previous tile is done
       uint32_t w[32];
 #pragma unroll
       for (int j = 0; j < 8; ++j) { w[4 * j] = qr[j].x; w[4 * j + 1] = qr[j].y; w[4 * j + 2] = qr[j].z; w[4 * j + 3] = qr[j].w; }
@@ -578,7 +539,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       ep_orow = o + (((long long)c.b * p.N + tok) * p.H + c.h) * C::D;
       ep_lrow = lse + ((long long)c.b * p.H + c.h) * p.N + tok;
     };
-    // O / l -> bf16 -> global, LSE, of the tile with running number T
+    // O / l -> bf16 -> global, LSE, of the tile with running number T (its row: pv_*)
     auto epilogue = [&](int T) {
       mbar_wait(bar_pvdone, (uint32_t)T & 1u);
       tc_fence_after();
@@ -586,73 +547,83 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       const float lsum = (lds32(ls) + lds32(ls + 512)) + (lds32(ls + 1024) + lds32(ls + 1536));
       const float m_ref = lds32(mref_sm + (uint32_t)((T & 1) * 128 + row) * 4u);
       const float inv = 1.f / lsum;
-#pragma unroll 1
-      for (int j = 0; j < C::D; j += 16) {
-        float ov[16];
-        tmem_ld16(tm + C::T_O + j, ov);
-        tmem_wait_ld();
+#pragma unroll
+      for (int j = 0; j < C::D; j += 32) {
+        uint32_t ov[32];
+        tmem_ld_n<32>(tm + C::T_O + j, ov);
+        if (j + 32 >= C::D) { tc_fence_before(); warp_arrive(bar_ofree); }      // O is in registers: the next tile may overwrite it
         if (pv_active) {
-          uint4 w0, w1;
-          w0.x = pack_bf16(ov[0] * inv, ov[1] * inv);   w0.y = pack_bf16(ov[2] * inv, ov[3] * inv);
-          w0.z = pack_bf16(ov[4] * inv, ov[5] * inv);   w0.w = pack_bf16(ov[6] * inv, ov[7] * inv);
-          w1.x = pack_bf16(ov[8] * inv, ov[9] * inv);   w1.y = pack_bf16(ov[10] * inv, ov[11] * inv);
-          w1.z = pack_bf16(ov[12] * inv, ov[13] * inv); w1.w = pack_bf16(ov[14] * inv, ov[15] * inv);
-          reinterpret_cast<uint4*>(pv_orow + j)[0] = w0;
-          reinterpret_cast<uint4*>(pv_orow + j)[1] = w1;
+#pragma unroll
+          for (int u = 0; u < 32; u += 8) {
+            uint4 w0;
+            w0.x = pack_bf16(__uint_as_float(ov[u]) * inv, __uint_as_float(ov[u + 1]) * inv);
+            w0.y = pack_bf16(__uint_as_float(ov[u + 2]) * inv, __uint_as_float(ov[u + 3]) * inv);
+            w0.z = pack_bf16(__uint_as_float(ov[u + 4]) * inv, __uint_as_float(ov[u + 5]) * inv);
+            w0.w = pack_bf16(__uint_as_float(ov[u + 6]) * inv, __uint_as_float(ov[u + 7]) * inv);
+            reinterpret_cast<uint4*>(pv_orow + j + u)[0] = w0;
+          }
         }
       }
-      tc_fence_before();
-      warp_arrive(bar_ofree);
       if (pv_active) {
         *pv_lrow = (m_ref + log2f(lsum)) * 0.69314718055994531f;
         if (!(lsum < kRowSumLimit)) {                 // overflow (or NaN): the fix-up kernel recomputes the row
           const unsigned long long idx = atomicAdd(p.fix, 1ull);
-          if (idx < p.fix_cap) p.fix[1 + idx] = (unsigned long long)(pv_lrow - lse);
+          if (idx < p.fix_cap) p.fix[2 + idx] = (unsigned long long)(pv_lrow - lse);
         }
       }
     };
-    // K plane `plane` of column number cl: rotate in place, hand to the issuer
+    // K plane `plane` of column number cl: rotate in place (A2), hand to the issuer.  The table has the K plane's
+    // geometry, so the work is linear over physical 16-byte chunks: chunk tid + 128 j, all offsets immediates.
     auto rot_k = [&](int cl, int plane) {
       const int li = cl * p.L + plane, s = li % C::NS;
       mbar_wait(bar_kfull(s), (uint32_t)(li / C::NS) & 1u);
       if (rope) {
-        const uint32_t kb = k_smem + s * C::STAGE;
         if constexpr (PAIR == 0) {
-          // The table has the K plane's geometry, so the loop is linear over physical 16-byte chunks.
-          constexpr int nch = C::NTOK * 8;
-#pragma unroll 1
-          for (int q0 = tid; q0 < nch; q0 += 512) {
+          constexpr int nch = C::NTOK * 8, FULL = nch / 128, REM = nch % 128;
+          const uint32_t kb = k_smem + s * C::STAGE + tid * 16, tb = t_smem + tid * 16;
+#pragma unroll
+          for (int j0 = 0; j0 < FULL; j0 += 4) {
             uint4 x[4], t[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-              if (q0 + 128 * j < nch) { x[j] = lds128(kb + (q0 + 128 * j) * 16); t[j] = lds128(t_smem + (q0 + 128 * j) * 16); }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) rot_chunk(x[j], t[j]);
+              if (j0 + j < FULL) { x[j] = lds128(kb + (j0 + j) * 2048); t[j] = lds128(tb + (j0 + j) * 2048); }
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-              if (q0 + 128 * j < nch) sts128(kb + (q0 + 128 * j) * 16, x[j]);
+              if (j0 + j < FULL) { rot_chunk(x[j], t[j]); sts128(kb + (j0 + j) * 2048, x[j]); }
+          }
+          if (REM > 0 && tid < REM) {
+            uint4 x = lds128(kb + FULL * 2048);
+            const uint4 t = lds128(tb + FULL * 2048);
+            rot_chunk(x, t);
+            sts128(kb + FULL * 2048, x);
           }
         } else {
-          constexpr int nit = C::NTOK * 4;
-#pragma unroll 1
-          for (int q0 = tid; q0 < nit; q0 += 256) {
+          // item tid + 128 j: row (tid >> 2) + 32 j, logical chunks cch (channels a) and cch + 4 (channels b)
+          constexpr int nit = C::NTOK * 4, FULL = nit / 128, REM = nit % 128;
+          const uint32_t r0 = (uint32_t)(tid >> 2), sw = r0 & 7u;
+          const uint32_t oa = r0 * 128 + (((uint32_t)cch ^ sw) << 4), ob = r0 * 128 + (((uint32_t)(cch + 4) ^ sw) << 4);
+          const uint32_t kb = k_smem + s * C::STAGE;
+#pragma unroll
+          for (int j0 = 0; j0 < FULL; j0 += 2) {
             uint4 a[2], b[2], tc_[2], ts_[2];
-            uint32_t ao[2], bo[2];
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const int r = (q0 + 128 * j) >> 2;
-              const uint32_t sw = (uint32_t)(r & 7);
-              ao[j] = r * 128 + (((uint32_t)cch ^ sw) << 4); bo[j] = r * 128 + (((uint32_t)(cch + 4) ^ sw) << 4);
-              if (q0 + 128 * j < nit) {
-                a[j] = lds128(kb + ao[j]); b[j] = lds128(kb + bo[j]);
-                tc_[j] = lds128(t_smem + ao[j]); ts_[j] = lds128(t_smem + bo[j]);
-              }
-            }
-#pragma unroll
-            for (int j = 0; j < 2; ++j) rot_chunks_half(a[j], b[j], tc_[j], ts_[j]);
 #pragma unroll
             for (int j = 0; j < 2; ++j)
-              if (q0 + 128 * j < nit) { sts128(kb + ao[j], a[j]); sts128(kb + bo[j], b[j]); }
+              if (j0 + j < FULL) {
+                a[j] = lds128(kb + oa + (j0 + j) * 4096); b[j] = lds128(kb + ob + (j0 + j) * 4096);
+                tc_[j] = lds128(t_smem + oa + (j0 + j) * 4096); ts_[j] = lds128(t_smem + ob + (j0 + j) * 4096);
+              }
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+              if (j0 + j < FULL) {
+                rot_chunks_half(a[j], b[j], tc_[j], ts_[j]);
+                sts128(kb + oa + (j0 + j) * 4096, a[j]); sts128(kb + ob + (j0 + j) * 4096, b[j]);
+              }
+          }
+          if (REM > 0 && tid < REM) {
+            uint4 a = lds128(kb + oa + FULL * 4096), b = lds128(kb + ob + FULL * 4096);
+            const uint4 tc_ = lds128(t_smem + oa + FULL * 4096), ts_ = lds128(t_smem + ob + FULL * 4096);
+            rot_chunks_half(a, b, tc_, ts_);
+            sts128(kb + oa + FULL * 4096, a); sts128(kb + ob + FULL * 4096, b);
           }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -660,56 +631,39 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       warp_arrive(bar_krot(s));
     };
 
-    // ---- static task order.  Per tile T: the rows of Q (one level at a time), Q~ -> TMEM | the K
-    // planes new to the tile, with the epilogue of tile T - 1 before the last of them (the last new plane may need
-    // the ring slot that the first P V of tile T releases, and that MMA waits for the epilogue).  Every wait of this
-    // sequence depends only on tasks that precede it.  One call site per task kind (code size).
+    // ---- static task order.  Per tile T: Q~ -> TMEM | the K planes new to the tile, with the
+    // epilogue of tile T - 1 before the last of them (the last new plane may need the ring slot that the first P V
+    // of tile T releases, and that MMA waits for the epilogue).  Every wait of this sequence depends only on tasks
+    // that precede it.  One call site per task kind (code size).
     ColIter it;
     col_begin(it);
     bool more = col_advance(it);
     int t = 0, T = 0;
-    bool fresh = true;                         // the next table is the first of a unit
     for (;;) {
       const Col& c = it.c;
       int pa = 0, pb = 0;
-      if (more) { pa = t == 0 ? tile_plo<C>(0, p.L) : tile_phi<C>(t - 1, p.L); pb = tile_phi<C>(t, p.L); }
-      const int nrot = pb - pa;
-      const int epos = more ? C::TL + max(nrot - 1, 0) : 0;       // position of the epilogue in the task list
-      const int ntask = more ? C::TL + nrot + 1 : 1;
+      if (more) {
+        if (rope && t == 0 && it.hh == 0) build_table(c);
+        q_task(c, t, T);
+        // the query row of the next tile -> L2
+        const __nv_bfloat16* nq = nullptr;
+        if (t + 1 < ntl) nq = q_row(c, t + 1);
+        else if (it.hh + 1 < p.hg) { Col n = c; ++n.h; nq = q_row(n, 0); }
+        else if ((it.u + gridDim.x) * p.hg < p.ncols) nq = q_row(column((int)((it.u + gridDim.x) * p.hg)), 0);
+        if (nq) asm volatile("prefetch.global.L2 [%0];" ::"l"(nq));
+        pa = t == 0 ? tile_plo<C>(0, p.L) : tile_phi<C>(t - 1, p.L); pb = tile_phi<C>(t, p.L);
+      } else {
+        pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow;
+      }
+      const int nrot = pb - pa, epos = max(nrot - 1, 0);
 #pragma unroll 1
-      for (int i = 0; i < ntask; ++i) {
-        const int kind = i == epos ? 2 : i < C::TL ? 0 : 1;
-        const int arg = kind == 0 ? i : pa + (i - C::TL) - (i > epos ? 1 : 0);
-        if (rope && kind != 2) {
-          ensure_table(c, fresh, kind == 0 ? min(C::TL * t + arg, p.L - 1) : arg);
-          fresh = false;
-        }
-        if (kind == 0) {
-          if (arg == ql) {                                           // (a warp's rows are rows of one level)
-            uint4 qr[8];
-            const uint4* src = reinterpret_cast<const uint4*>(q_row(c, t));
-#pragma unroll
-            for (int j = 0; j < 8; ++j) qr[j] = __ldg(src + j);
-            if (rope) q_rotate(c, qr);
-            if (T > 0) { mbar_wait(bar_qfree, (uint32_t)(T - 1) & 1u); tc_fence_after(); }
-            q_store(c, t, qr);
-            // the query row of the next tile -> L2
-            const __nv_bfloat16* nq = nullptr;
-            if (t + 1 < ntl) nq = q_row(c, t + 1);
-            else if (it.hh + 1 < p.hg) { Col n = c; ++n.h; nq = q_row(n, 0); }
-            else if ((it.u + gridDim.x) * p.hg < p.ncols) nq = q_row(column((int)((it.u + gridDim.x) * p.hg)), 0);
-            if (nq) asm volatile("prefetch.global.L2 [%0];" ::"l"(nq));
-          }
-        } else if (kind == 1) {
-          rot_k(it.cl, arg);
-        } else if (T > 0) {
-          if (!more) { pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow; }
-          epilogue(T - 1);
-        }
+      for (int i = 0; i <= nrot; ++i) {
+        if (i == epos) { if (T > 0) epilogue(T - 1); }
+        else rot_k(it.cl, pa + i - (i > epos ? 1 : 0));
       }
       if (!more) break;
       ++T;
-      if (++t >= ntl) { t = 0; more = col_advance(it); fresh = more && it.hh == 0; }
+      if (++t >= ntl) { t = 0; more = col_advance(it); }
     }
   } else {
     // =========================== softmax ===========================
@@ -890,8 +844,8 @@ na3d_fix_rows_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
                      const float* __restrict__ freqs, __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                      const unsigned long long* __restrict__ fix, unsigned int cap, Problem p) {
   const unsigned long long listed = fix[0];
-  if (listed == 0) return;
-  const bool all = listed > cap;                                    // the list overflowed: every row
+  const bool all = listed > cap || fix[1] != 0;                     // the list overflowed / level-dependent coordinates: every row
+  if (listed == 0 && !all) return;
   const unsigned long long total = all ? (unsigned long long)p.rows() : listed;
   const int lane = threadIdx.x & 31;
   const unsigned long long w0 = (unsigned long long)blockIdx.x * 4 + (threadIdx.x >> 5), nw = (unsigned long long)gridDim.x * 4;
@@ -908,7 +862,7 @@ na3d_fix_rows_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
     ra = (float)(a_ * cs - b_ * sn); rb = (float)(a_ * sn + b_ * cs);
   };
   for (unsigned long long i = w0; i < total; i += nw) {
-    const unsigned long long rid = all ? i : fix[1 + i];          // (b * H + h) * N + token
+    const unsigned long long rid = all ? i : fix[2 + i];          // (b * H + h) * N + token
     const long long tok = (long long)(rid % (unsigned long long)p.N);
     const int h = (int)((rid / (unsigned long long)p.N) % (unsigned long long)p.H);
     const long long b = (long long)(rid / (unsigned long long)p.N / (unsigned long long)p.H);
@@ -1015,7 +969,7 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
     if (e != cudaSuccess) return e;
     ds->attr[ai] = true;
   }
-  cudaError_t e = cudaMemsetAsync(fix, 0, 8, stream);
+  cudaError_t e = cudaMemsetAsync(fix, 0, 16, stream);
   if (e != cudaSuccess) return e;
   prof_begin("na3d_fwd_plane", stream);
   kernel<<<(unsigned)grid, kPlaneThreads, C::SMEM_BYTES, stream>>>(tk, tv, (const __nv_bfloat16*)q, coords, freqs,
@@ -1041,10 +995,10 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   X(1, 5, 5, 4)                 \
   X(2, 3, 3, 4)
 
-size_t plane_fwd_workspace_bytes() { return 8 + 8 * (size_t)kFixCap; }
+size_t plane_fwd_workspace_bytes() { return 16 + 8 * (size_t)kFixCap; }
 
 bool plane_fwd_supported(const Problem& p) {
-  if (p.dtype != 1 || p.D != 64 || p.kL != 3) return false;
+  if (p.dtype != 1 || p.D != 64 || p.kL != 3 || p.A > 2) return false;   // (A = 3: the level is a rotary axis, no shared table)
 #define X(I_, KY_, KX_, NS_)                                  \
   if (p.kY == KY_ && p.kX == KX_) return plane_shape_ok<PlaneCfg<KY_, KX_, NS_>>(p);
   STRATA_PLANE_CONFIGS(X)
