@@ -43,8 +43,8 @@
 //          interleaved pairing the two halves of a pair are gathered into separate words and left in that order:
 //          the same permutation of the 8 channels of every 16-byte chunk is applied to Q and K, which leaves
 //          Q K^T unchanged.
-//   20     TMA producer of K / V planes (ring of NS stages); TMEM owner        21  MMA issuer, one elected lane
-//   22-23  idle (they complete the fourth warpgroup: setmaxnreg is a warpgroup instruction)
+//   20     TMA producer of K planes (ring of NSK stages); TMEM owner          21  MMA issuer, one elected lane
+//   22     TMA producer of V planes (ring of NSV stages)                      23  idle (completes the warpgroup)
 //
 // x fold: the x window of a query covers kX of the HX halo columns; with kX <= HX / 2 at most one of the columns c
 // and c + HX / 2 is inside it, so the two halves of every key row are FOLDED with a per-thread bit select before
@@ -59,7 +59,7 @@ namespace {
 
 using namespace tc;
 
-template <int KY_, int KX_, int NS_>
+template <int KY_, int KX_, int NSK_, int NSV_>
 struct PlaneCfg {
   static constexpr int D = 64, KL = 3, KY = KY_, KX = KX_;
   static constexpr int TL = 2, TY = 8, TX = 8, M = 128;
@@ -73,14 +73,14 @@ struct PlaneCfg {
   static constexpr int PW = HX / 2;                                  // packed P words per key row
   static constexpr int NF = (HALF + 1) / 2;                          // packed folded P words per key row
   static constexpr bool FULLFOLD = (KX == HALF);                     // exactly one of the columns c, c + HALF is in the window
-  static constexpr int NS = NS_;                                     // K / V ring stages
+  static constexpr int NSK = NSK_, NSV = NSV_;                       // K / V ring stages (a K plane is loaded and rotated well ahead)
   static constexpr int STAGE = N * 128;
   static constexpr int T_O = 0, T_S = D, T_Q = D + 2 * N, T_COLS = T_Q + D / 2;
   static constexpr int PADW = N / 2 - PW * HY;                       // P words behind the last key row
-  static constexpr int NBARS = 4 * NS + 8;
+  static constexpr int NBARS = 3 * NSK + 2 * NSV + 8;
   static constexpr int CC_BYTES = NTOK * 16;
   static constexpr int XCH_BYTES = (2 * 4 * 128 + 2 * 128 + 4 * 128) * 4;   // row sums, references, maxima
-  static constexpr int SMEM_BYTES = 1024 + 2 * NS * STAGE + STAGE + CC_BYTES + XCH_BYTES + 8 * NBARS + 16 + 512;
+  static constexpr int SMEM_BYTES = 1024 + (NSK + NSV) * STAGE + STAGE + CC_BYTES + XCH_BYTES + 8 * NBARS + 16 + 512;
   static_assert(KY % 2 == 1 && KX % 2 == 1 && KY >= 3, "odd windows only (HX, HY even)");
   static_assert(KX <= HALF, "the x fold needs kX <= HX / 2");
   static_assert(HX <= 16 && NTOK <= 256, "halo of at most 256 keys per plane");
@@ -102,7 +102,7 @@ struct PlaneParams {
 };
 
 constexpr int kPlaneThreads = 768;
-constexpr int kWarpAux = 16, kWarpTma = 20, kWarpMma = 21;
+constexpr int kWarpAux = 16, kWarpTma = 20, kWarpMma = 21, kWarpTmaV = 22;
 constexpr int kBarPair = 1;               // named barriers 1-8: the two warps of a (pair, subpartition), 64 threads
 constexpr int kBarRef = 9;                // 9-12: reference hand-off of a subpartition (64 arrive, 64 sync)
 constexpr int kBarAux = 13;               // the aux warpgroup, 128 threads
@@ -234,19 +234,20 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
-  const uint32_t k_smem = base;                                        // [NS] K planes
-  const uint32_t v_smem = k_smem + C::NS * C::STAGE;                   // [NS] V planes
-  const uint32_t t_smem = v_smem + C::NS * C::STAGE;                   // (cos, sin) table of the halo, in K-plane geometry
+  const uint32_t k_smem = base;                                        // [NSK] K planes
+  const uint32_t v_smem = k_smem + C::NSK * C::STAGE;                  // [NSV] V planes
+  const uint32_t t_smem = v_smem + C::NSV * C::STAGE;                   // (cos, sin) table of the halo, in K-plane geometry
   const uint32_t cc_smem = t_smem + C::STAGE;                          // coordinates of the halo tokens, float4 each
   const uint32_t lsum_sm = cc_smem + C::CC_BYTES;                      // [2 tile parities][4 warpgroups][128 rows] partial row sums
   const uint32_t mref_sm = lsum_sm + 2 * 4 * 128 * 4;                  // [2 tile parities][128 rows] references
   const uint32_t mx_sm = mref_sm + 2 * 128 * 4;                        // [2 pairs][2 halves][128 rows] maxima of a first plane
   const uint32_t bars = mx_sm + 4 * 128 * 4;
   auto bar_kfull = [&](int s) { return bars + 8u * s; };                          // TMA -> aux
-  auto bar_vfull = [&](int s) { return bars + 8u * (C::NS + s); };                // TMA -> issuer
-  auto bar_krot = [&](int s) { return bars + 8u * (2 * C::NS + s); };             // aux (4 warps) -> issuer
-  auto bar_kvempty = [&](int s) { return bars + 8u * (3 * C::NS + s); };          // issuer commit -> TMA
-  const uint32_t bar_sfull = bars + 8u * (4 * C::NS);                             // [2] issuer commit -> softmax pair
+  auto bar_krot = [&](int s) { return bars + 8u * (C::NSK + s); };                // aux (4 warps) -> issuer
+  auto bar_kempty = [&](int s) { return bars + 8u * (2 * C::NSK + s); };          // issuer commit (last Q K^T of the plane) -> TMA
+  auto bar_vfull = [&](int s) { return bars + 8u * (3 * C::NSK + s); };           // TMA -> issuer
+  auto bar_vempty = [&](int s) { return bars + 8u * (3 * C::NSK + C::NSV + s); }; // issuer commit (last P V of the plane) -> TMA
+  const uint32_t bar_sfull = bars + 8u * (3 * C::NSK + 2 * C::NSV);               // [2] issuer commit -> softmax pair
   const uint32_t bar_pfull = bar_sfull + 16;                                      // [2] 8 softmax warps -> issuer
   const uint32_t bar_qready = bar_pfull + 16;                                     // aux (4 warps) -> issuer: Q~ of the tile is in TMEM
   const uint32_t bar_qfree = bar_qready + 8;                                      // issuer commit -> aux: every Q K^T of the tile is done
@@ -299,9 +300,8 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   // ---- one-time setup
   if (warp == kWarpTma && lane == 0) {
     tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_v);
-    for (int s = 0; s < C::NS; ++s) {
-      mbar_init(bar_kfull(s), 1); mbar_init(bar_vfull(s), 1); mbar_init(bar_krot(s), 4); mbar_init(bar_kvempty(s), 1);
-    }
+    for (int s = 0; s < C::NSK; ++s) { mbar_init(bar_kfull(s), 1); mbar_init(bar_krot(s), 4); mbar_init(bar_kempty(s), 1); }
+    for (int s = 0; s < C::NSV; ++s) { mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 1); }
     mbar_init(bar_sfull, 1); mbar_init(bar_sfull + 8, 1);
     mbar_init(bar_pfull, 8); mbar_init(bar_pfull + 8, 8);
     mbar_init(bar_qready, 4); mbar_init(bar_qfree, 1); mbar_init(bar_pvdone, 1); mbar_init(bar_ofree, 4);
@@ -316,7 +316,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   }
   // K and V stages start as zeros: the rows behind the halo (N - NTOK) are keys outside every window (P = 0
   // there), which must hold finite numbers.
-  for (uint32_t off = threadIdx.x * 16u; off < 2u * C::NS * C::STAGE; off += kPlaneThreads * 16u)
+  for (uint32_t off = threadIdx.x * 16u; off < (uint32_t)(C::NSK + C::NSV) * C::STAGE; off += kPlaneThreads * 16u)
     asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(k_smem + off), "r"(0u) : "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   tc_fence_before();
@@ -325,21 +325,24 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   const uint32_t tmem = *tmem_word_ptr;
 
   if (warp >= kWarpTma) reg_dec<24>();
-  if (warp == kWarpTma) {
-    // =========================== TMA producer: K / V planes ===========================
+  if (warp == kWarpTma || warp == kWarpTmaV) {
+    // =========================== TMA producers: K planes (warp 20), V planes (warp 22) ===========================
+    const bool isv = warp == kWarpTmaV;
+    const int ns = isv ? C::NSV : C::NSK;
+    const uint32_t stage0 = isv ? v_smem : k_smem;
+    const CUtensorMap* map = isv ? &tm_v : &tm_k;
     ColIter it;
     col_begin(it);
     while (col_advance(it)) {
       const Col& c = it.c;
       for (int plane = 0; plane < p.L; ++plane) {
-        const int li = it.cl * p.L + plane, s = li % C::NS;
-        const uint32_t ph = (uint32_t)(li / C::NS) & 1u;
-        mbar_wait(bar_kvempty(s), ph ^ 1u);
+        const int li = it.cl * p.L + plane, s = li % ns;
+        const uint32_t ph = (uint32_t)(li / ns) & 1u;
+        const uint32_t full = isv ? bar_vfull(s) : bar_kfull(s);
+        mbar_wait(isv ? bar_vempty(s) : bar_kempty(s), ph ^ 1u);
         if (elect_one()) {
-          mbar_expect_tx(bar_kfull(s), (uint32_t)(C::NTOK * 128));
-          tma_load_5d(k_smem + s * C::STAGE, &tm_k, bar_kfull(s), 0, c.h, c.hs_x, c.hs_y, c.b * p.L + plane);
-          mbar_expect_tx(bar_vfull(s), (uint32_t)(C::NTOK * 128));
-          tma_load_5d(v_smem + s * C::STAGE, &tm_v, bar_vfull(s), 0, c.h, c.hs_x, c.hs_y, c.b * p.L + plane);
+          mbar_expect_tx(full, (uint32_t)(C::NTOK * 128));
+          tma_load_5d(stage0 + s * C::STAGE, map, full, 0, c.h, c.hs_x, c.hs_y, c.b * p.L + plane);
         }
         __syncwarp();
       }
@@ -366,9 +369,10 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     constexpr uint32_t idesc_pv = instr_desc(C::M, C::D, true);
 
     auto issue_qk = [&]() {
-      const int li = wq.cl * p.L + wq.plane, s = li % C::NS;
-      const uint32_t ph = (uint32_t)(li / C::NS) & 1u;
+      const int li = wq.cl * p.L + wq.plane, s = li % C::NSK;
+      const uint32_t ph = (uint32_t)(li / C::NSK) & 1u;
       const bool first = wq.plane == wq.plo, last = wq.plane == wq.phi - 1;
+      const bool release = (int)lastuse[wq.plane] == wq.t;
       if (first) mbar_wait<false>(bar_qready, (uint32_t)wq.tiles & 1u);          // Q~ of the tile is in TMEM
       mbar_wait<false>(bar_krot(s), ph);                                           // K plane rotated
       tc_fence_after();
@@ -379,6 +383,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
         for (int ks = 0; ks < C::D / 16; ++ks)
           umma_ts(d_tm, tmem + C::T_Q + 8u * ks, desc_from_lo(lo_k + 2u * ks), idesc_qk, ks > 0 ? 1u : 0u);
         umma_commit(bar_sfull + 8u * (iq & 1));
+        if (release) umma_commit(bar_kempty(s));
         if (last) umma_commit(bar_qfree);
       }
       __syncwarp();
@@ -386,8 +391,8 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       cur_next(wq);
     };
     auto issue_pv = [&]() {
-      const int li = wp.cl * p.L + wp.plane, s = li % C::NS;
-      const uint32_t ph = (uint32_t)(li / C::NS) & 1u;
+      const int li = wp.cl * p.L + wp.plane, s = li % C::NSV;
+      const uint32_t ph = (uint32_t)(li / C::NSV) & 1u;
       const bool first = wp.plane == wp.plo, last = wp.plane == wp.phi - 1;
       const bool release = (int)lastuse[wp.plane] == wp.t;
       mbar_wait<false>(bar_pfull + 8u * (ip & 1), (uint32_t)(ip >> 1) & 1u);      // P of the item is in TMEM
@@ -401,7 +406,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
 #pragma unroll
         for (int ks = 0; ks < C::N / 16; ++ks)
           umma_ts(tmem + C::T_O, a_tm + 8u * ks, desc_from_lo(lo_v + 128u * ks), idesc_pv, ks > 0 ? 1u : acc0);
-        if (release) umma_commit(bar_kvempty(s));
+        if (release) umma_commit(bar_vempty(s));
         if (last) umma_commit(bar_pvdone);
       }
       __syncwarp();
@@ -414,7 +419,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       issue_pv();
       if (wq.valid) issue_qk();
     }
-  } else if (warp > kWarpMma) {
+  } else if (warp > kWarpTmaV) {
     // (idle)
   } else if (warp >= kWarpAux) {
     // =========================== aux warpgroup ===========================
@@ -499,13 +504,15 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       const long long tok = ((long long)lv * p.Y + y) * p.X + x;
       return q + (((long long)c.b * p.N + tok) * p.H + c.h) * C::D;
     };
-    // The query row of tile t (prefetched into L2 a tile earlier): global -> registers -> rotated (A2) -> TMEM (bf16
-    // pairs, K-major: the A operand of Q K^T).  T: running number of the tile.
-    auto q_task = [&](const Col& c, int t, int T) {
-      uint4 qr[8];
+    // The query row of a tile: global -> registers (a tile ahead) -> rotated (A2) -> TMEM (bf16 pairs, K-major: the A
+    // operand of Q K^T).  T: running number of the tile.
+    uint4 qr[8];
+    auto q_fetch = [&](const Col& c, int t) {
       const uint4* src = reinterpret_cast<const uint4*>(q_row(c, t));
 #pragma unroll
       for (int j = 0; j < 8; ++j) qr[j] = __ldg(src + j);
+    };
+    auto q_task = [&](const Col& c, int t, int T) {
       if (rope) {
         const int tr = (qy + c.y0 - c.hs_y) * C::HX + qx + c.x0 - c.hs_x;       // table row of the query's token
         const uint32_t trb = t_smem + tr * 128, tsw = (uint32_t)(tr & 7);
@@ -575,8 +582,8 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     // K plane `plane` of column number cl: rotate in place (A2), hand to the issuer.  The table has the K plane's
     // geometry, so the work is linear over physical 16-byte chunks: chunk tid + 128 j, all offsets immediates.
     auto rot_k = [&](int cl, int plane) {
-      const int li = cl * p.L + plane, s = li % C::NS;
-      mbar_wait(bar_kfull(s), (uint32_t)(li / C::NS) & 1u);
+      const int li = cl * p.L + plane, s = li % C::NSK;
+      mbar_wait(bar_kfull(s), (uint32_t)(li / C::NSK) & 1u);
       if (rope) {
         if constexpr (PAIR == 0) {
           constexpr int nch = C::NTOK * 8, FULL = nch / 128, REM = nch % 128;
@@ -631,40 +638,42 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       warp_arrive(bar_krot(s));
     };
 
-    // ---- static task order.  Per tile T: Q~ -> TMEM | the K planes new to the tile, with the
-    // epilogue of tile T - 1 before the last of them (the last new plane may need the ring slot that the first P V
-    // of tile T releases, and that MMA waits for the epilogue).  Every wait of this sequence depends only on tasks
-    // that precede it.  One call site per task kind (code size).
+    // ---- static task order.  The K ring is one stage deeper than a tile needs, so the planes
+    // new to a tile are rotated a tile ahead.  Per tile T: Q~(T) -> TMEM (the row was fetched a tile ago; fetch the
+    // next) | the epilogue of tile T - 1 | the table of the next unit if one starts | the K planes new to tile T + 1.
+    // Every wait of this sequence depends only on tasks that precede it: the ring slot of plane p is released by
+    // the last Q K^T of plane p - NSK, which is one of the first two items of tile T (issued as soon as Q~(T) and
+    // its planes are there) or earlier.
     ColIter it;
     col_begin(it);
     bool more = col_advance(it);
     int t = 0, T = 0;
-    for (;;) {
-      const Col& c = it.c;
-      int pa = 0, pb = 0;
-      if (more) {
-        if (rope && t == 0 && it.hh == 0) build_table(c);
-        q_task(c, t, T);
-        // the query row of the next tile -> L2
-        const __nv_bfloat16* nq = nullptr;
-        if (t + 1 < ntl) nq = q_row(c, t + 1);
-        else if (it.hh + 1 < p.hg) { Col n = c; ++n.h; nq = q_row(n, 0); }
-        else if ((it.u + gridDim.x) * p.hg < p.ncols) nq = q_row(column((int)((it.u + gridDim.x) * p.hg)), 0);
-        if (nq) asm volatile("prefetch.global.L2 [%0];" ::"l"(nq));
-        pa = t == 0 ? tile_plo<C>(0, p.L) : tile_phi<C>(t - 1, p.L); pb = tile_phi<C>(t, p.L);
-      } else {
-        pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow;
-      }
-      const int nrot = pb - pa, epos = max(nrot - 1, 0);
+    if (more) {
+      q_fetch(it.c, 0);
+      if (rope) build_table(it.c);
 #pragma unroll 1
-      for (int i = 0; i <= nrot; ++i) {
-        if (i == epos) { if (T > 0) epilogue(T - 1); }
-        else rot_k(it.cl, pa + i - (i > epos ? 1 : 0));
-      }
-      if (!more) break;
-      ++T;
-      if (++t >= ntl) { t = 0; more = col_advance(it); }
+      for (int pl = 0; pl < tile_phi<C>(0, p.L); ++pl) rot_k(0, pl);
     }
+    while (more) {
+      const Col c = it.c;
+      const int cl = it.cl;
+      q_task(c, t, T);
+      // the tile after this one
+      const bool same_col = t + 1 < ntl;
+      bool have_next = same_col;
+      if (!same_col) { more = col_advance(it); have_next = more; }
+      if (have_next) q_fetch(same_col ? c : it.c, same_col ? t + 1 : 0);
+      if (T > 0) epilogue(T - 1);
+      if (have_next) {
+        if (rope && !same_col && it.hh == 0) build_table(it.c);
+        const int pa = same_col ? tile_phi<C>(t, p.L) : 0, pb = tile_phi<C>(same_col ? t + 1 : 0, p.L);
+#pragma unroll 1
+        for (int pl = pa; pl < pb; ++pl) rot_k(same_col ? cl : it.cl, pl);
+      }
+      ++T;
+      t = same_col ? t + 1 : 0;
+    }
+    if (T > 0) { pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow; epilogue(T - 1); }
   } else {
     // =========================== softmax ===========================
     reg_inc<88>();
@@ -989,18 +998,18 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
 
 }  // namespace
 
-// (index, kY, kX, NS) instantiations (head_dim 64, k_L = 3).
+// (index, kY, kX, K stages, V stages) instantiations (head_dim 64, k_L = 3).
 #define STRATA_PLANE_CONFIGS(X) \
-  X(0, 7, 7, 3)                 \
-  X(1, 5, 5, 4)                 \
-  X(2, 3, 3, 4)
+  X(0, 7, 7, 4, 3)              \
+  X(1, 5, 5, 4, 3)              \
+  X(2, 3, 3, 4, 3)
 
 size_t plane_fwd_workspace_bytes() { return 16 + 8 * (size_t)kFixCap; }
 
 bool plane_fwd_supported(const Problem& p) {
   if (p.dtype != 1 || p.D != 64 || p.kL != 3 || p.A > 2) return false;   // (A = 3: the level is a rotary axis, no shared table)
-#define X(I_, KY_, KX_, NS_)                                  \
-  if (p.kY == KY_ && p.kX == KX_) return plane_shape_ok<PlaneCfg<KY_, KX_, NS_>>(p);
+#define X(I_, KY_, KX_, NSK_, NSV_)                           \
+  if (p.kY == KY_ && p.kX == KX_) return plane_shape_ok<PlaneCfg<KY_, KX_, NSK_, NSV_>>(p);
   STRATA_PLANE_CONFIGS(X)
 #undef X
   return false;
@@ -1008,9 +1017,9 @@ bool plane_fwd_supported(const Problem& p) {
 
 cudaError_t launch_fwd_plane(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
                              const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches) {
-#define X(I_, KY_, KX_, NS_)                                  \
+#define X(I_, KY_, KX_, NSK_, NSV_)                           \
   if (p.kY == KY_ && p.kX == KX_)                             \
-    return launch_plane<PlaneCfg<KY_, KX_, NS_>>(p, I_, q, k, v, coords, freqs, o, lse, fix, stream, launches);
+    return launch_plane<PlaneCfg<KY_, KX_, NSK_, NSV_>>(p, I_, q, k, v, coords, freqs, o, lse, fix, stream, launches);
   STRATA_PLANE_CONFIGS(X)
 #undef X
   return cudaErrorNotSupported;
