@@ -27,11 +27,13 @@
 // scheduler hide each other's latencies, and a plane costs each warp one hand-off.
 // TMEM (512 columns): O [0, 64) | S0 | S1 (2 x 208) | Q~ [480, 512) (bf16, the A operand of Q K^T).
 //
-// The reference of a row (no running maximum, no rescaling): exp2(s - m) with m = the maximum over the FIRST plane
-// of the row's window.  Every plane uses the same m, so O and the row sum need no correction; the first plane
-// contributes a 1, so nothing underflows to an empty row.  What can go wrong is overflow: a later plane more
-// than ~2^100 above the first one.  The epilogue sees it in the row sum, puts the row on a list, and a small SIMT
-// kernel recomputes the listed rows with a true two-pass softmax after the main kernel (na3d_fix_rows_kernel).
+// No running maximum, no rescaling, no reference at all: P = exp2(s * scale * log2 e).  With the inputs this path is
+// built for (QK-RMSNorm: |logit| <= sqrt(d)) the exponentials sit in the middle of the fp32 / bf16
+// exponent range; every plane uses the same (zero) reference, so O and the row sum need no correction, and a
+// softmax warp needs nothing from the other warps that share its rows.  What can go wrong is a row whose
+// exponentials leave the range: the epilogue checks the row sum (2^-80 < l < 2^100, i.e. the row maximum roughly
+// within -55 .. +69), puts any other row on a list, and a small SIMT kernel recomputes the listed rows with a
+// true two-pass softmax after the main kernel (na3d_fix_rows_kernel).  The result is exact either way.
 //
 // Warps (768 threads; registers via setmaxnreg: softmax 88, aux 104, control 24):
 //   0-15   softmax (warp w: TMEM subpartition w & 3, pair w >> 3, half (w >> 2) & 1)
@@ -79,7 +81,7 @@ struct PlaneCfg {
   static constexpr int PADW = N / 2 - PW * HY;                       // P words behind the last key row
   static constexpr int NBARS = 3 * NSK + 2 * NSV + 8;
   static constexpr int CC_BYTES = NTOK * 16;
-  static constexpr int XCH_BYTES = (2 * 4 * 128 + 2 * 128 + 4 * 128) * 4;   // row sums, references, maxima
+  static constexpr int XCH_BYTES = 2 * 4 * 128 * 4;                  // partial row sums
   static constexpr int SMEM_BYTES = 1024 + (NSK + NSV) * STAGE + STAGE + CC_BYTES + XCH_BYTES + 8 * NBARS + 16 + 512;
   static_assert(KY % 2 == 1 && KX % 2 == 1 && KY >= 3, "odd windows only (HX, HY even)");
   static_assert(KX <= HALF, "the x fold needs kX <= HX / 2");
@@ -104,10 +106,9 @@ struct PlaneParams {
 constexpr int kPlaneThreads = 768;
 constexpr int kWarpAux = 16, kWarpTma = 20, kWarpMma = 21, kWarpTmaV = 22;
 constexpr int kBarPair = 1;               // named barriers 1-8: the two warps of a (pair, subpartition), 64 threads
-constexpr int kBarRef = 9;                // 9-12: reference hand-off of a subpartition (64 arrive, 64 sync)
 constexpr int kBarAux = 13;               // the aux warpgroup, 128 threads
 constexpr int kMaxLevels = 256;
-constexpr float kRowSumLimit = 1.2676506e30f;   // 2^100: row sums above this go to the fix-up kernel
+constexpr float kRowSumMax = 1.2676506e30f, kRowSumMin = 8.2718061e-25f;   // 2^100, 2^-80: row sums outside go to the fix-up kernel
 
 // ------------------------------------------------------------------------------------------------
 // small device helpers
@@ -148,7 +149,6 @@ __device__ __forceinline__ void warp_arrive(uint32_t bar) {
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 // ---- A2 in packed bf16x2 arithmetic.  Table words: C = (cos m, cos m+1), S = (sin m, sin m+1).
 __device__ __forceinline__ uint32_t bmul2(uint32_t a, uint32_t b) {
   uint32_t d;
@@ -228,7 +228,7 @@ __device__ __forceinline__ uint64_t desc_from_lo(uint32_t lo) { return ((uint64_
 template <class C, int PAIR>   // PAIR: strata_rope_pairing_t of the rotation
 __global__ void __launch_bounds__(kPlaneThreads, 1)
 na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
-                      const __nv_bfloat16* __restrict__ q, const float* __restrict__ coords,
+                      const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k, const float* __restrict__ coords,
                       const float* __restrict__ freqs, __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                       const PlaneParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -239,9 +239,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   const uint32_t t_smem = v_smem + C::NSV * C::STAGE;                   // (cos, sin) table of the halo, in K-plane geometry
   const uint32_t cc_smem = t_smem + C::STAGE;                          // coordinates of the halo tokens, float4 each
   const uint32_t lsum_sm = cc_smem + C::CC_BYTES;                      // [2 tile parities][4 warpgroups][128 rows] partial row sums
-  const uint32_t mref_sm = lsum_sm + 2 * 4 * 128 * 4;                  // [2 tile parities][128 rows] references
-  const uint32_t mx_sm = mref_sm + 2 * 128 * 4;                        // [2 pairs][2 halves][128 rows] maxima of a first plane
-  const uint32_t bars = mx_sm + 4 * 128 * 4;
+  const uint32_t bars = lsum_sm + 2 * 4 * 128 * 4;
   auto bar_kfull = [&](int s) { return bars + 8u * s; };                          // TMA -> aux
   auto bar_krot = [&](int s) { return bars + 8u * (C::NSK + s); };                // aux (4 warps) -> issuer
   auto bar_kempty = [&](int s) { return bars + 8u * (2 * C::NSK + s); };          // issuer commit (last Q K^T of the plane) -> TMA
@@ -251,8 +249,8 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
   const uint32_t bar_pfull = bar_sfull + 16;                                      // [2] 8 softmax warps -> issuer
   const uint32_t bar_qready = bar_pfull + 16;                                     // aux (4 warps) -> issuer: Q~ of the tile is in TMEM
   const uint32_t bar_qfree = bar_qready + 8;                                      // issuer commit -> aux: every Q K^T of the tile is done
-  const uint32_t bar_pvdone = bar_qfree + 8;                                      // issuer commit -> aux: O of the tile is complete
-  const uint32_t bar_ofree = bar_pvdone + 8;                                      // aux (4 warps) -> issuer: O has been read out
+  const uint32_t bar_pvdone = bar_qfree + 8;                                      // issuer commit -> softmax pair of the tile's last plane: O is complete
+  const uint32_t bar_ofree = bar_pvdone + 8;                                      // that pair (8 warps) -> issuer: O has been read out
   const uint32_t tmem_word = bars + 8u * C::NBARS;
   uint32_t* tmem_word_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_word - raw));
   uint8_t* lastuse = smem_raw + (tmem_word + 16 - raw);                // [L] last tile that needs the plane
@@ -304,7 +302,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     for (int s = 0; s < C::NSV; ++s) { mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 1); }
     mbar_init(bar_sfull, 1); mbar_init(bar_sfull + 8, 1);
     mbar_init(bar_pfull, 8); mbar_init(bar_pfull + 8, 8);
-    mbar_init(bar_qready, 4); mbar_init(bar_qfree, 1); mbar_init(bar_pvdone, 1); mbar_init(bar_ofree, 4);
+    mbar_init(bar_qready, 4); mbar_init(bar_qfree, 1); mbar_init(bar_pvdone, 1); mbar_init(bar_ofree, 8);
     fence_barrier_init();
   }
   if (warp == kWarpTma) tmem_alloc(tmem_word, 512);
@@ -496,9 +494,6 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       bar_sync(kBarAux, 128);
     };
 
-    __nv_bfloat16 *ep_orow = nullptr, *pv_orow = nullptr;     // output row / LSE of the tile whose Q~ was stored last, of the one before
-    float *ep_lrow = nullptr, *pv_lrow = nullptr;
-    bool ep_active = false, pv_active = false;
     auto q_row = [&](const Col& c, int t) {
       const int lv = min(C::TL * t + ql, p.L - 1), y = min(c.y0 + qy, p.Y - 1), x = min(c.x0 + qx, p.X - 1);
       const long long tok = ((long long)lv * p.Y + y) * p.X + x;
@@ -538,46 +533,6 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       tmem_wait_st();
       tc_fence_before();
       warp_arrive(bar_qready);
-      const int lvl = C::TL * t + ql;
-      const int al = min(lvl, p.L - 1), ay = min(c.y0 + qy, p.Y - 1), ax = min(c.x0 + qx, p.X - 1);
-      const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
-      pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow;
-      ep_active = lvl < p.L && c.y0 + qy < p.Y && c.x0 + qx < p.X;
-      ep_orow = o + (((long long)c.b * p.N + tok) * p.H + c.h) * C::D;
-      ep_lrow = lse + ((long long)c.b * p.H + c.h) * p.N + tok;
-    };
-    // O / l -> bf16 -> global, LSE, of the tile with running number T (its row: pv_*)
-    auto epilogue = [&](int T) {
-      mbar_wait(bar_pvdone, (uint32_t)T & 1u);
-      tc_fence_after();
-      const uint32_t ls = lsum_sm + (uint32_t)((T & 1) * 4 * 128 + row) * 4u;
-      const float lsum = (lds32(ls) + lds32(ls + 512)) + (lds32(ls + 1024) + lds32(ls + 1536));
-      const float m_ref = lds32(mref_sm + (uint32_t)((T & 1) * 128 + row) * 4u);
-      const float inv = 1.f / lsum;
-#pragma unroll
-      for (int j = 0; j < C::D; j += 32) {
-        uint32_t ov[32];
-        tmem_ld_n<32>(tm + C::T_O + j, ov);
-        if (j + 32 >= C::D) { tc_fence_before(); warp_arrive(bar_ofree); }      // O is in registers: the next tile may overwrite it
-        if (pv_active) {
-#pragma unroll
-          for (int u = 0; u < 32; u += 8) {
-            uint4 w0;
-            w0.x = pack_bf16(__uint_as_float(ov[u]) * inv, __uint_as_float(ov[u + 1]) * inv);
-            w0.y = pack_bf16(__uint_as_float(ov[u + 2]) * inv, __uint_as_float(ov[u + 3]) * inv);
-            w0.z = pack_bf16(__uint_as_float(ov[u + 4]) * inv, __uint_as_float(ov[u + 5]) * inv);
-            w0.w = pack_bf16(__uint_as_float(ov[u + 6]) * inv, __uint_as_float(ov[u + 7]) * inv);
-            reinterpret_cast<uint4*>(pv_orow + j + u)[0] = w0;
-          }
-        }
-      }
-      if (pv_active) {
-        *pv_lrow = (m_ref + log2f(lsum)) * 0.69314718055994531f;
-        if (!(lsum < kRowSumLimit)) {                 // overflow (or NaN): the fix-up kernel recomputes the row
-          const unsigned long long idx = atomicAdd(p.fix, 1ull);
-          if (idx < p.fix_cap) p.fix[2 + idx] = (unsigned long long)(pv_lrow - lse);
-        }
-      }
     };
     // K plane `plane` of column number cl: rotate in place (A2), hand to the issuer.  The table has the K plane's
     // geometry, so the work is linear over physical 16-byte chunks: chunk tid + 128 j, all offsets immediates.
@@ -640,7 +595,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
 
     // ---- static task order.  The K ring is one stage deeper than a tile needs, so the planes
     // new to a tile are rotated a tile ahead.  Per tile T: Q~(T) -> TMEM (the row was fetched a tile ago; fetch the
-    // next) | the epilogue of tile T - 1 | the table of the next unit if one starts | the K planes new to tile T + 1.
+    // next, its reference) | the table of the next unit if one starts | the K planes new to tile T + 1.
     // Every wait of this sequence depends only on tasks that precede it: the ring slot of plane p is released by
     // the last Q K^T of plane p - NSK, which is one of the first two items of tile T (issued as soon as Q~(T) and
     // its planes are there) or earlier.
@@ -662,9 +617,8 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       const bool same_col = t + 1 < ntl;
       bool have_next = same_col;
       if (!same_col) { more = col_advance(it); have_next = more; }
-      if (have_next) q_fetch(same_col ? c : it.c, same_col ? t + 1 : 0);
-      if (T > 0) epilogue(T - 1);
       if (have_next) {
+        q_fetch(same_col ? c : it.c, same_col ? t + 1 : 0);
         if (rope && !same_col && it.hh == 0) build_table(it.c);
         const int pa = same_col ? tile_phi<C>(t, p.L) : 0, pb = tile_phi<C>(same_col ? t + 1 : 0, p.L);
 #pragma unroll 1
@@ -673,7 +627,6 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
       ++T;
       t = same_col ? t + 1 : 0;
     }
-    if (T > 0) { pv_active = ep_active; pv_orow = ep_orow; pv_lrow = ep_lrow; epilogue(T - 1); }
   } else {
     // =========================== softmax ===========================
     reg_inc<88>();
@@ -684,14 +637,18 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     const uint32_t s_tm = pinned(tmem + ((uint32_t)(sp * 32) << 16) + C::T_S + pair * C::N);   // S of this pair's items; P goes over its front
     const float cs = p.scale_log2e;
     const uint32_t bar_s = pinned(bar_sfull + 8u * pair), bar_p = pinned(bar_pfull + 8u * pair);
-    const int bar_pr = kBarPair + pair * 4 + sp, bar_rf = kBarRef + sp;
-    const uint32_t mx_mine = mx_sm + (uint32_t)((pair * 2 + half) * 128 + row) * 4u;
-    const uint32_t mx_other = mx_sm + (uint32_t)((pair * 2 + (half ^ 1)) * 128 + row) * 4u;
+    const uint32_t bar_pr = pinned((uint32_t)(kBarPair + pair * 4 + sp));
+    const uint32_t lane0 = pinned(lane == 0 ? 1u : 0u);
+    const uint32_t ls_base = pinned(lsum_sm + (uint32_t)(wg * 128 + row) * 4u);
+    const uint32_t ls_row = pinned(lsum_sm + (uint32_t)row * 4u);
+    const uint32_t o_tm = pinned(tmem + ((uint32_t)(sp * 32) << 16) + C::T_O + half * (C::D / 2));   // this warp's half of the O row
+    int ax = 0, ay = 0;                             // this query's token (clamped to the grid)
+    bool active_xy = false;
 
     // per-unit constants of this query row (the columns of a unit share the tile, hence the windows)
     int rw = 0;                                     // first key row of this warp
     int r0 = 0;                                     // first key row the subpartition needs
-    uint32_t rowbits = 0;                           // halo rows inside this query's window
+    uint32_t rowbits = 0;                           // halo rows inside this query's window, from row rw
     uint32_t m_lo[C::HALF];                         // x fold: all ones: column c is in the window (else c + HALF, or neither)
     float xz[C::HALF];                              // 0 if one of the two is in the window, else -inf
     uint32_t psel[C::PW];                           // un-fold selectors, see below
@@ -701,12 +658,13 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
     while (col_advance(it)) {
       const Col& c = it.c;
       if (it.hh == 0) {
-        const int ax = min(c.x0 + qx, p.X - 1), ay = min(c.y0 + qy, p.Y - 1);
+        ax = min(c.x0 + qx, p.X - 1); ay = min(c.y0 + qy, p.Y - 1);
+        active_xy = c.x0 + qx < p.X && c.y0 + qy < p.Y;
         const int lo_x = window_start(ax, C::KX, p.X) - c.hs_x;
         const int lo_y = window_start(ay, C::KY, p.Y) - c.hs_y;
         r0 = min(__reduce_min_sync(0xffffffffu, lo_y), C::R0MAX);
         rw = r0 + half * C::NR;
-        rowbits = ((1u << C::KY) - 1u) << lo_y;
+        rowbits = (((1u << C::KY) - 1u) << lo_y) >> rw;
 #pragma unroll
         for (int cc_ = 0; cc_ < C::HALF; ++cc_) {
           const bool in_lo = cc_ >= lo_x && cc_ < lo_x + C::KX, in_hi = cc_ + C::HALF >= lo_x && cc_ + C::HALF < lo_x + C::KX;
@@ -732,10 +690,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
         const int al = min(C::TL * tile + ql, p.L - 1);
         const int pw_lo = window_start(al, C::KL, p.L);              // planes of this query (warp-uniform): [pw_lo, pw_lo + KL)
         const int plo = tile_plo<C>(tile, p.L), phi = tile_phi<C>(tile, p.L);
-        float m_ref = 0.f, lsum = 0.f;
-        bool have_ref = false;
-        const uint32_t ls_addr = lsum_sm + (uint32_t)(((T & 1) * 4 + wg) * 128 + row) * 4u;
-        const uint32_t mr_addr = mref_sm + (uint32_t)((T & 1) * 128 + row) * 4u;
+        float lsum = 0.f;
 #pragma unroll 1
         for (int plane = plo; plane < phi; ++plane, ++g) {
           if ((g & 1) != pair) continue;
@@ -750,42 +705,31 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
             for (int u = 0; u < NZ; ++u) z[u] = 0u;
             tmem_st_n<NZ>(s_tm + half * NZ, z);
           } else {
-            // ---- this warp's key rows of S -> registers, folded
+            // ---- this warp's key rows of S -> registers, folded; two rows per TMEM load
             float v[C::NR][C::HALF];
+            {
+              const uint32_t s_row = s_tm + rw * C::HX;
 #pragma unroll
-            for (int r = 0; r < C::NR; ++r) {
-              uint32_t sv[C::HX];
-              tmem_ld_n<C::HX>(s_tm + (rw + r) * C::HX, sv);
+              for (int r = 0; r < C::NR; r += 2) {
+                uint32_t sv[32];
+                if (r + 1 < C::NR) { tmem_ld_x32(s_row + r * C::HX, sv); tmem_wait_ld(); reg_fence_16(sv); reg_fence_16(sv + 16); }
+                else { tmem_ld_x16(s_row + r * C::HX, sv); tmem_wait_ld(); reg_fence_16(sv); }   // (columns behind the row: the next row or pad)
 #pragma unroll
-              for (int cc_ = 0; cc_ < C::HALF; ++cc_) v[r][cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[cc_], sv[cc_ + C::HALF]));
-            }
-            const uint32_t bits = rowbits >> rw;                     // bit r: key row rw + r is in this query's window
-            if (plane == pw_lo) {
-              // ---- first plane of these queries: the reference is its maximum (both warps of the subpartition)
-              float mx = -INFINITY;
+                for (int q2 = 0; q2 < 2; ++q2)
+                  if (r + q2 < C::NR) {
 #pragma unroll
-              for (int r = 0; r < C::NR; ++r) {
-                float rm = -INFINITY;
-#pragma unroll
-                for (int cc_ = 0; cc_ < C::HALF; ++cc_) rm = fmaxf(rm, C::FULLFOLD ? v[r][cc_] * cs : fmaf(v[r][cc_], cs, xz[cc_]));
-                if ((bits >> r) & 1u) mx = fmaxf(mx, rm);
+                    for (int cc_ = 0; cc_ < C::HALF; ++cc_)
+                      v[r + q2][cc_] = __uint_as_float(bitsel(m_lo[cc_], sv[q2 * C::HX + cc_], sv[q2 * C::HX + cc_ + C::HALF]));
+                  }
               }
-              sts32(mx_mine, mx);
-              bar_sync(bar_pr, 64);                                  // (also: every S row of the subpartition is in registers)
-              m_ref = fmaxf(mx, lds32(mx_other));
-              if (half == 0) sts32(mr_addr, m_ref);
-              bar_arrive(bar_rf, 128);                               // the other pair takes the reference from mr_addr
-            } else {
-              if (!have_ref) { bar_sync(bar_rf, 128); m_ref = lds32(mr_addr); }
-              bar_sync(bar_pr, 64);                                  // every S row of the subpartition is in registers
             }
-            have_ref = true;
+            bar_sync(bar_pr, 64);                                    // every S row of the subpartition is in registers: P may go over S
             // ---- exponentials, row sums, P (bf16, un-folded) over the S rows
             uint32_t pw[C::NR * C::PW];
             float e0 = 0.f, e1 = 0.f;
 #pragma unroll
             for (int r = 0; r < C::NR; ++r) {
-              const float br = ((bits >> r) & 1u) ? -m_ref : -INFINITY;
+              const float br = ((rowbits >> r) & 1u) ? 0.f : -INFINITY;
               float pr[C::HALF + 1];
               pr[C::HALF] = 0.f;
 #pragma unroll
@@ -810,25 +754,70 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
             }
             lsum += e0 + e1;
             tmem_st_n<C::NR * C::PW>(s_tm + rw * C::PW, pw);
-            // ---- key rows no query of the subpartition attends, pad keys: P = 0
-            uint32_t z[C::PW > C::PADW ? C::PW : C::PADW];
+            // ---- key rows no query of the subpartition attends, pad keys: P = 0.  Away from the grid border the
+            // needed rows are the first or the last NEED rows of the halo.
+            constexpr int ZW = C::R0MAX * C::PW + C::PADW;
+            uint32_t z[ZW];
 #pragma unroll
-            for (int u = 0; u < (C::PW > C::PADW ? C::PW : C::PADW); ++u) z[u] = 0u;
+            for (int u = 0; u < ZW; ++u) z[u] = 0u;
             if (half == 0) {
+              if (r0 == C::R0MAX) tmem_st_n<C::R0MAX * C::PW>(s_tm, z);
+              else {
 #pragma unroll
-              for (int k = 0; k < C::R0MAX; ++k)
-                if (k < r0) tmem_st_n<C::PW>(s_tm + k * C::PW, z);
+                for (int kk = 0; kk < C::R0MAX; ++kk)
+                  if (kk < r0) tmem_st_n<C::PW>(s_tm + kk * C::PW, z);
+              }
             } else {
+              if (r0 == 0) tmem_st_n<ZW>(s_tm + C::NEED * C::PW, z);
+              else {
 #pragma unroll
-              for (int k = 0; k < C::R0MAX; ++k)
-                if (r0 + C::NEED + k < C::HY) tmem_st_n<C::PW>(s_tm + (r0 + C::NEED + k) * C::PW, z);
-              if constexpr (C::PADW > 0) tmem_st_n<C::PADW>(s_tm + C::HY * C::PW, z);
+                for (int kk = 0; kk < C::R0MAX; ++kk)
+                  if (r0 + C::NEED + kk < C::HY) tmem_st_n<C::PW>(s_tm + (r0 + C::NEED + kk) * C::PW, z);
+                if constexpr (C::PADW > 0) tmem_st_n<C::PADW>(s_tm + C::HY * C::PW, z);
+              }
             }
-            sts32(ls_addr, lsum);
+            sts32(ls_base + (uint32_t)(T & 1) * 2048u, lsum);
           }
           tmem_wait_st();
           tc_fence_before();
-          warp_arrive(bar_p);
+          __syncwarp();
+          if (lane0) mbar_arrive(bar_p);
+          if (plane == phi - 1) {
+            // ---- this pair handled the last plane of the tile: its epilogue (O / l -> bf16 -> global, LSE), in the
+            // shadow of the P V and Q K^T the pair waits for anyway.  Each of the two warps of a subpartition takes
+            // half of the O row.
+            mbar_wait(bar_pvdone, (uint32_t)T & 1u);
+            tc_fence_after();
+            const uint32_t la = ls_row + (uint32_t)(T & 1) * 2048u;      // (read before O is released: tile T + 2 reuses the slots)
+            const float ltot = (lds32(la) + lds32(la + 512)) + (lds32(la + 1024) + lds32(la + 1536));
+            uint32_t ov[C::D / 2];
+            tmem_ld_n<C::D / 2>(o_tm, ov);
+            tc_fence_before();
+            __syncwarp();
+            if (lane0) mbar_arrive(bar_ofree);                       // O is in registers: the next tile may overwrite it
+            if (active_xy && C::TL * tile + ql < p.L) {
+              const float inv = 1.f / ltot;
+              const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
+              __nv_bfloat16* orow = o + (((long long)c.b * p.N + tok) * p.H + c.h) * C::D + half * (C::D / 2);
+#pragma unroll
+              for (int u = 0; u < C::D / 2; u += 8) {
+                uint4 w0;
+                w0.x = pack_bf16(__uint_as_float(ov[u]) * inv, __uint_as_float(ov[u + 1]) * inv);
+                w0.y = pack_bf16(__uint_as_float(ov[u + 2]) * inv, __uint_as_float(ov[u + 3]) * inv);
+                w0.z = pack_bf16(__uint_as_float(ov[u + 4]) * inv, __uint_as_float(ov[u + 5]) * inv);
+                w0.w = pack_bf16(__uint_as_float(ov[u + 6]) * inv, __uint_as_float(ov[u + 7]) * inv);
+                reinterpret_cast<uint4*>(orow + u)[0] = w0;
+              }
+              if (half == 0) {
+                const long long rid = ((long long)c.b * p.H + c.h) * p.N + tok;
+                lse[rid] = log2f(ltot) * 0.69314718055994531f;
+                if (!(ltot < kRowSumMax && ltot > kRowSumMin)) {   // out of the safe range (or NaN): the fix-up kernel recomputes the row
+                  const unsigned long long idx = atomicAdd(p.fix, 1ull);
+                  if (idx < p.fix_cap) p.fix[2 + idx] = (unsigned long long)rid;
+                }
+              }
+            }
+          }
         }
       }
     }
@@ -981,7 +970,7 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   cudaError_t e = cudaMemsetAsync(fix, 0, 16, stream);
   if (e != cudaSuccess) return e;
   prof_begin("na3d_fwd_plane", stream);
-  kernel<<<(unsigned)grid, kPlaneThreads, C::SMEM_BYTES, stream>>>(tk, tv, (const __nv_bfloat16*)q, coords, freqs,
+  kernel<<<(unsigned)grid, kPlaneThreads, C::SMEM_BYTES, stream>>>(tk, tv, (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, coords, freqs,
                                                                   (__nv_bfloat16*)o, lse, sp);
   prof_end(stream);
   if (launches) ++*launches;
