@@ -98,16 +98,18 @@ class ClockSampler:
 
 
 def measured_traffic(workload: str, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu captures
-    (profiles/*traffic.csv: workload,kernel,dram_bytes_per_launch,capture); None if never captured."""
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `workload`, from the committed ncu
+    captures (profiles/*traffic.csv: workload,kernel,dram_bytes_per_launch,capture,commit), newest file first.
+    Returns (bytes, "capture @ commit") or (None, None) if that kernel was never captured: the number is a
+    property of the capture named beside it, not of this run."""
     import csv
     import glob
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*traffic.csv")), reverse=True):
         with open(path) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == workload and row["kernel"] == kernel:
-                    return float(row["dram_bytes_per_launch"])
-    return None
+                    return float(row["dram_bytes_per_launch"]), f"{row.get('capture', '?')} @ {row.get('commit', '?')}"
+    return None, None
 
 
 def flops_of(w: wl.Workload) -> float:
@@ -322,8 +324,9 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
     t_hbm = bytes_ / (peaks["hbm_gbs"] * 1e9)
     t_tc = flops / (peaks["bf16_tflops"] * 1e12)
     achieved = bytes_ / (dom_ms * 1e-3) / 1e9
+    traffic, traffic_capture = measured_traffic(w.name, dom)
     roofline = {"bound": "hbm", "kernel": dom, "kernel_ms": dom_ms, "achieved": achieved, "peak": peaks["hbm_gbs"],
-                "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": measured_traffic(w.name, dom),
+                "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_capture": traffic_capture,
                 "peak_source": peaks["source"], "algorithmic_bytes": bytes_,
                 "roofline_ms": max(t_hbm, t_tc) * 1e3, "step_frac_of_roofline": max(t_hbm, t_tc) * 1e3 / ms,
                 "kernels_ms": per_kernel}

@@ -1,4 +1,4 @@
-// bwd_common.cuh -- pieces shared by the tensor-core backward kernels (na3d_bwd_tc.cu, na3d_bwd_tc2.cu);
+// bwd_common.cuh -- pieces of the tensor-core backward kernels (na3d_bwd_tc2.cu);
 // include after tc_common.cuh.
 #pragma once
 
@@ -13,16 +13,7 @@ struct BwdParams {
   long long N;
   float scale, scale_log2e;
   int pairing;   // strata_rope_pairing_t of the fused un-rotation
-#ifdef STRATA_TRACE
-  unsigned long long* trace;   // debug: clock64 stamps of one CTA, [event][chunk]
-  int trace_cta;
-#endif
 };
-#ifdef STRATA_TRACE
-#define BTRACE(ev, idx) do { if (p.trace && (int)blockIdx.x == p.trace_cta && (idx) < 64) p.trace[(ev) * 64 + (idx)] = clock64(); } while (0)
-#else
-#define BTRACE(ev, idx) do {} while (0)
-#endif
 
 
 // packed fp32 pairs (one instruction for two columns)

@@ -15,7 +15,7 @@ struct Problem {
   int A;        // rotary axes (0 = no RoPE)
   int pairing;  // 0: (2j, 2j+1)   1: (j, j + D/2)
   int dtype;    // 0 f32, 1 bf16
-  int force_tile;  // tcgen05: use the one-tile-per-CTA kernel even where the level-sweep kernel applies
+  int force_tile;  // tcgen05: use the one-tile-per-CTA kernel on pre-rotated operands even where the fused forward applies
   float scale;  // resolved softmax scale (> 0)
   long long N;  // L * Y * X
   __host__ __device__ long long rows() const { return (long long)B * N * H; }    // (b, token, h) rows
@@ -52,24 +52,9 @@ cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1,
                                void* y0, void* y1, int out_dtype, const float* coords,
                                const float* freqs, float sign, cudaStream_t stream, int* launches);
 
-// rope.cu: A1 as a table, [B, L, Y, X, D/2] half2 (cos, sin), for the fused tensor-core kernels.
-cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
-                              cudaStream_t stream, int* launches);
-
 // rope.cu: A1 as an fp32 table [B, L, Y, X, D/2] float2 (cos, sin), for the backward epilogues (B4).
 cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* coords, const float* freqs,
                                   cudaStream_t stream, int* launches);
-
-// na3d_fwd_fused.cu: tcgen05 forward with the rotation of Q and K fused in (un-rotated bf16 operands).
-bool fused_fwd_supported(const Problem& p);
-cudaError_t launch_fwd_fused(const Problem& p, const void* q, const void* k, const void* v, const void* table,
-                             void* o, float* lse, cudaStream_t stream, int* launches);
-
-// na3d_fwd_sweep.cu: tcgen05 forward, everything (A1-A6) in one kernel: un-rotated bf16 operands, coordinates and
-// frequencies in, O and LSE out; no workspace.
-bool sweep_fwd_supported(const Problem& p);
-cudaError_t launch_fwd_sweep2(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
-                              const float* freqs, void* o, float* lse, cudaStream_t stream, int* launches);
 
 // na3d_fwd_plane.cu: tcgen05 forward (head_dim 64, k_L = 3), everything (A1-A6) in one kernel; whole key planes per
 // softmax hand-off, Q~ in TMEM.  `fix` is plane_fwd_workspace_bytes() of device scratch (rows for the fix-up kernel).
@@ -91,11 +76,6 @@ bool tc_bwd_supported(const Problem& p);
 cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
                           const void* d_o, const float* lse, void* stat, const void* rtab, void* dq, void* dk,
                           void* dv, cudaStream_t stream, int* launches);
-
-// na3d_tc_fwd_sweep.cu: tcgen05 forward, one CTA per level column (head_dim 64, k_L = 3).
-bool tc_sweep_supported(const Problem& p);
-cudaError_t launch_fwd_sweep(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
-                             float* lse, cudaStream_t stream, int* launches);
 
 // na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands.
 bool tc_fwd_supported(const Problem& p);

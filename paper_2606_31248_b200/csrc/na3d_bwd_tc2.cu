@@ -16,8 +16,6 @@
 // 10 gradient-MMA issuer.
 // Group g takes the chunks of global index parity g; in the epilogue group 0 writes acc1 (dQ or dK,
 // un-rotated), group 1 writes acc2 (dV, MODE 1 only).
-#include <cstdio>
-#include <cstdlib>
 #include <type_traits>
 
 #include "tc_common.cuh"
@@ -178,7 +176,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           const int s = Cn % C::NSTAGE, buf = Cn % C::NBUF;
           mbar_wait<false>(bar_full(s), (uint32_t)(Cn / C::NSTAGE) & 1u);
           mbar_wait<false>(bar_sdfree(buf), ((uint32_t)(Cn / C::NBUF) & 1u) ^ 1u);    // gradient MMAs of chunk Cn - NBUF are done
-          BTRACE(0, Cn);
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
           const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
@@ -187,7 +184,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
           umma_commit(bar_sfull(buf));
-          BTRACE(1, Cn);
           if (c == n - 1) umma_commit(bar_aempty(par));           // the operand tiles are free after these MMAs
         }
       }
@@ -205,7 +201,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           const int s = Cn % C::NSTAGE, buf = Cn % C::NBUF;
           mbar_wait<false>(bar_pfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
           if (c == 0) mbar_wait<false>(bar_accfree(ai), ((uint32_t)ak & 1u) ^ 1u);   // epilogue of the last tile on this accumulator
-          BTRACE(2, Cn);
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
           const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
@@ -216,7 +211,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           }
           umma_commit(bar_empty(s));
           umma_commit(bar_sdfree(buf));
-          BTRACE(3, Cn);
           if (c == n - 1) umma_commit(bar_accdone(ai));
         }
       }
@@ -309,7 +303,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
             const int buf = Cn % C::NBUF;
             const uint32_t sd = tm + C::TMEM_SD + 128 * buf;
             mbar_wait(bar_sfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
-            if (et == 0) BTRACE(4 + 2 * g, Cn);
             tc_fence_after();
             if (__any_sync(0xffffffffu, anyrow && xm != 0u)) {
               auto batch = [&](auto h0c, auto nbc) {
@@ -361,7 +354,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
             }
             tmem_wait_st();
             tc_fence_before();
-            if (et == 0) BTRACE(5 + 2 * g, Cn);
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_pfull(buf));
           }
@@ -442,8 +434,11 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   }
 }
 
+DeviceState g_states[64];
+std::mutex g_mu;
+
 template <class C>
-cudaError_t launch_bwd2_cfg(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
+cudaError_t launch_bwd2_cfg(int slot, const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
                             const float2* stat, const void* rtab, void* dq, void* dk, void* dv,
                             cudaStream_t stream, int* launches) {
   CUtensorMap tq_t, tdo_t, tk_c, tv_c, tk_t, tv_t, tq_c, tdo_c;
@@ -456,34 +451,14 @@ cudaError_t launch_bwd2_cfg(const Problem& p, const void* qr, const void* kr, co
   bp.B = p.B; bp.H = p.H; bp.L = p.L; bp.Y = p.Y; bp.X = p.X; bp.N = p.N;
   bp.ntl = (p.L + C::TL - 1) / C::TL; bp.nty = (p.Y + C::TY - 1) / C::TY; bp.ntx = (p.X + C::TX - 1) / C::TX;
   bp.scale = p.scale; bp.scale_log2e = p.scale * 1.4426950408889634f; bp.pairing = p.pairing;
-#ifdef STRATA_TRACE
-  {
-    const char* e = getenv("STRATA_TRACE_PTR");
-    bp.trace = e ? (unsigned long long*)strtoull(e, nullptr, 0) : nullptr;
-    const char* cc = getenv("STRATA_TRACE_CTA");
-    bp.trace_cta = cc ? atoi(cc) : 0;
-  }
-#endif
   const long long ntiles = (long long)p.B * p.H * bp.ntl * bp.nty * bp.ntx;
   if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
-  static int sm_count = 0;
-  if (sm_count == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        sm_count <= 0) {
-      (void)cudaGetLastError();
-      sm_count = 148;
-    }
-  }
-  const unsigned grid = (unsigned)(ntiles < sm_count ? ntiles : sm_count);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(na3d_bwd_tc2_kernel<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(na3d_bwd_tc2_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  DeviceState* ds = device_state(g_states, g_mu);
+  if (!ds) return cudaErrorInvalidDevice;
+  const unsigned grid = (unsigned)(ntiles < ds->sm_count ? ntiles : ds->sm_count);
+  cudaError_t e = ensure_smem_attr(ds, g_mu, 2 * slot, na3d_bwd_tc2_kernel<C, 0>, C::SMEM_BYTES);
+  if (e == cudaSuccess) e = ensure_smem_attr(ds, g_mu, 2 * slot + 1, na3d_bwd_tc2_kernel<C, 1>, C::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
   prof_begin("na3d_bwd_dq_tcgen05", stream);
   na3d_bwd_tc2_kernel<C, 0><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, (const float4*)rtab,
                                                                           (__nv_bfloat16*)dq, nullptr, bp, (int)ntiles);
@@ -502,12 +477,12 @@ cudaError_t launch_bwd2_cfg(const Problem& p, const void* qr, const void* kr, co
 cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
                                 const void* stat, const void* rtab, void* dq, void* dk, void* dv,
                                 cudaStream_t stream, int* launches) {
-#define X(KL_, KY_, KX_)                                        \
+#define X(I_, KL_, KY_, KX_)                                   \
   if (p.kL == KL_ && p.kY == KY_ && p.kX == KX_)                \
-    return launch_bwd2_cfg<Bwd2Cfg<KL_, KY_, KX_>>(p, qr, kr, v, d_o, (const float2*)stat, rtab, dq, dk, dv, stream, launches);
-  X(3, 7, 7)
-  X(3, 5, 5)
-  X(3, 3, 3)
+    return launch_bwd2_cfg<Bwd2Cfg<KL_, KY_, KX_>>(I_, p, qr, kr, v, d_o, (const float2*)stat, rtab, dq, dk, dv, stream, launches);
+  X(0, 3, 7, 7)
+  X(1, 3, 5, 5)
+  X(2, 3, 3, 3)
 #undef X
   return cudaErrorNotSupported;
 }

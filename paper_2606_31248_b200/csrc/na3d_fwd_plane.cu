@@ -52,8 +52,6 @@
 // and c + HX / 2 is inside it, so the two halves of every key row are FOLDED with a per-thread bit select before
 // the exponential (half the MUFU work); P is packed to bf16 folded and un-folded by one byte permute per output
 // word (a masked slot replicates the zero sign bit).
-#include <mutex>
-
 #include "tc_common.cuh"
 
 namespace strata {
@@ -149,6 +147,7 @@ __device__ __forceinline__ void warp_arrive(uint32_t bar) {
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 // ---- A2 in packed bf16x2 arithmetic.  Table words: C = (cos m, cos m+1), S = (sin m, sin m+1).
 __device__ __forceinline__ uint32_t bmul2(uint32_t a, uint32_t b) {
   uint32_t d;
@@ -723,7 +722,10 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
                   }
               }
             }
-            bar_sync(bar_pr, 64);                                    // every S row of the subpartition is in registers: P may go over S
+            // P goes over the front of S.  The P rows of the first warp land on S rows it has read itself (P row r is
+            // in S row r / 2); those of the second warp land on S rows of the first: it waits (below, before its
+            // stores) until the first one has its rows in registers.
+            if (half == 0) bar_arrive(bar_pr, 64);
             // ---- exponentials, row sums, P (bf16, un-folded) over the S rows
             uint32_t pw[C::NR * C::PW];
             float e0 = 0.f, e1 = 0.f;
@@ -753,6 +755,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
                 pw[r * C::PW + jj] = prmt(f[((2 * jj) % C::HALF) / 2], f[((2 * jj + 1) % C::HALF) / 2], psel[jj]);
             }
             lsum += e0 + e1;
+            if (half == 1) bar_sync(bar_pr, 64);
             tmem_st_n<C::NR * C::PW>(s_tm + rw * C::PW, pw);
             // ---- key rows no query of the subpartition attends, pad keys: P = 0.  Away from the grid border the
             // needed rows are the first or the last NEED rows of the halo.
@@ -911,26 +914,8 @@ bool plane_shape_ok(const Problem& p) {
 template <class C>
 bool make_plane_map(CUtensorMap* map, const void* ptr, const Problem& p) { return make_map(map, ptr, p, C::HX, C::HY, 1); }
 
-// per-device launch state (attribute set, SM count)
-struct DeviceState {
-  int sm_count = 0;
-  bool attr[8] = {};
-};
-DeviceState* device_state() {
-  static std::mutex mu;
-  static DeviceState states[64];
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return nullptr; }
-  std::lock_guard<std::mutex> lock(mu);
-  DeviceState* s = &states[dev];
-  if (s->sm_count == 0) {
-    if (cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || s->sm_count <= 0) {
-      (void)cudaGetLastError();
-      s->sm_count = 148;
-    }
-  }
-  return s;
-}
+DeviceState g_states[64];
+std::mutex g_mu;
 
 template <class C>
 cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const void* k, const void* v, const float* coords,
@@ -947,7 +932,7 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   const long long ncols = (long long)p.B * p.H * sp.nty * sp.ntx;
   if (ncols > 0x7fffffffLL / 256) return cudaErrorInvalidValue;
   sp.ncols = (int)ncols;
-  DeviceState* ds = device_state();
+  DeviceState* ds = device_state(g_states, g_mu);
   if (!ds) return cudaErrorInvalidDevice;
   // Heads per unit: as many as possible (the rotary table of a tile is built once per unit) while the units still
   // spread evenly over the SMs (at most ~3 % more units on the busiest CTA than on average).
@@ -962,12 +947,9 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   const long long grid = nunits < ds->sm_count ? nunits : ds->sm_count;      // persistent: one CTA per SM
   auto kernel = p.pairing ? na3d_fwd_plane_kernel<C, 1> : na3d_fwd_plane_kernel<C, 0>;
   const int ai = 2 * cfg_index + (p.pairing ? 1 : 0);
-  if (!ds->attr[ai]) {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    ds->attr[ai] = true;
-  }
-  cudaError_t e = cudaMemsetAsync(fix, 0, 16, stream);
+  cudaError_t e = ensure_smem_attr(ds, g_mu, ai, kernel, C::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(fix, 0, 16, stream);
   if (e != cudaSuccess) return e;
   prof_begin("na3d_fwd_plane", stream);
   kernel<<<(unsigned)grid, kPlaneThreads, C::SMEM_BYTES, stream>>>(tk, tv, (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, coords, freqs,

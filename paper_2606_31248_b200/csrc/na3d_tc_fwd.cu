@@ -324,8 +324,11 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
 // ------------------------------------------------------------------------------------------------
 // Host side: tensor maps + launch
 // ------------------------------------------------------------------------------------------------
+DeviceState g_states[64];
+std::mutex g_mu;
+
 template <class C>
-cudaError_t launch_cfg(const Problem& p, const void* qr, const void* kr, const void* v, void* o, float* lse,
+cudaError_t launch_cfg(int slot, const Problem& p, const void* qr, const void* kr, const void* v, void* o, float* lse,
                        cudaStream_t stream, int* launches) {
   CUtensorMap tq, tk, tv;
   if (!make_map(&tq, qr, p, C::TX, C::TY, C::TL) || !make_map(&tk, kr, p, C::HX, C::CY, 1) ||
@@ -337,12 +340,10 @@ cudaError_t launch_cfg(const Problem& p, const void* qr, const void* kr, const v
   tp.scale_log2e = p.scale * 1.4426950408889634f;
   const long long grid = (long long)p.B * p.H * tp.ntl * tp.nty * tp.ntx;
   if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(na3d_fwd_tc_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  DeviceState* ds = device_state(g_states, g_mu);
+  if (!ds) return cudaErrorInvalidDevice;
+  cudaError_t e = ensure_smem_attr(ds, g_mu, slot, na3d_fwd_tc_kernel<C>, C::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
   prof_begin("na3d_fwd_tcgen05", stream);
   na3d_fwd_tc_kernel<C><<<(unsigned)grid, kThreads, C::SMEM_BYTES, stream>>>(tq, tk, tv, (__nv_bfloat16*)o, lse, tp);
   prof_end(stream);
@@ -354,15 +355,14 @@ cudaError_t launch_cfg(const Problem& p, const void* qr, const void* kr, const v
 
 // Shapes the tensor-core path covers: bf16, head_dim 64 / 128, the window sizes instantiated below.
 #define STRATA_TC_CONFIGS(X) \
-  X(64, 3, 7, 7)             \
-  X(128, 5, 9, 9)            \
-  X(64, 3, 5, 5)             \
-  X(64, 3, 3, 3)
+  X(0, 64, 3, 7, 7)          \
+  X(1, 128, 5, 9, 9)         \
+  X(2, 64, 3, 5, 5)          \
+  X(3, 64, 3, 3, 3)
 
 bool tc_fwd_supported(const Problem& p) {
   if (p.dtype != 1) return false;
-  if (!p.force_tile && tc_sweep_supported(p)) return true;
-#define X(D_, KL_, KY_, KX_) \
+#define X(I_, D_, KL_, KY_, KX_) \
   if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_) return true;
   STRATA_TC_CONFIGS(X)
 #undef X
@@ -371,10 +371,9 @@ bool tc_fwd_supported(const Problem& p) {
 
 cudaError_t launch_fwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
                           float* lse, cudaStream_t stream, int* launches) {
-  if (!p.force_tile && tc_sweep_supported(p)) return launch_fwd_sweep(p, qr, kr, v, o, lse, stream, launches);
-#define X(D_, KL_, KY_, KX_)                                               \
+#define X(I_, D_, KL_, KY_, KX_)                                           \
   if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)               \
-    return launch_cfg<Cfg<D_, KL_, KY_, KX_>>(p, qr, kr, v, o, lse, stream, launches);
+    return launch_cfg<Cfg<D_, KL_, KY_, KX_>>(I_, p, qr, kr, v, o, lse, stream, launches);
   STRATA_TC_CONFIGS(X)
 #undef X
   return cudaErrorNotSupported;

@@ -68,37 +68,6 @@ rope_rotate_kernel(const TIn* __restrict__ x0, const TIn* __restrict__ x1, TOut*
   }
 }
 
-// A1 for the fused tensor-core kernels: one 2*D-byte table row per token (all heads of a token share
-// it) of bf16x2 words, two per pair of rotary pairs (m, m+1), m even:
-//   word m     = (cos phi[t][m], cos phi[t][m+1])      word m + 1 = (sin phi[t][m], sin phi[t][m+1])
-// -- the operand layout of the packed bf16x2 rotation in na3d_fwd_fused.cu.  One thread per (token, m).
-__global__ void __launch_bounds__(256)
-rope_table_kernel(uint4* __restrict__ table, const float* __restrict__ coords, const float* __restrict__ freqs,
-                  long long tokens, int half, int A) {
-  const int eighth = half >> 2;                       // one thread per (token, 4 pairs) = one 16-byte store
-  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= tokens * eighth) return;
-  const long long t = gid / eighth;
-  const int m = 4 * (int)(gid - t * eighth);
-  // The table is rounded to bf16 (2^-9): an fp32 angle (|phi| <~ 2e3 rad -> 1e-4 rad of rounding), a two-term
-  // Cody-Waite reduction to [-pi, pi] and the MUFU sin / cos (2^-21 abs on that range) are far inside that.
-  float cs[4], sn[4];
-#pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    float phi = 0.f;
-    for (int a = 0; a < A; ++a) phi = fmaf(coords[t * A + a], freqs[a * half + m + u], phi);
-    const float n = rintf(phi * 0.15915494309189535f);
-    const float r = fmaf(n, 1.7484555e-7f, fmaf(n, -6.2831854820251465f, phi));    // 2 pi = 6.2831854820251465 - 1.7484555e-7
-    __sincosf(r, &sn[u], &cs[u]);
-  }
-  const __nv_bfloat162 c0 = __floats2bfloat162_rn(cs[0], cs[1]), s0 = __floats2bfloat162_rn(sn[0], sn[1]);
-  const __nv_bfloat162 c1 = __floats2bfloat162_rn(cs[2], cs[3]), s1 = __floats2bfloat162_rn(sn[2], sn[3]);
-  uint4 w;
-  w.x = *reinterpret_cast<const uint32_t*>(&c0); w.y = *reinterpret_cast<const uint32_t*>(&s0);
-  w.z = *reinterpret_cast<const uint32_t*>(&c1); w.w = *reinterpret_cast<const uint32_t*>(&s1);
-  table[gid] = w;
-}
-
 // A1 + A2 for bf16 -> bf16 (the operands of the tensor-core kernels that take pre-rotated Q, K): 16-byte
 // accesses, one thread per (token, group of 8 channels) looping over the heads and both tensors with the
 // group's cos / sin in registers.  The result is rounded to bf16 (2^-9), so the angle is reduced and
@@ -188,20 +157,6 @@ cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* co
   if (grid <= 0 || grid > 0x7fffffffLL) return cudaErrorInvalidValue;
   prof_begin("rope_table_f32", stream);
   rope_table_f32_kernel<<<(unsigned)grid, 256, 0, stream>>>((float2*)table, coords, freqs, tokens, p.D / 2, p.A);
-  prof_end(stream);
-  if (launches) ++*launches;
-  return cudaGetLastError();
-}
-
-cudaError_t launch_rope_table(const Problem& p, void* table, const float* coords, const float* freqs,
-                              cudaStream_t stream, int* launches) {
-  const long long tokens = (long long)p.B * p.N;
-  const long long threads = tokens * (p.D / 8);
-  const int block = 256;
-  const long long grid = (threads + block - 1) / block;
-  if (grid <= 0 || grid > 0x7fffffffLL || (p.D & 7)) return cudaErrorInvalidValue;
-  prof_begin("rope_table", stream);
-  rope_table_kernel<<<(unsigned)grid, block, 0, stream>>>((uint4*)table, coords, freqs, tokens, p.D / 2, p.A);
   prof_end(stream);
   if (launches) ++*launches;
   return cudaGetLastError();

@@ -2,8 +2,6 @@
 // carving, kernel-family dispatch, host-buffer variants.  No arithmetic lives here.
 #include "../../include/strata_na3d.h"
 
-#include <cstdlib>
-
 #include "common.cuh"
 
 namespace {
@@ -50,18 +48,14 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
 }
 
 // Kernel path of a call.  The public strata_impl_t only distinguishes SIMT from TCGEN05.
-enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_FUSED = 3, PATH_TC_SWEEP = 4, PATH_TC_PLANE = 5 };
+enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_PLANE = 3 };
 
-// AUTO -> fused tcgen05 kernel when it covers the problem, else the tcgen05 tile kernel on pre-rotated
-// operands, else SIMT.  PATH_NONE when `impl` asks for a family that does not cover the problem.
+// AUTO -> the fused tcgen05 forward (na3d_fwd_plane.cu) when it covers the problem, else the tcgen05 tile kernels on
+// pre-rotated operands, else SIMT.  PATH_NONE when `impl` asks for a family that does not cover the problem.
 Path select_path(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
   if (d->impl == STRATA_IMPL_SIMT) return PATH_SIMT;
-  if (!backward && !p.force_tile && !getenv("STRATA_OLD_SWEEP") && strata::plane_fwd_supported(p)) return PATH_TC_PLANE;
-  const bool sweep_ok = !backward && !p.force_tile && !getenv("STRATA_OLD_FUSED") && strata::sweep_fwd_supported(p);
-  if (sweep_ok) return PATH_TC_SWEEP;
-  const bool fused_ok = !backward && !p.force_tile && strata::fused_fwd_supported(p);
+  if (!backward && !p.force_tile && strata::plane_fwd_supported(p)) return PATH_TC_PLANE;
   const bool tc_ok = backward ? strata::tc_bwd_supported(p) : strata::tc_fwd_supported(p);
-  if (fused_ok) return PATH_TC_FUSED;
   if (tc_ok) return PATH_TC_PREROT;
   return d->impl == STRATA_IMPL_AUTO ? PATH_SIMT : PATH_NONE;
 }
@@ -88,8 +82,6 @@ size_t ws_bytes(const Problem& p, Path path, bool backward) {
     return 2 * align_up(e * 2) + align_up(2 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
   if (path == PATH_TC_PLANE) return align_up(strata::plane_fwd_workspace_bytes());
-  if (path == PATH_TC_SWEEP) return 0;
-  if (path == PATH_TC_FUSED) return align_up((size_t)p.B * p.N * p.D * 2);   // (cos, sin) half2 table
   if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
   return 2 * align_up(e * 4);                                            // qr, kr (f32)
 }
@@ -186,15 +178,6 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
   if (path == PATH_TC_PLANE) {
     void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
     e = strata::launch_fwd_plane(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);
-  } else if (path == PATH_TC_SWEEP) {
-    e = strata::launch_fwd_sweep2(p, q, k, v, coords, freqs, o, lse, st, &launches);
-  } else if (path == PATH_TC_FUSED) {
-    void* table = ws.take<char>((size_t)p.B * p.N * p.D * 2);
-    if (p.A > 0) {
-      e = strata::launch_rope_table(p, table, coords, freqs, st, &launches);
-      if (e != cudaSuccess) return cuda_status(e);
-    }
-    e = strata::launch_fwd_fused(p, q, k, v, table, o, lse, st, &launches);
   } else if (path == PATH_TC_PREROT) {
     void* qr = ws.take<char>((size_t)p.elems() * 2);
     void* kr = ws.take<char>((size_t)p.elems() * 2);

@@ -2,6 +2,8 @@
 // helper shared by the tensor-core kernels.  sm_100a only.
 #pragma once
 #include <cuda.h>
+
+#include <mutex>
 #ifdef STRATA_DEBUG_SYNC
 #include <cstdio>
 #endif
@@ -157,17 +159,45 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 inline EncodeTiledFn encode_fn() {
   static EncodeTiledFn fn = nullptr;
-  static bool tried = false;
-  if (!tried) {
-    tried = true;
+  static std::once_flag once;
+  std::call_once(once, [] {
     void* sym = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
         qres == cudaDriverEntryPointSuccess)
       fn = reinterpret_cast<EncodeTiledFn>(sym);
     (void)cudaGetLastError();
-  }
+  });
   return fn;
+}
+
+// Per-DEVICE launch state of one kernel family: the SM count and which kernels already have their dynamic
+// shared-memory limit raised (cudaFuncSetAttribute is per device).  One instance per translation unit.
+struct DeviceState {
+  int sm_count = 0;
+  bool attr[16] = {};
+};
+inline DeviceState* device_state(DeviceState (&states)[64], std::mutex& mu) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return nullptr; }
+  std::lock_guard<std::mutex> lock(mu);
+  DeviceState* s = &states[dev];
+  if (s->sm_count == 0) {
+    if (cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || s->sm_count <= 0) {
+      (void)cudaGetLastError();
+      s->sm_count = 148;
+    }
+  }
+  return s;
+}
+// Raises the dynamic shared-memory limit of `kernel` once per device (slot: index of the kernel in the family).
+template <class K>
+inline cudaError_t ensure_smem_attr(DeviceState* ds, std::mutex& mu, int slot, K kernel, int bytes) {
+  std::lock_guard<std::mutex> lock(mu);
+  if (ds->attr[slot]) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) ds->attr[slot] = true;
+  return e;
 }
 
 // Tensor [B*L, Y, X, H, D] bf16 as a rank-5 map (fastest first: d, h, x, y, b*l); box = 64 channels of
