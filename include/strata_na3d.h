@@ -146,6 +146,28 @@ int strata_na3d_profile_read(float* ms, const char** names, int capacity);
 int strata_na3d_window_start(int i, int k, int n);
 int strata_na3d_inverse_window(int j, int k, int n, int* lo, int* hi);
 
+/* ---- geometry of the StereoRoPE inputs on the device --------------------------------------
+ * Both calls are elementwise over n points, asynchronous on `stream`, and take DEVICE pointers.  lat / lon are
+ * float64 radians (the coordinates reach ~1.5e3 at l_scale of the 2048^2-cell faces: float32 inputs would not
+ * resolve the float32 result).
+ *
+ * strata_stereo_coords: eq. (1).  Tile-centred stereographic coordinates of the points
+ * (lat[i], lon[i]) about the tile centre (lat0, lon0), divided by l_scale = sqrt(4 pi / n_total):
+ *   cos c = sin p0 sin p + cos p0 cos p cos(l - l0),  k = 2 / (1 + cos c),
+ *   x = (k / l_scale) cos p sin(l - l0),  y = (k / l_scale) (cos p0 sin p - sin p0 cos p cos(l - l0)).
+ * Writes coords[i * stride + 0] = x, coords[i * stride + 1] = y (float32; stride >= 2: the [.., A] layout of
+ * strata_na3d_fwd's coords with A = stride).  INVALID_ARG if n < 0, stride < 2, n_total <= 0 or a pointer is NULL.
+ *
+ * strata_wind_to_tile_frame: eq. (2).  The wind (u[i], v[i]) (East, North at its own point)
+ * as a 3D vector, projected onto the tangent plane at the tile centre, in the centre's East-North frame:
+ *   v3 = u e + v n,  v_perp = v3 - (v3 . r0) r0,  u_loc = v_perp . e0,  v_loc = v_perp . n0.
+ * u_loc / v_loc may alias u / v. */
+strata_status_t strata_stereo_coords(const double* lat, const double* lon, long long n, double lat0, double lon0,
+                                     double n_total, float* coords, int stride, void* stream);
+strata_status_t strata_wind_to_tile_frame(const float* u, const float* v, const double* lat, const double* lon,
+                                          long long n, double lat0, double lon0, float* u_loc, float* v_loc,
+                                          void* stream);
+
 const char* strata_status_string(strata_status_t status);
 int strata_version(void);
 

@@ -24,7 +24,8 @@ IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_TILE = 0, 1, 2, 3
 EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
            "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",
            "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
-           "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_status_string", "strata_version")
+           "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_stereo_coords",
+           "strata_wind_to_tile_frame", "strata_status_string", "strata_version")
 
 
 class StrataError(RuntimeError):
@@ -106,6 +107,12 @@ def lib() -> ctypes.CDLL:
         L.strata_na3d_window_start.argtypes = [i32, i32, i32]
         L.strata_na3d_inverse_window.restype = i32
         L.strata_na3d_inverse_window.argtypes = [i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i32)]
+        L.strata_stereo_coords.restype = i32
+        L.strata_stereo_coords.argtypes = [vp, vp, ctypes.c_longlong, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                           vp, i32, vp]
+        L.strata_wind_to_tile_frame.restype = i32
+        L.strata_wind_to_tile_frame.argtypes = [vp, vp, vp, vp, ctypes.c_longlong, ctypes.c_double, ctypes.c_double,
+                                                vp, vp, vp]
         L.strata_status_string.restype = ctypes.c_char_p
         L.strata_status_string.argtypes = [i32]
         L.strata_version.restype = i32
@@ -218,6 +225,29 @@ def strata_na3d_fwd_host(desc, q, k, v, coords, freqs, o, lse, workspace, stream
 def strata_na3d_bwd_host(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None):
     _check(strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream,
                                   host=True), "strata_na3d_bwd_host")
+
+
+# ------------------------------------------------------------------ geometry
+def strata_stereo_coords(lat, lon, lat0: float, lon0: float, n_total: float, coords, stride: int = 2, stream=None):
+    """Eq. (1) on the device: lat, lon float64 CUDA tensors of n points -> coords[i * stride + {0, 1}] (float32)."""
+    n = lat.numel()
+    if lon.numel() != n or lat.dtype != torch.float64 or lon.dtype != torch.float64 or coords.dtype != torch.float32:
+        raise TypeError("lat, lon: float64 tensors of equal size; coords: float32")
+    if coords.numel() < n * stride:
+        raise ValueError("coords too small")
+    _check(lib().strata_stereo_coords(_ptr(lat), _ptr(lon), n, float(lat0), float(lon0), float(n_total), _ptr(coords),
+                                      int(stride), _stream_handle(stream)), "strata_stereo_coords")
+
+
+def strata_wind_to_tile_frame(u, v, lat, lon, lat0: float, lon0: float, u_loc, v_loc, stream=None):
+    """Eq. (2) on the device: winds (u, v) float32 at (lat, lon) float64 -> (u_loc, v_loc) float32."""
+    n = u.numel()
+    for t, dt in ((u, torch.float32), (v, torch.float32), (u_loc, torch.float32), (v_loc, torch.float32),
+                  (lat, torch.float64), (lon, torch.float64)):
+        if t.numel() != n or t.dtype != dt:
+            raise TypeError("u, v, u_loc, v_loc: float32; lat, lon: float64; all of one size")
+    _check(lib().strata_wind_to_tile_frame(_ptr(u), _ptr(v), _ptr(lat), _ptr(lon), n, float(lat0), float(lon0),
+                                           _ptr(u_loc), _ptr(v_loc), _stream_handle(stream)), "strata_wind_to_tile_frame")
 
 
 # ------------------------------------------------------------------ convenience: allocate + call

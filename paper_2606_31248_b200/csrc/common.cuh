@@ -63,6 +63,14 @@ size_t plane_fwd_workspace_bytes();
 cudaError_t launch_fwd_plane(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
                              const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches);
 
+cudaError_t launch_fix_rows(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
+                            const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches);
+
+// na3d_column.cu: column-wise attention (window (L, 1, 1)), bf16, head_dim 64, L <= 32; same `fix`.
+bool column_fwd_supported(const Problem& p);
+cudaError_t launch_fwd_column(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
+                              const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches);
+
 // na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
 cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             void* o, float* lse, cudaStream_t stream, int* launches);

@@ -1,0 +1,85 @@
+// geometry.cu -- the StereoRoPE inputs on the device: eq. (1) (tile-centred stereographic coordinates)
+// and eq. (2) (winds in the tile centre's East-North frame).  Elementwise, HBM-bound (16 bytes of
+// lat / lon in per point); float64 arithmetic because the coordinates (up to ~1.5e3 in units of l_scale) are handed
+// to the attention kernels as float32 and must be correct to the last bit or two of that.
+#include "../../include/strata_na3d.h"
+
+#include "common.cuh"
+
+namespace strata {
+namespace {
+
+// eq. (1)
+__global__ void __launch_bounds__(256)
+stereo_coords_kernel(const double* __restrict__ lat, const double* __restrict__ lon, long long n, double sin0,
+                     double cos0, double lon0, double inv_ell, float* __restrict__ coords, int stride) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    double sp, cp, sd, cd;
+    sincos(lat[i], &sp, &cp);
+    sincos(lon[i] - lon0, &sd, &cd);
+    const double cosc = sin0 * sp + cos0 * cp * cd;
+    const double k = 2.0 / (1.0 + cosc) * inv_ell;
+    coords[i * stride] = (float)(k * cp * sd);
+    coords[i * stride + 1] = (float)(k * (cos0 * sp - sin0 * cp * cd));
+  }
+}
+
+// eq. (2): v3 = u e + v n in geocentric Cartesian axes (x through (lat, lon) = (0, 0), z the pole); the radial part
+// at the tile centre is removed, then the components along e0 and n0 are taken.
+__global__ void __launch_bounds__(256)
+wind_frame_kernel(const float* __restrict__ u, const float* __restrict__ v, const double* __restrict__ lat,
+                  const double* __restrict__ lon, long long n, double sin0, double cos0, double sl0, double cl0,
+                  float* __restrict__ u_loc, float* __restrict__ v_loc) {
+  const double r0x = cos0 * cl0, r0y = cos0 * sl0, r0z = sin0;
+  const double e0x = -sl0, e0y = cl0;
+  const double n0x = -sin0 * cl0, n0y = -sin0 * sl0, n0z = cos0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    double sp, cp, sl, cl;
+    sincos(lat[i], &sp, &cp);
+    sincos(lon[i], &sl, &cl);
+    const double uu = (double)u[i], vv = (double)v[i];
+    double x = -uu * sl - vv * sp * cl, y = uu * cl - vv * sp * sl, z = vv * cp;
+    const double rad = x * r0x + y * r0y + z * r0z;
+    x -= rad * r0x; y -= rad * r0y; z -= rad * r0z;
+    u_loc[i] = (float)(x * e0x + y * e0y);
+    v_loc[i] = (float)(x * n0x + y * n0y + z * n0z);
+  }
+}
+
+unsigned grid_for(long long n) {
+  const long long b = (n + 255) / 256;
+  return (unsigned)(b < 1 ? 1 : b > 148 * 32 ? 148 * 32 : b);
+}
+
+}  // namespace
+}  // namespace strata
+
+extern "C" {
+
+strata_status_t strata_stereo_coords(const double* lat, const double* lon, long long n, double lat0, double lon0,
+                                     double n_total, float* coords, int stride, void* stream) {
+  if (n < 0 || stride < 2 || !(n_total > 0.0) || !lat || !lon || !coords) return STRATA_ERR_INVALID_ARG;
+  if (n == 0) return STRATA_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const double inv_ell = 1.0 / sqrt(4.0 * 3.14159265358979323846 / n_total);
+  strata::prof_begin("stereo_coords", st);
+  strata::stereo_coords_kernel<<<strata::grid_for(n), 256, 0, st>>>(lat, lon, n, sin(lat0), cos(lat0), lon0, inv_ell, coords, stride);
+  strata::prof_end(st);
+  if (cudaGetLastError() != cudaSuccess) return STRATA_ERR_CUDA;
+  return STRATA_OK;
+}
+
+strata_status_t strata_wind_to_tile_frame(const float* u, const float* v, const double* lat, const double* lon,
+                                          long long n, double lat0, double lon0, float* u_loc, float* v_loc,
+                                          void* stream) {
+  if (n < 0 || !u || !v || !lat || !lon || !u_loc || !v_loc) return STRATA_ERR_INVALID_ARG;
+  if (n == 0) return STRATA_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  strata::prof_begin("wind_to_tile_frame", st);
+  strata::wind_frame_kernel<<<strata::grid_for(n), 256, 0, st>>>(u, v, lat, lon, n, sin(lat0), cos(lat0), sin(lon0), cos(lon0), u_loc, v_loc);
+  strata::prof_end(st);
+  if (cudaGetLastError() != cudaSuccess) return STRATA_ERR_CUDA;
+  return STRATA_OK;
+}
+
+}  // extern "C"

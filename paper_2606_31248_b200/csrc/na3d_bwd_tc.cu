@@ -48,7 +48,8 @@ cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr
 #define STRATA_BWD_CONFIGS(X) \
   X(3, 7, 7)                  \
   X(3, 5, 5)                  \
-  X(3, 3, 3)
+  X(3, 3, 3)                  \
+  X(9, 9, 9)
 
 bool tc_bwd_supported(const Problem& p) {
   if (p.dtype != 1 || p.D != 64) return false;

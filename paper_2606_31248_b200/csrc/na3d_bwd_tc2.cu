@@ -483,6 +483,7 @@ cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr
   X(0, 3, 7, 7)
   X(1, 3, 5, 5)
   X(2, 3, 3, 3)
+  X(3, 9, 9, 9)
 #undef X
   return cudaErrorNotSupported;
 }

@@ -958,13 +958,7 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   if (launches) ++*launches;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  prof_begin("na3d_fix_rows", stream);
-  na3d_fix_rows_kernel<<<ds->sm_count, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k,
-                                                         (const __nv_bfloat16*)v, coords, freqs, (__nv_bfloat16*)o, lse,
-                                                         reinterpret_cast<const unsigned long long*>(fix), kFixCap, p);
-  prof_end(stream);
-  if (launches) ++*launches;
-  return cudaGetLastError();
+  return launch_fix_rows(p, q, k, v, coords, freqs, o, lse, fix, stream, launches);
 }
 
 }  // namespace
@@ -976,6 +970,19 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
   X(2, 3, 3, 4, 3)
 
 size_t plane_fwd_workspace_bytes() { return 16 + 8 * (size_t)kFixCap; }
+
+// The rows listed in `fix` (plane_fwd_workspace_bytes() of device memory: [0] count, [1] != 0: every row, [2 ...] row
+// ids), recomputed with the two-pass SIMT softmax.  head_dim 64, bf16.
+cudaError_t launch_fix_rows(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
+                            const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches) {
+  prof_begin("na3d_fix_rows", stream);
+  na3d_fix_rows_kernel<<<148, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v,
+                                                coords, freqs, (__nv_bfloat16*)o, lse,
+                                                reinterpret_cast<const unsigned long long*>(fix), kFixCap, p);
+  prof_end(stream);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
 
 bool plane_fwd_supported(const Problem& p) {
   if (p.dtype != 1 || p.D != 64 || p.kL != 3 || p.A > 2) return false;   // (A = 3: the level is a rotary axis, no shared table)

@@ -48,13 +48,14 @@ bool make_problem(const strata_na3d_desc_t* d, Problem* p, strata_status_t* why)
 }
 
 // Kernel path of a call.  The public strata_impl_t only distinguishes SIMT from TCGEN05.
-enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_PLANE = 3 };
+enum Path { PATH_NONE = -1, PATH_SIMT = 1, PATH_TC_PREROT = 2, PATH_TC_PLANE = 3, PATH_COLUMN = 4 };
 
 // AUTO -> the fused tcgen05 forward (na3d_fwd_plane.cu) when it covers the problem, else the tcgen05 tile kernels on
 // pre-rotated operands, else SIMT.  PATH_NONE when `impl` asks for a family that does not cover the problem.
 Path select_path(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
   if (d->impl == STRATA_IMPL_SIMT) return PATH_SIMT;
   if (!backward && !p.force_tile && strata::plane_fwd_supported(p)) return PATH_TC_PLANE;
+  if (!backward && !p.force_tile && strata::column_fwd_supported(p)) return PATH_COLUMN;
   const bool tc_ok = backward ? strata::tc_bwd_supported(p) : strata::tc_fwd_supported(p);
   if (tc_ok) return PATH_TC_PREROT;
   return d->impl == STRATA_IMPL_AUTO ? PATH_SIMT : PATH_NONE;
@@ -63,7 +64,7 @@ Path select_path(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
 int select_impl(const strata_na3d_desc_t* d, const Problem& p, bool backward) {
   const Path path = select_path(d, p, backward);
   if (path == PATH_NONE) return -1;
-  return path == PATH_SIMT ? STRATA_IMPL_SIMT : STRATA_IMPL_TCGEN05;
+  return path == PATH_SIMT ? STRATA_IMPL_SIMT : STRATA_IMPL_TCGEN05;   // (the column kernel counts as the tensor-core family)
 }
 
 struct Carve {
@@ -81,7 +82,7 @@ size_t ws_bytes(const Problem& p, Path path, bool backward) {
   if (backward && path == PATH_TC_PREROT)                               // qr, kr (bf16), stat (float2), fp32 rotary table
     return 2 * align_up(e * 2) + align_up(2 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
-  if (path == PATH_TC_PLANE) return align_up(strata::plane_fwd_workspace_bytes());
+  if (path == PATH_TC_PLANE || path == PATH_COLUMN) return align_up(strata::plane_fwd_workspace_bytes());
   if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
   return 2 * align_up(e * 4);                                            // qr, kr (f32)
 }
@@ -178,6 +179,9 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
   if (path == PATH_TC_PLANE) {
     void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
     e = strata::launch_fwd_plane(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);
+  } else if (path == PATH_COLUMN) {
+    void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
+    e = strata::launch_fwd_column(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);
   } else if (path == PATH_TC_PREROT) {
     void* qr = ws.take<char>((size_t)p.elems() * 2);
     void* kr = ws.take<char>((size_t)p.elems() * 2);

@@ -103,6 +103,18 @@ def config(index: int) -> Workload:
     raise ValueError(f"no BASELINE.json config {index}")
 
 
+def production(which: str) -> Workload:
+    """The paper's own attention shapes (PAPER.md:325-326 Table S1, 454): 24 levels, 16 heads, head_dim 1024 / 16 =
+    64, NATTEN kernel size 9 (read as 9 x 9 x 9, DESIGN.md R2), tiles of 64 x 64 or 128 x 128 cells at patch size 4;
+    inputs as QK-RMSNorm leaves them.  "col*": the column-wise attention blocks that alternate with
+    them: every level of one (y, x) column.  Not BASELINE.json configs: extra bench / parity shapes."""
+    s = BASE_SEED + 50
+    shapes = {"prod16": ((24, 16, 16), (9, 9, 9)), "prod32": ((24, 32, 32), (9, 9, 9)),
+              "col16": ((24, 16, 16), (24, 1, 1)), "col32": ((24, 32, 32), (24, 1, 1))}
+    grid, window = shapes[which]
+    return Workload(f"{which}_fwd", -1, 8 if grid[1] == 16 else 2, 16, 64, grid, window, "bf16", value_scale="qknorm", seed=s)
+
+
 def small(name: str = "small", **kw) -> Workload:
     """Ad-hoc small workload for parity sweeps; keyword overrides on a 1x2x32 default."""
     base = Workload(name, -1, 1, 2, 32, (3, 6, 7), (3, 3, 3), "f32", seed=BASE_SEED + 99)

@@ -293,6 +293,47 @@ def test_device_error_paths_and_stream():
     assert binding.strata_na3d_last_launch_count() >= 2
 
 
+def _guarded(shape, dtype, guard=8192):
+    """A tensor carved out of a larger byte buffer with canary bands on both sides."""
+    n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+    pad = (n + 255) // 256 * 256
+    raw = torch.full((guard + pad + guard,), 0xA5, dtype=torch.uint8, device="cuda")
+    view = raw[guard:guard + n].view(dtype).view(shape)
+    return raw, view, guard, n
+
+
+def _guards_intact(raw, guard, n):
+    return bool((raw[:guard] == 0xA5).all()) and bool((raw[guard + n:] == 0xA5).all())
+
+
+@pytest.mark.parametrize("case", [dict(grid=(5, 11, 13), window=(3, 7, 7), heads=2, head_dim=64),
+                                  dict(grid=(8, 17, 9), window=(3, 5, 5), heads=3, head_dim=64, batch=2),
+                                  dict(grid=(6, 10, 17), window=(5, 9, 9), heads=1, head_dim=128),
+                                  dict(grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32, dtype="f32")])
+def test_no_write_outside_the_output_buffers(case):
+    """compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md): every output and the workspace sit
+    between canary bands here, ragged shapes, forward and backward; a stray store shows up in a band."""
+    kw = dict(dtype="bf16")
+    kw.update(case)
+    w = wl.small(name="guard", **kw)
+    inp = wl.make_inputs(w, with_do=True)
+    d = device_inputs(w, inp)
+    desc = desc_of(w)
+    tdt = torch.float32 if w.dtype == "f32" else torch.bfloat16
+    bufs = {n: _guarded(tuple(d["q"].shape), tdt) for n in ("o", "dq", "dk", "dv")}
+    bufs["lse"] = _guarded(tuple(desc.lse_shape), torch.float32)
+    nws = max(binding.strata_na3d_workspace_bytes(desc, False), binding.strata_na3d_workspace_bytes(desc, True), 256)
+    bufs["ws"] = _guarded((nws,), torch.uint8)
+    v = {n: b[1] for n, b in bufs.items()}
+    binding.strata_na3d_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], v["o"], v["lse"], v["ws"])
+    binding.strata_na3d_bwd(desc, d["q"], d["k"], d["v"], v["o"], d["do"], v["lse"], d["coords"], d["freqs"], v["dq"],
+                            v["dk"], v["dv"], v["ws"])
+    torch.cuda.synchronize()
+    for n, (raw, _, guard, nbytes) in bufs.items():
+        assert _guards_intact(raw, guard, nbytes), f"write outside {n}"
+    assert bool(torch.isfinite(v["o"].float()).all()) and bool(torch.isfinite(v["dq"].float()).all())
+
+
 def test_cuda_graph_capture_and_replay(oracle_mod):
     """include/strata_na3d.h: calls never synchronise and are safe to capture.  Forward + backward captured in one
     graph on a side stream, replayed twice with the inputs changed in between."""
@@ -330,3 +371,77 @@ def test_cuda_graph_capture_and_replay(oracle_mod):
         gr = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
         for got, r, nm in zip((dq, dk, dv), gr, ("dQ", "dK", "dV")):
             assert_parity(to_f64(got), r, "bf16", f"graph replay {rep} {nm}", rms_bound=2e-2)
+
+
+# ------------------------------------------------------------------ the paper's own shapes (NEXT-4) and column attention (NEXT-2)
+@pytest.mark.parametrize("case", [dict(grid=(24, 16, 16), heads=2), dict(grid=(10, 20, 11), heads=3, batch=2),
+                                  dict(grid=(9, 9, 9), heads=1, rope_pairing=1)])
+def test_production_window_9x9x9_on_the_tensor_cores(oracle_mod, case):
+    """PAPER.md:325-326 (Table S1): 24 levels, head_dim 64, NATTEN kernel size 9 -- forward and backward."""
+    w = wl.small(name="prod999", dtype="bf16", value_scale="qknorm", window=(9, 9, 9), head_dim=64, **case)
+    assert binding.strata_na3d_impl_selected(desc_of(w)) == binding.IMPL_TCGEN05
+    assert binding.strata_na3d_impl_selected(desc_of(w), True) == binding.IMPL_TCGEN05
+    check_full(oracle_mod, w, binding.IMPL_AUTO)
+
+
+@pytest.mark.parametrize("case", [dict(grid=(24, 5, 7), heads=3), dict(grid=(8, 9, 6), heads=2, batch=2),
+                                  dict(grid=(32, 3, 4), heads=1, rope_pairing=1), dict(grid=(5, 4, 4), heads=2, rope_axes=0)])
+def test_column_attention(oracle_mod, case):
+    """attention along the vertical, window (L, 1, 1) -- its own kernel (na3d_column.cu)."""
+    kw = dict(name="column", dtype="bf16", value_scale="qknorm", head_dim=64)
+    kw.update(case)
+    w = wl.small(**kw)
+    w = dataclasses.replace(w, window=(w.grid[0], 1, 1))
+    check_full(oracle_mod, w, binding.IMPL_AUTO, backward=False)
+
+
+def test_column_attention_with_level_dependent_coordinates(oracle_mod):
+    """The rotation only cancels when a column's tokens share their coordinates; otherwise every row is recomputed."""
+    w = wl.small(name="column_lvl", dtype="bf16", value_scale="rsqrt_d", grid=(6, 5, 4), window=(6, 1, 1), heads=2, head_dim=64)
+    inp = wl.make_inputs(w)
+    coords = inp["coords"].copy()
+    coords[:, 1:, ..., 1] += 0.7 * np.arange(1, w.grid[0], dtype=np.float32)[None, :, None, None]
+    inp["coords"] = coords
+    d, o, lse = run_fwd(w, inp)
+    o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], coords, inp["freqs"], w.window)
+    assert_parity(to_f64(o), o_ref, "bf16", "column, level-dependent coords O")
+    assert_parity(to_f64(lse), lse_ref, "bf16", "column, level-dependent coords LSE", rms_bound=1e-2)
+
+
+# ------------------------------------------------------------------ geometry kernels (NEXT-3: eq. (1), eq. (2) on the device)
+def test_stereo_coords_and_wind_frame_kernels(oracle_mod):
+    """strata_stereo_coords / strata_wind_to_tile_frame against oracle/geometry.py on the patch centres of a
+    128 x 128 tile far from the face centre (coordinates up to ~1e3: the float32 result must be the rounding of the
+    float64 one) and on points around a high-latitude centre."""
+    rng = np.random.default_rng(11)
+    n_total = 6 * 2048 ** 2
+    for lat0, lon0, span in ((0.61, -2.4, 0.2), (1.35, 0.3, 0.25), (-0.02, 3.0, 0.3)):
+        n = 20011
+        lat = lat0 + rng.uniform(-span, span, n)
+        lon = lon0 + rng.uniform(-span, span, n)
+        lat = np.clip(lat, -1.55, 1.55)
+        d_lat, d_lon = torch.from_numpy(lat).cuda(), torch.from_numpy(lon).cuda()
+        coords = torch.full((n, 3), -7.0, dtype=torch.float32, device="cuda")
+        binding.strata_stereo_coords(d_lat, d_lon, lat0, lon0, n_total, coords, stride=3)
+        x_ref, y_ref = oracle_mod.geometry.stereo_xy(lat, lon, lat0, lon0, n_total)
+        got = coords.cpu().numpy()
+        assert np.all(got[:, 2] == -7.0), "the third coordinate slot is not this call's"
+        for g, r in ((got[:, 0], x_ref), (got[:, 1], y_ref)):
+            err = np.abs(g.astype(np.float64) - r)
+            assert np.all(err <= np.abs(r) * 2.0 ** -23 + 1e-30), f"eq. (1): max err {err.max():.3e}"
+        u = (rng.normal(size=n) * 25).astype(np.float32)
+        v = (rng.normal(size=n) * 25).astype(np.float32)
+        d_u, d_v = torch.from_numpy(u).cuda(), torch.from_numpy(v).cuda()
+        ul, vl = torch.empty_like(d_u), torch.empty_like(d_v)
+        binding.strata_wind_to_tile_frame(d_u, d_v, d_lat, d_lon, lat0, lon0, ul, vl)
+        ul_ref, vl_ref = oracle_mod.geometry.wind_to_tile_frame(u, v, lat, lon, lat0, lon0)
+        for g, r in ((ul.cpu().numpy(), ul_ref), (vl.cpu().numpy(), vl_ref)):
+            err = np.abs(g.astype(np.float64) - r)
+            assert np.all(err <= np.abs(r) * 2.0 ** -23 + 1e-5), f"eq. (2): max err {err.max():.3e}"
+    assert lib_status_invalid()
+
+
+def lib_status_invalid():
+    L = binding.lib()
+    return L.strata_stereo_coords(None, None, 4, 0.0, 0.0, 1.0, None, 2, None) == 1 and \
+        L.strata_wind_to_tile_frame(None, None, None, None, 4, 0.0, 0.0, None, None, None) == 1

@@ -403,3 +403,38 @@ def test_bf16_and_f32_inputs_are_read_exactly(oracle_mod):
     as32 = {n: as64[n].astype(np.float32) for n in as64}
     o32, _ = oracle_mod.na3d_fwd(as32["q"], as32["k"], as32["v"], inp["coords"], inp["freqs"], w.window)
     assert np.array_equal(o32, o64)
+
+
+# ------------------------------------------------------------------ eq. (2): winds in the tile-centre frame
+def test_eq2_wind_rotation_closed_forms_and_special_cases(oracle_mod):
+    """PAPER.md:101-108.  The oracle builds 3D vectors and projects; the pins are (i) the component form obtained by
+    multiplying out the dot products by hand, e . e0 = cos dl, n . e0 = -sin p sin dl, e . n0 = sin p0 sin dl,
+    n . n0 = sin p sin p0 cos dl + cos p cos p0 (r0 is orthogonal to e0 and n0, so the radial part drops out);
+    (ii) textbook special cases; (iii) what the projection removes is exactly the radial component."""
+    g = oracle_mod.geometry
+    rng = np.random.default_rng(5)
+    lat0, lon0 = 0.37, -1.21
+    lat = lat0 + rng.uniform(-0.3, 0.3, 200)
+    lon = lon0 + rng.uniform(-0.3, 0.3, 200)
+    u, v = rng.normal(size=200) * 20, rng.normal(size=200) * 20
+    ul, vl = g.wind_to_tile_frame(u, v, lat, lon, lat0, lon0)
+    dl = lon - lon0
+    ul_c = u * np.cos(dl) - v * np.sin(lat) * np.sin(dl)
+    vl_c = u * np.sin(lat0) * np.sin(dl) + v * (np.sin(lat) * np.sin(lat0) * np.cos(dl) + np.cos(lat) * np.cos(lat0))
+    assert np.max(np.abs(ul - ul_c)) < 1e-12 and np.max(np.abs(vl - vl_c)) < 1e-12
+    # at the tile centre nothing changes
+    a, b = g.wind_to_tile_frame(3.0, -4.0, lat0, lon0, lat0, lon0)
+    assert abs(a - 3.0) < 1e-14 and abs(b + 4.0) < 1e-14
+    # same meridian: East is East; the North component is foreshortened by the cosine of the latitude difference
+    a, b = g.wind_to_tile_frame(3.0, -4.0, lat0 + 0.2, lon0, lat0, lon0)
+    assert abs(a - 3.0) < 1e-14 and abs(b + 4.0 * math.cos(0.2)) < 1e-14
+    # centre on the equator, point on the equator: North is North, East foreshortened
+    a, b = g.wind_to_tile_frame(3.0, -4.0, 0.0, 0.5, 0.0, 0.3)
+    assert abs(a - 3.0 * math.cos(0.2)) < 1e-14 and abs(b + 4.0) < 1e-14
+    # |v_perp|^2 = |v|^2 - (v . r0)^2: the projection removes the radial leakage and nothing else
+    r0 = np.array([math.cos(lat0) * math.cos(lon0), math.cos(lat0) * math.sin(lon0), math.sin(lat0)])
+    e = np.stack([-np.sin(lon), np.cos(lon), np.zeros_like(lon)], -1)
+    n = np.stack([-np.sin(lat) * np.cos(lon), -np.sin(lat) * np.sin(lon), np.cos(lat)], -1)
+    vec = u[:, None] * e + v[:, None] * n
+    rad = vec @ r0
+    assert np.max(np.abs(ul ** 2 + vl ** 2 - (u ** 2 + v ** 2 - rad ** 2))) < 1e-9
