@@ -31,7 +31,14 @@ import numpy as np  # noqa: E402
 
 from paper_2606_31248_b200 import workloads as wl  # noqa: E402
 
-WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4}
+WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4,
+             # not BASELINE.json configs: the paper's own attention shapes (workloads.production), as extras
+             "prod16": "prod16", "prod32": "prod32", "col16": "col16", "col32": "col32"}
+
+
+def workload_of(key: str) -> wl.Workload:
+    idx = WORKLOADS[key]
+    return wl.config(idx) if isinstance(idx, int) else wl.production(idx)
 METRIC = "na3d_stereorope_useful_tflops"
 
 
@@ -357,9 +364,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--extras", default="cfg1,cfg2,cfg4", help="other configs summarised in the same line ('' = none)")
+    ap.add_argument("--extras", default="cfg1,cfg2,cfg4,prod32,col32", help="other configs summarised in the same line ('' = none)")
     args = ap.parse_args()
-    w = wl.config(WORKLOADS[args.workload])
+    w = workload_of(args.workload)
     if args.impl == "reference":
         run_reference(args, w)
         return
@@ -382,7 +389,7 @@ def main():
     if args.extras and world == 1:
         short = argparse.Namespace(**{**vars(args), "steps": max(3, min(args.steps, 10)), "e2e_steps": 1})
         for name in [x for x in args.extras.split(",") if x and x != args.workload]:
-            r = measure(wl.config(WORKLOADS[name]), short, None, rank, peaks, with_e2e=False, with_cpu=False)
+            r = measure(workload_of(name), short, None, rank, peaks, with_e2e=False, with_cpu=False)
             others[name] = {"ms_per_step": r["ms_per_step"], "tflops": r["tflops"], "tokens_per_s": r["tokens_per_s"],
                             "frac_of_roofline": r["roofline"]["step_frac_of_roofline"], "impl": r["impl"],
                             "kernels_ms": r["roofline"]["kernels_ms"]}
