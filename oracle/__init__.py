@@ -21,6 +21,7 @@ import numpy as np
 
 from . import build as _build
 from . import geometry  # noqa: F401
+from . import normgate as _normgate
 
 _LIB = None
 
@@ -149,3 +150,13 @@ def na3d_bwd_rows(q, k, v, d_o, coords, freqs, window, idx, scale=None, pairing:
                                _ptr(freqs), ctypes.c_longlong(idx.size), _ptr(idx),
                                _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]))
     return tuple(outs)
+
+
+def na3d_normgate_fwd(q, k, v, gate, coords, freqs, window, eps: float = 1e-6, scale=None, pairing: int = 0):
+    """QK-RMSNorm -> StereoRoPE + NA3D -> sigmoid head gate.  Returns (o, lse, a) (oracle/normgate.py)."""
+    return _normgate.fwd(na3d_fwd, q, k, v, gate, coords, freqs, window, eps, scale, pairing)
+
+
+def na3d_normgate_bwd(q, k, v, gate, d_o, coords, freqs, window, eps: float = 1e-6, scale=None, pairing: int = 0):
+    """Gradients of the above wrt q, k, v and the gate logits: (dq, dk, dv, dgate)."""
+    return _normgate.bwd(na3d_fwd, na3d_bwd, q, k, v, gate, d_o, coords, freqs, window, eps, scale, pairing)

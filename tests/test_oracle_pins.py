@@ -438,3 +438,74 @@ def test_eq2_wind_rotation_closed_forms_and_special_cases(oracle_mod):
     vec = u[:, None] * e + v[:, None] * n
     rad = vec @ r0
     assert np.max(np.abs(ul ** 2 + vl ** 2 - (u ** 2 + v ** 2 - rad ** 2))) < 1e-9
+
+
+# ------------------------------------------------------------------ QK-RMSNorm + sigmoid head gate
+def _ng_inputs(rng, grid=(3, 4, 5), H=2, D=8, A=2):
+    B = 1
+    shape = (B,) + grid + (H, D)
+    q, k, v = (rng.normal(size=shape) for _ in range(3))
+    gate = rng.normal(size=(B,) + grid + (H,))
+    coords = rng.normal(size=(B,) + grid + (A,)).astype(np.float32) * 3
+    freqs = rng.uniform(0.1, 1.0, size=(A, D // 2)).astype(np.float32)
+    return q, k, v, gate, coords, freqs
+
+
+def test_normgate_forward_properties(oracle_mod):
+    rng = np.random.default_rng(21)
+    q, k, v, gate, coords, freqs = _ng_inputs(rng)
+    window = (3, 3, 3)
+    o, lse, a = oracle_mod.na3d_normgate_fwd(q, k, v, gate, coords, freqs, window, eps=0.0)
+    # (i) what reaches the attention has RMS 1 per (token, head) vector: same result from explicitly normalised inputs
+    qn = q / np.sqrt(np.mean(q ** 2, -1, keepdims=True))
+    kn = k / np.sqrt(np.mean(k ** 2, -1, keepdims=True))
+    assert np.allclose(np.sqrt(np.mean(qn ** 2, -1)), 1.0, atol=1e-14)
+    a2, lse2 = oracle_mod.na3d_fwd(qn, kn, v, coords, freqs, window)
+    assert np.max(np.abs(a - a2)) < 1e-13 and np.max(np.abs(lse - lse2)) < 1e-13
+    # (ii) RMSNorm without a learnable scale forgets the length of q and k (eps = 0): positive per-row factors change nothing
+    fq = rng.uniform(0.2, 5.0, size=q.shape[:-1] + (1,))
+    fk = rng.uniform(0.2, 5.0, size=k.shape[:-1] + (1,))
+    o3, lse3, _ = oracle_mod.na3d_normgate_fwd(q * fq, k * fk, v, gate, coords, freqs, window, eps=0.0)
+    assert np.max(np.abs(o - o3)) < 1e-12 and np.max(np.abs(lse - lse3)) < 1e-12
+    # (iii) |logit| <= scale * d after the normalisation (what it is for: "bounding the logit magnitude")
+    assert np.max(np.abs(lse)) <= (1.0 / math.sqrt(8)) * 8 + math.log(27) + 1e-9
+    # (iv) the gate: one factor per (token, head), sigmoid(0) = 1/2, sigmoid(+40) = 1, no gate = a
+    assert np.max(np.abs(o - a / (1.0 + np.exp(-gate))[..., None])) < 1e-14
+    o0, _, _ = oracle_mod.na3d_normgate_fwd(q, k, v, np.zeros_like(gate), coords, freqs, window, eps=0.0)
+    assert np.max(np.abs(o0 - 0.5 * a)) < 1e-14
+    o1, _, _ = oracle_mod.na3d_normgate_fwd(q, k, v, np.full_like(gate, 40.0), coords, freqs, window, eps=0.0)
+    on, _, _ = oracle_mod.na3d_normgate_fwd(q, k, v, None, coords, freqs, window, eps=0.0)
+    assert np.max(np.abs(o1 - a)) < 1e-12 and np.max(np.abs(on - a)) == 0.0
+    # (v) eps: the denominator is sqrt(mean x^2 + eps) -- a single vector by hand
+    x = np.array([[[[[[3.0, 4.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0]]]]]])
+    from oracle import normgate
+    assert np.allclose(normgate.rmsnorm(x, 0.875)[0, 0, 0, 0, 0, :2], np.array([3.0, 4.0]) / 2.0, atol=1e-15)   # mean = 25/8, + 7/8 = 4
+
+
+def test_normgate_backward_vs_finite_differences(oracle_mod):
+    rng = np.random.default_rng(22)
+    q, k, v, gate, coords, freqs = _ng_inputs(rng, grid=(3, 3, 4), H=1, D=4)
+    window = (3, 3, 3)
+    eps = 1e-3
+    d_o = rng.normal(size=q.shape)
+    dq, dk, dv, dg = oracle_mod.na3d_normgate_bwd(q, k, v, gate, d_o, coords, freqs, window, eps=eps)
+
+    def loss(q_, k_, v_, g_):
+        o, _, _ = oracle_mod.na3d_normgate_fwd(q_, k_, v_, g_, coords, freqs, window, eps=eps)
+        return float(np.sum(o * d_o))
+
+    h = 1e-6
+    for name, x, g in (("q", q, dq), ("k", k, dk), ("v", v, dv), ("gate", gate, dg)):
+        flat = x.reshape(-1)
+        for idx in rng.choice(flat.size, size=12, replace=False):
+            old = flat[idx]
+            flat[idx] = old + h
+            lp = loss(q, k, v, gate)
+            flat[idx] = old - h
+            lm = loss(q, k, v, gate)
+            flat[idx] = old
+            fd = (lp - lm) / (2 * h)
+            assert abs(fd - g.reshape(-1)[idx]) <= 1e-6 * max(1.0, abs(fd)), (name, idx, fd, g.reshape(-1)[idx])
+    # with eps = 0 the output does not depend on |q|: the gradient is orthogonal to q, row by row
+    dq0, dk0, _, _ = oracle_mod.na3d_normgate_bwd(q, k, v, gate, d_o, coords, freqs, window, eps=0.0)
+    assert np.max(np.abs(np.sum(dq0 * q, -1))) < 1e-12 and np.max(np.abs(np.sum(dk0 * k, -1))) < 1e-12
