@@ -110,6 +110,29 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc,
                                 void* dq, void* dk, void* dv,
                                 void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- QK-RMSNorm and the sigmoid head gate around the attention (App. B.5) -------------------------
+ * "QK RMSNorm, which applies RMSNorm (without learnable scale) to the query and key vectors before their dot
+ * product" and "gated attention, which applies a head-specific sigmoid gate to the attention output":
+ *   q^ = q / sqrt(mean_c q_c^2 + eps)  (per (token, head) vector; same for k),   a, lse = NA3D(RoPE(q^), RoPE(k^), v),
+ *   o = sigmoid(gate[b, l, y, x, h]) * a.
+ * gate: float32 logits [B, L, Y, X, H] (DEVICE), NULL = no gate.  eps >= 0.  lse is that of the normalised logits.
+ * The backward takes the GATED output o of the forward and the gradient d_o wrt it; writes dq, dk, dv and, with a
+ * gate, dgate [B, L, Y, X, H] float32.  Workspace: strata_na3d_normgate_workspace_bytes (device memory).
+ * In this version the normalisation and the gate run as streaming kernels around strata_na3d_fwd / _bwd (one extra
+ * read + write of Q and K, one of O); everything else (layouts, asynchrony, errors) as for those calls. */
+size_t strata_na3d_normgate_workspace_bytes(const strata_na3d_desc_t* desc, int backward);
+strata_status_t strata_na3d_normgate_fwd(const strata_na3d_desc_t* desc,
+                                         const void* q, const void* k, const void* v,
+                                         const float* coords, const float* freqs, const float* gate, float eps,
+                                         void* o, float* lse,
+                                         void* workspace, size_t workspace_bytes, void* stream);
+strata_status_t strata_na3d_normgate_bwd(const strata_na3d_desc_t* desc,
+                                         const void* q, const void* k, const void* v,
+                                         const void* o, const void* d_o, const float* lse,
+                                         const float* coords, const float* freqs, const float* gate, float eps,
+                                         void* dq, void* dk, void* dv, float* dgate,
+                                         void* workspace, size_t workspace_bytes, void* stream);
+
 /* Same operations on HOST buffers; `workspace` is DEVICE memory of at least
  * strata_na3d_host_workspace_bytes().  Asynchronous on `stream`. */
 strata_status_t strata_na3d_fwd_host(const strata_na3d_desc_t* desc,

@@ -23,6 +23,7 @@ IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_TILE = 0, 1, 2, 3
 
 EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
            "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",
+           "strata_na3d_normgate_workspace_bytes", "strata_na3d_normgate_fwd", "strata_na3d_normgate_bwd",
            "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
            "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_stereo_coords",
            "strata_wind_to_tile_frame", "strata_status_string", "strata_version")
@@ -98,6 +99,12 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, name)
             f.restype = i32
             f.argtypes = [dp] + [vp] * 12 + [sz, vp]
+        L.strata_na3d_normgate_workspace_bytes.restype = sz
+        L.strata_na3d_normgate_workspace_bytes.argtypes = [dp, i32]
+        L.strata_na3d_normgate_fwd.restype = i32
+        L.strata_na3d_normgate_fwd.argtypes = [dp] + [vp] * 6 + [ctypes.c_float] + [vp] * 3 + [sz, vp]
+        L.strata_na3d_normgate_bwd.restype = i32
+        L.strata_na3d_normgate_bwd.argtypes = [dp] + [vp] * 9 + [ctypes.c_float] + [vp] * 5 + [sz, vp]
         L.strata_na3d_last_launch_count.restype = i32
         L.strata_na3d_set_profiling.restype = None
         L.strata_na3d_set_profiling.argtypes = [i32]
@@ -215,6 +222,27 @@ def strata_na3d_fwd(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None
 def strata_na3d_bwd(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None):
     _check(strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream),
            "strata_na3d_bwd")
+
+
+def strata_na3d_normgate_workspace_bytes(desc, backward: bool) -> int:
+    return int(lib().strata_na3d_normgate_workspace_bytes(ctypes.byref(desc.c()), 1 if backward else 0))
+
+
+def strata_na3d_normgate_fwd(desc, q, k, v, coords, freqs, gate, eps, o, lse, workspace, stream=None):
+    """QK-RMSNorm -> StereoRoPE + NA3D -> sigmoid head gate (gate: float32 [B,L,Y,X,H] logits or None)."""
+    ws_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    _check(int(lib().strata_na3d_normgate_fwd(ctypes.byref(desc.c()), _ptr(q), _ptr(k), _ptr(v), _ptr(coords), _ptr(freqs),
+                                              _ptr(gate), float(eps), _ptr(o), _ptr(lse), _ptr(workspace), ws_bytes,
+                                              _stream_handle(stream))), "strata_na3d_normgate_fwd")
+
+
+def strata_na3d_normgate_bwd(desc, q, k, v, o, d_o, lse, coords, freqs, gate, eps, dq, dk, dv, dgate, workspace,
+                             stream=None):
+    ws_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    _check(int(lib().strata_na3d_normgate_bwd(ctypes.byref(desc.c()), _ptr(q), _ptr(k), _ptr(v), _ptr(o), _ptr(d_o),
+                                              _ptr(lse), _ptr(coords), _ptr(freqs), _ptr(gate), float(eps), _ptr(dq),
+                                              _ptr(dk), _ptr(dv), _ptr(dgate), _ptr(workspace), ws_bytes,
+                                              _stream_handle(stream))), "strata_na3d_normgate_bwd")
 
 
 def strata_na3d_fwd_host(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None):

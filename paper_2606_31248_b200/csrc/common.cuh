@@ -74,16 +74,25 @@ cudaError_t launch_fwd_column(const Problem& p, const void* q, const void* k, co
 // na3d_simt.cu: fp32 CUDA-core kernels on pre-rotated fp32 operands (qr, kr in workspace).
 cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
                             void* o, float* lse, cudaStream_t stream, int* launches);
+// (d_o_main: the upstream gradient the main kernels use; d_o only enters B1 with o -- they differ for the gated
+// attention of PAPER.md:390, where D_i = sum_c dO_c o_c with the gated output and the raw gradient)
 cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
-                            const void* o, const void* d_o, const float* lse, float* delta,
+                            const void* o, const void* d_o, const void* d_o_main, const float* lse, float* delta,
                             float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches);
 
 // na3d_bwd_tc.cu: tcgen05 backward on pre-rotated bf16 operands (head_dim 64).  stat is [B, H, N] float2
 // scratch; rtab the fp32 rotary table (nullptr: no rotation): the epilogues apply B4 and write bf16 dq, dk.
 bool tc_bwd_supported(const Problem& p);
 cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
-                          const void* d_o, const float* lse, void* stat, const void* rtab, void* dq, void* dk,
-                          void* dv, cudaStream_t stream, int* launches);
+                          const void* d_o, const void* d_o_main, const float* lse, void* stat, const void* rtab, void* dq,
+                          void* dk, void* dv, cudaStream_t stream, int* launches);
+
+// normgate.cu: the elementwise steps of QK-RMSNorm and the sigmoid head gate, rows in memory order.
+cudaError_t launch_rmsnorm_rows(const Problem& p, const void* x, void* y, float eps, cudaStream_t st, int* launches);
+cudaError_t launch_gate_rows(const Problem& p, const void* x, void* y, const float* gate, cudaStream_t st, int* launches);
+cudaError_t launch_rmsnorm_bwd_rows(const Problem& p, const void* x, void* dx, float eps, cudaStream_t st, int* launches);
+cudaError_t launch_dgate_rows(const Problem& p, const void* d_o, const void* o, const float* gate, float* dgate,
+                              cudaStream_t st, int* launches);
 
 // na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands.
 bool tc_fwd_supported(const Problem& p);

@@ -62,8 +62,8 @@ bool tc_bwd_supported(const Problem& p) {
 
 // B1 (+ lse in the exp2 domain) -> stat, then the two persistent kernels of na3d_bwd_tc2.cu.
 cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, const void* o,
-                          const void* d_o, const float* lse, void* stat, const void* rtab, void* dq, void* dk,
-                          void* dv, cudaStream_t stream, int* launches) {
+                          const void* d_o, const void* d_o_main, const float* lse, void* stat, const void* rtab, void* dq,
+                          void* dk, void* dv, cudaStream_t stream, int* launches) {
   if (!tc_bwd_supported(p)) return cudaErrorNotSupported;
   const long long rows = p.rows(), sgrid = (rows * 8 + 255) / 256;
   if (sgrid > 0x7fffffffLL) return cudaErrorInvalidValue;
@@ -73,7 +73,7 @@ cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, cons
   if (launches) *launches += 1;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  return launch_bwd_tc2_main(p, qr, kr, v, d_o, (float2*)stat, rtab, dq, dk, dv, stream, launches);
+  return launch_bwd_tc2_main(p, qr, kr, v, d_o_main, (float2*)stat, rtab, dq, dk, dv, stream, launches);
 }
 
 }  // namespace strata

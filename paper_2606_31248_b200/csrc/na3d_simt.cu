@@ -266,7 +266,7 @@ cudaError_t fwd_t(const Problem& p, const float* qr, const float* kr, const void
 
 template <int D, typename TV>
 cudaError_t bwd_t(const Problem& p, const float* qr, const float* kr, const void* v, const void* o,
-                  const void* d_o, const float* lse, float* delta, float* dqr, float* dkr, void* dv,
+                  const void* d_o, const void* d_o_main, const float* lse, float* delta, float* dqr, float* dkr, void* dv,
                   cudaStream_t st, int* launches) {
   const long long rows_per_block = kBlock / (D / 32);
   const long long grid = (p.rows() + rows_per_block - 1) / rows_per_block;
@@ -275,10 +275,10 @@ cudaError_t bwd_t(const Problem& p, const float* qr, const float* kr, const void
   na3d_delta_kernel<D, TV><<<(unsigned)grid, kBlock, 0, st>>>((const TV*)o, (const TV*)d_o, delta, p);
   prof_end(st);
   prof_begin("na3d_dq_simt", st);
-  na3d_dq_simt_kernel<D, TV><<<(unsigned)grid, kBlock, 0, st>>>(qr, kr, (const TV*)v, (const TV*)d_o, lse, delta, dqr, p);
+  na3d_dq_simt_kernel<D, TV><<<(unsigned)grid, kBlock, 0, st>>>(qr, kr, (const TV*)v, (const TV*)d_o_main, lse, delta, dqr, p);
   prof_end(st);
   prof_begin("na3d_dkdv_simt", st);
-  na3d_dkdv_simt_kernel<D, TV><<<(unsigned)grid, kBlock, 0, st>>>(qr, kr, (const TV*)v, (const TV*)d_o, lse, delta, dkr, (TV*)dv, p);
+  na3d_dkdv_simt_kernel<D, TV><<<(unsigned)grid, kBlock, 0, st>>>(qr, kr, (const TV*)v, (const TV*)d_o_main, lse, delta, dkr, (TV*)dv, p);
   prof_end(st);
   if (launches) *launches += 3;
   return cudaGetLastError();
@@ -306,9 +306,9 @@ cudaError_t launch_fwd_simt(const Problem& p, const float* qr, const float* kr, 
 }
 
 cudaError_t launch_bwd_simt(const Problem& p, const float* qr, const float* kr, const void* v,
-                            const void* o, const void* d_o, const float* lse, float* delta,
+                            const void* o, const void* d_o, const void* d_o_main, const float* lse, float* delta,
                             float* dqr, float* dkr, void* dv, cudaStream_t stream, int* launches) {
-  STRATA_DISPATCH(bwd_t, p, qr, kr, v, o, d_o, lse, delta, dqr, dkr, dv, stream, launches);
+  STRATA_DISPATCH(bwd_t, p, qr, kr, v, o, d_o, d_o_main, lse, delta, dqr, dkr, dv, stream, launches);
 }
 
 }  // namespace strata

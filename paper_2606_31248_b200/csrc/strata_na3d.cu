@@ -200,8 +200,8 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
   return STRATA_OK;
 }
 
-strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, const void* k,
-                                const void* v, const void* o, const void* d_o, const float* lse,
+static strata_status_t bwd_impl(const strata_na3d_desc_t* desc, const void* q, const void* k,
+                                const void* v, const void* o, const void* d_o, const void* d_o_main, const float* lse,
                                 const float* coords, const float* freqs, void* dq, void* dk,
                                 void* dv, void* workspace, size_t workspace_bytes, void* stream) {
   Problem p; strata_status_t why;
@@ -231,7 +231,7 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, c
       e = strata::launch_rope_table_f32(p, rtab, coords, freqs, st, &launches);
       if (e != cudaSuccess) return cuda_status(e);
     }
-    e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, lse, stat, p.A > 0 ? rtab : nullptr, dq, dk, dv, st, &launches);
+    e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, d_o_main, lse, stat, p.A > 0 ? rtab : nullptr, dq, dk, dv, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
     g_last_launches = launches;
     return STRATA_OK;
@@ -243,10 +243,90 @@ strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, c
   float* delta = ws.take<float>(stat_bytes(p));
   e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 0, coords, freqs, 1.f, st, &launches);
   if (e != cudaSuccess) return cuda_status(e);
-  e = strata::launch_bwd_simt(p, qr, kr, v, o, d_o, lse, delta, dqr, dkr, dv, st, &launches);
+  e = strata::launch_bwd_simt(p, qr, kr, v, o, d_o, d_o_main, lse, delta, dqr, dkr, dv, st, &launches);
   if (e != cudaSuccess) return cuda_status(e);
   // B4: dq = R(-phi) dqrot, dk = R(-phi) dkrot, rounded to the tensor dtype
   e = strata::launch_rope_rotate(p, dqr, dkr, 0, dq, dk, p.dtype, coords, freqs, -1.f, st, &launches);
+  if (e != cudaSuccess) return cuda_status(e);
+  g_last_launches = launches;
+  return STRATA_OK;
+}
+
+strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc, const void* q, const void* k,
+                                const void* v, const void* o, const void* d_o, const float* lse,
+                                const float* coords, const float* freqs, void* dq, void* dk,
+                                void* dv, void* workspace, size_t workspace_bytes, void* stream) {
+  return bwd_impl(desc, q, k, v, o, d_o, d_o, lse, coords, freqs, dq, dk, dv, workspace, workspace_bytes, stream);
+}
+
+// ---- QK-RMSNorm + sigmoid head gate around the attention --------------------------------------------
+size_t strata_na3d_normgate_workspace_bytes(const strata_na3d_desc_t* desc, int backward) {
+  Problem p; strata_status_t why;
+  if (!make_problem(desc, &p, &why)) return 0;
+  const Path path = select_path(desc, p, backward != 0);
+  if (path == PATH_NONE) return 0;
+  return (backward ? 3 : 2) * align_up(tensor_bytes(p)) + ws_bytes(p, path, backward != 0);
+}
+
+strata_status_t strata_na3d_normgate_fwd(const strata_na3d_desc_t* desc, const void* q, const void* k, const void* v,
+                                         const float* coords, const float* freqs, const float* gate, float eps,
+                                         void* o, float* lse, void* workspace, size_t workspace_bytes, void* stream) {
+  Problem p; strata_status_t why;
+  if (!make_problem(desc, &p, &why)) return why;
+  if (!q || !k || !o || !(eps >= 0.f)) return STRATA_ERR_INVALID_ARG;
+  if (misaligned(q) || misaligned(k) || misaligned(gate) || misaligned(workspace)) return STRATA_ERR_INVALID_ARG;
+  const size_t need = strata_na3d_normgate_workspace_bytes(desc, 0);
+  if (need == 0) return STRATA_ERR_UNSUPPORTED;
+  if (!workspace || workspace_bytes < need) return STRATA_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  Carve ws{reinterpret_cast<char*>(workspace), 0};
+  void* qn = ws.take<char>(tensor_bytes(p));
+  void* kn = ws.take<char>(tensor_bytes(p));
+  int launches = 0;
+  cudaError_t e = strata::launch_rmsnorm_rows(p, q, qn, eps, st, &launches);
+  if (e == cudaSuccess) e = strata::launch_rmsnorm_rows(p, k, kn, eps, st, &launches);
+  if (e != cudaSuccess) return cuda_status(e);
+  strata_status_t s = strata_na3d_fwd(desc, qn, kn, v, coords, freqs, o, lse, ws.base + ws.off, workspace_bytes - ws.off, stream);
+  if (s != STRATA_OK) return s;
+  launches += g_last_launches;
+  if (gate) {
+    e = strata::launch_gate_rows(p, o, o, gate, st, &launches);
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  g_last_launches = launches;
+  return STRATA_OK;
+}
+
+strata_status_t strata_na3d_normgate_bwd(const strata_na3d_desc_t* desc, const void* q, const void* k, const void* v,
+                                         const void* o, const void* d_o, const float* lse, const float* coords,
+                                         const float* freqs, const float* gate, float eps, void* dq, void* dk, void* dv,
+                                         float* dgate, void* workspace, size_t workspace_bytes, void* stream) {
+  Problem p; strata_status_t why;
+  if (!make_problem(desc, &p, &why)) return why;
+  if (!q || !k || !o || !d_o || !dq || !dk || !(eps >= 0.f) || (gate && !dgate)) return STRATA_ERR_INVALID_ARG;
+  if (misaligned(q) || misaligned(k) || misaligned(gate) || misaligned(dgate) || misaligned(workspace))
+    return STRATA_ERR_INVALID_ARG;
+  const size_t need = strata_na3d_normgate_workspace_bytes(desc, 1);
+  if (need == 0) return STRATA_ERR_UNSUPPORTED;
+  if (!workspace || workspace_bytes < need) return STRATA_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  Carve ws{reinterpret_cast<char*>(workspace), 0};
+  void* qn = ws.take<char>(tensor_bytes(p));
+  void* kn = ws.take<char>(tensor_bytes(p));
+  void* da = ws.take<char>(tensor_bytes(p));
+  int launches = 0;
+  cudaError_t e = strata::launch_rmsnorm_rows(p, q, qn, eps, st, &launches);
+  if (e == cudaSuccess) e = strata::launch_rmsnorm_rows(p, k, kn, eps, st, &launches);
+  // o = s a: the attention sees da = s dO, and B1's D_i = sum_c da_c a_c = sum_c dO_c o_c (raw gradient, gated output)
+  if (e == cudaSuccess && gate) e = strata::launch_gate_rows(p, d_o, da, gate, st, &launches);
+  if (e == cudaSuccess && gate) e = strata::launch_dgate_rows(p, d_o, o, gate, dgate, st, &launches);
+  if (e != cudaSuccess) return cuda_status(e);
+  strata_status_t s = bwd_impl(desc, qn, kn, v, o, d_o, gate ? da : d_o, lse, coords, freqs, dq, dk, dv, ws.base + ws.off,
+                               workspace_bytes - ws.off, stream);
+  if (s != STRATA_OK) return s;
+  launches += g_last_launches;
+  e = strata::launch_rmsnorm_bwd_rows(p, q, dq, eps, st, &launches);      // dq^, dk^ -> dq, dk (in place)
+  if (e == cudaSuccess) e = strata::launch_rmsnorm_bwd_rows(p, k, dk, eps, st, &launches);
   if (e != cudaSuccess) return cuda_status(e);
   g_last_launches = launches;
   return STRATA_OK;

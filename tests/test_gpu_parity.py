@@ -408,6 +408,55 @@ def test_column_attention_with_level_dependent_coordinates(oracle_mod):
     assert_parity(to_f64(lse), lse_ref, "bf16", "column, level-dependent coords LSE", rms_bound=1e-2)
 
 
+# ------------------------------------------------------------------ QK-RMSNorm + sigmoid head gate (NEXT-1)
+@pytest.mark.parametrize("case", [dict(dtype="bf16", grid=(8, 18, 21), window=(3, 7, 7), heads=2, head_dim=64),          # fused fwd, tcgen05 bwd
+                                  dict(dtype="bf16", grid=(6, 10, 9), window=(5, 9, 9), heads=1, head_dim=128),         # tile fwd, SIMT bwd
+                                  dict(dtype="f32", grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32),
+                                  dict(dtype="bf16", grid=(5, 9, 12), window=(3, 5, 5), heads=3, head_dim=64, gate=False)])
+def test_qk_rmsnorm_and_head_gate(oracle_mod, case):
+    kw = dict(case)
+    with_gate = kw.pop("gate", True)
+    w = wl.small(name="normgate", value_scale="unit", **kw)
+    inp = wl.make_inputs(w, with_do=True)
+    rng = np.random.default_rng(w.seed + 3)
+    # un-normalised inputs of very different lengths per row: the kernel must do the normalising
+    fac = rng.uniform(0.25, 4.0, size=inp["q"].shape[:-1] + (1,)).astype(np.float32)
+    if w.dtype == "bf16":
+        q32 = wl.bf16_bits_to_f32(inp["q"]) * fac
+        inp["q"] = wl.f32_to_bf16_bits(q32)
+    else:
+        inp["q"] = (inp["q"] * fac).astype(np.float32)
+    gate_np = (rng.normal(size=(w.batch,) + w.grid + (w.heads,)) * 2).astype(np.float32) if with_gate else None
+    eps = 1e-5
+    d = device_inputs(w, inp)
+    desc = desc_of(w)
+    gate = torch.from_numpy(gate_np).cuda() if with_gate else None
+    o = torch.empty_like(d["q"])
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
+    ws = binding.alloc_workspace(max(binding.strata_na3d_normgate_workspace_bytes(desc, False),
+                                     binding.strata_na3d_normgate_workspace_bytes(desc, True)), "cuda")
+    binding.strata_na3d_normgate_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], gate, eps, o, lse, ws)
+    dq, dk, dv = (torch.empty_like(d["q"]) for _ in range(3))
+    dgate = torch.empty_like(gate) if with_gate else None
+    binding.strata_na3d_normgate_bwd(desc, d["q"], d["k"], d["v"], o, d["do"], lse, d["coords"], d["freqs"], gate, eps,
+                                     dq, dk, dv, dgate, ws)
+    torch.cuda.synchronize()
+    o_ref, lse_ref, _ = oracle_mod.na3d_normgate_fwd(inp["q"], inp["k"], inp["v"], gate_np, inp["coords"], inp["freqs"],
+                                                     w.window, eps=eps)
+    assert_parity(to_f64(o), o_ref, w.dtype, "normgate O")
+    assert_parity(to_f64(lse), lse_ref, "f32" if w.dtype == "f32" else "bf16", "normgate LSE", rms_bound=1e-2)
+    rq, rk, rv, rg = oracle_mod.na3d_normgate_bwd(inp["q"], inp["k"], inp["v"], gate_np, inp["do"], inp["coords"],
+                                                  inp["freqs"], w.window, eps=eps)
+    rb = None if w.dtype == "f32" else 2e-2
+    # dq = r (dq^ - ...): the per-row factor r = 1 / rms(q) (x 0.25 .. 4 here) scales the gradient and with it the
+    # error of the attention backward; the tolerances are held on dq / r, i.e. at the scale of the un-scaled rows
+    assert_parity(to_f64(dq) * fac.astype(np.float64), rq * fac, w.dtype, "normgate dQ (per unit of 1 / rms scale)", rms_bound=rb)
+    assert_parity(to_f64(dk), rk, w.dtype, "normgate dK", rms_bound=rb)
+    assert_parity(to_f64(dv), rv, w.dtype, "normgate dV", rms_bound=rb)
+    if with_gate:
+        assert_parity(to_f64(dgate), rg, w.dtype, "normgate dgate", rms_bound=rb)
+
+
 # ------------------------------------------------------------------ geometry kernels (NEXT-3: eq. (1), eq. (2) on the device)
 def test_stereo_coords_and_wind_frame_kernels(oracle_mod):
     """strata_stereo_coords / strata_wind_to_tile_frame against oracle/geometry.py on the patch centres of a
