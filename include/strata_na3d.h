@@ -134,7 +134,12 @@ strata_status_t strata_na3d_normgate_bwd(const strata_na3d_desc_t* desc,
                                          void* workspace, size_t workspace_bytes, void* stream);
 
 /* Same operations on HOST buffers; `workspace` is DEVICE memory of at least
- * strata_na3d_host_workspace_bytes().  Asynchronous on `stream`. */
+ * strata_na3d_host_workspace_bytes() (two staging slots of ONE sample each + the device scratch of a one-sample
+ * call).  The samples of the batch are independent: they go through one at a time, the copies in of
+ * sample b + 1 and the copies out of sample b - 1 overlapping the kernels of sample b on two internal streams that
+ * are joined back into `stream` before the call returns.  Asynchronous and ordered on `stream`; the host buffers
+ * should be page-locked (pageable memory makes the copies synchronous) and must stay valid until the work on `stream`
+ * has completed. */
 strata_status_t strata_na3d_fwd_host(const strata_na3d_desc_t* desc,
                                      const void* q, const void* k, const void* v,
                                      const float* coords, const float* freqs,

@@ -100,6 +100,57 @@ size_t stat_bytes(const Problem& p) { return (size_t)p.B * p.H * p.N * 4; }
 size_t coords_bytes(const Problem& p) { return (size_t)p.B * p.N * p.A * 4; }
 size_t freqs_bytes(const Problem& p) { return (size_t)p.A * (p.D / 2) * 4; }
 
+
+// ---- host entry points: two staging slots of ONE sample each; copies in, kernels and copies out of consecutive
+// samples overlap on three streams (the caller's stream runs the kernels; two internal streams carry the copies and
+// are joined back into it before the call returns, so the call stays asynchronous and ordered on `stream`).
+struct HostLayout {
+  size_t tensor, stat, coords, freqs, slot, inner, total;          // bytes (aligned) of the per-sample pieces
+};
+HostLayout host_layout(const Problem& p1, Path path, bool backward) {
+  HostLayout h;
+  h.tensor = align_up(tensor_bytes(p1)); h.stat = align_up(stat_bytes(p1));
+  h.coords = align_up(coords_bytes(p1)); h.freqs = align_up(freqs_bytes(p1));
+  h.slot = (backward ? 8 : 4) * h.tensor + h.stat + h.coords;
+  h.inner = align_up(ws_bytes(p1, path, backward));
+  h.total = 2 * h.slot + h.freqs + h.inner;
+  return h;
+}
+struct HostPipe {
+  int dev = -1;
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t entry = nullptr, in_ready[2] = {}, compute_done[2] = {}, out_done[2] = {};
+};
+HostPipe* host_pipe() {
+  thread_local HostPipe pipes[8];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+  HostPipe* hp = nullptr;
+  for (HostPipe& c : pipes) if (c.dev == dev) { hp = &c; break; }
+  if (!hp) {
+    for (HostPipe& c : pipes) if (c.dev < 0) { hp = &c; break; }
+    if (!hp) return nullptr;
+    bool ok = cudaStreamCreateWithFlags(&hp->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&hp->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&hp->entry, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i)
+      ok = cudaEventCreateWithFlags(&hp->in_ready[i], cudaEventDisableTiming) == cudaSuccess &&
+           cudaEventCreateWithFlags(&hp->compute_done[i], cudaEventDisableTiming) == cudaSuccess &&
+           cudaEventCreateWithFlags(&hp->out_done[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { (void)cudaGetLastError(); return nullptr; }
+    hp->dev = dev;
+  }
+  return hp;
+}
+#define STRATA_CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_status(e_); } while (0)
+
+// One pass of the per-sample pipeline.  n_in / n_out: tensors of the sample copied in / out (q, k, v[, o, d_o] /
+// o | dq, dk, dv); lse goes in (backward) or out (forward).
+strata_status_t host_pipeline(const strata_na3d_desc_t* desc, bool backward, const void* const* h_in, int n_in,
+                              void* const* h_out, int n_out, const float* h_lse_in, float* h_lse_out,
+                              const float* h_coords, const float* h_freqs, void* workspace, size_t workspace_bytes,
+                              cudaStream_t st);
+
 }  // namespace
 
 namespace strata {
@@ -144,12 +195,13 @@ size_t strata_na3d_workspace_bytes(const strata_na3d_desc_t* desc, int backward)
 size_t strata_na3d_host_workspace_bytes(const strata_na3d_desc_t* desc, int backward) {
   Problem p; strata_status_t why;
   if (!make_problem(desc, &p, &why)) return 0;
-  const Path path = select_path(desc, p, backward != 0);
+  strata_na3d_desc_t d1 = *desc;
+  d1.batch = 1;                                                     // the host entry points work one sample at a time
+  Problem p1;
+  if (!make_problem(&d1, &p1, &why)) return 0;
+  const Path path = select_path(&d1, p1, backward != 0);
   if (path == PATH_NONE) return 0;
-  const size_t t = align_up(tensor_bytes(p)), s = align_up(stat_bytes(p));
-  const size_t geo = align_up(coords_bytes(p)) + align_up(freqs_bytes(p));
-  const size_t staged = backward ? 8 * t + s + geo : 4 * t + s + geo;
-  return staged + ws_bytes(p, path, backward != 0);
+  return host_layout(p1, path, backward != 0).total;
 }
 
 int strata_na3d_impl_selected(const strata_na3d_desc_t* desc, int backward) {
@@ -336,35 +388,11 @@ strata_status_t strata_na3d_fwd_host(const strata_na3d_desc_t* desc, const void*
                                      const void* v, const float* coords, const float* freqs,
                                      void* o, float* lse, void* workspace, size_t workspace_bytes,
                                      void* stream) {
-  Problem p; strata_status_t why;
-  if (!make_problem(desc, &p, &why)) return why;
   if (!q || !k || !v || !o || !lse) return STRATA_ERR_INVALID_ARG;
-  if (p.A > 0 && (!coords || !freqs)) return STRATA_ERR_INVALID_ARG;
-  const size_t need = strata_na3d_host_workspace_bytes(desc, 0);
-  if (need == 0) return STRATA_ERR_UNSUPPORTED;
-  if (!workspace || workspace_bytes < need) return STRATA_ERR_WORKSPACE;
-  if (misaligned(workspace)) return STRATA_ERR_INVALID_ARG;
-  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  Carve ws{reinterpret_cast<char*>(workspace), 0};
-  const size_t tb = tensor_bytes(p), sb = stat_bytes(p), cb = coords_bytes(p), fb = freqs_bytes(p);
-  void* dq_ = ws.take<char>(tb); void* dk_ = ws.take<char>(tb); void* dv_ = ws.take<char>(tb);
-  void* do_ = ws.take<char>(tb);
-  float* dlse = ws.take<float>(sb);
-  float* dco = ws.take<float>(cb); float* dfr = ws.take<float>(fb);
-  cudaError_t e;
-  if ((e = cudaMemcpyAsync(dq_, q, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  if ((e = cudaMemcpyAsync(dk_, k, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  if ((e = cudaMemcpyAsync(dv_, v, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  if (p.A > 0) {
-    if ((e = cudaMemcpyAsync(dco, coords, cb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-    if ((e = cudaMemcpyAsync(dfr, freqs, fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  }
-  strata_status_t s = strata_na3d_fwd(desc, dq_, dk_, dv_, dco, dfr, do_, dlse, ws.base + ws.off,
-                                      workspace_bytes - ws.off, stream);
-  if (s != STRATA_OK) return s;
-  if ((e = cudaMemcpyAsync(o, do_, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_status(e);
-  if ((e = cudaMemcpyAsync(lse, dlse, sb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_status(e);
-  return STRATA_OK;
+  const void* in[3] = {q, k, v};
+  void* out[1] = {o};
+  return host_pipeline(desc, false, in, 3, out, 1, nullptr, lse, coords, freqs, workspace, workspace_bytes,
+                       reinterpret_cast<cudaStream_t>(stream));
 }
 
 strata_status_t strata_na3d_bwd_host(const strata_na3d_desc_t* desc, const void* q, const void* k,
@@ -372,40 +400,11 @@ strata_status_t strata_na3d_bwd_host(const strata_na3d_desc_t* desc, const void*
                                      const float* lse, const float* coords, const float* freqs,
                                      void* dq, void* dk, void* dv, void* workspace,
                                      size_t workspace_bytes, void* stream) {
-  Problem p; strata_status_t why;
-  if (!make_problem(desc, &p, &why)) return why;
   if (!q || !k || !v || !o || !d_o || !lse || !dq || !dk || !dv) return STRATA_ERR_INVALID_ARG;
-  if (p.A > 0 && (!coords || !freqs)) return STRATA_ERR_INVALID_ARG;
-  const size_t need = strata_na3d_host_workspace_bytes(desc, 1);
-  if (need == 0) return STRATA_ERR_UNSUPPORTED;
-  if (!workspace || workspace_bytes < need) return STRATA_ERR_WORKSPACE;
-  if (misaligned(workspace)) return STRATA_ERR_INVALID_ARG;
-  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  Carve ws{reinterpret_cast<char*>(workspace), 0};
-  const size_t tb = tensor_bytes(p), sb = stat_bytes(p), cb = coords_bytes(p), fb = freqs_bytes(p);
-  const void* hsrc[5] = {q, k, v, o, d_o};
-  void* dsrc[5];
-  for (int i = 0; i < 5; ++i) dsrc[i] = ws.take<char>(tb);
-  void* dout[3];
-  for (int i = 0; i < 3; ++i) dout[i] = ws.take<char>(tb);
-  float* dlse = ws.take<float>(sb);
-  float* dco = ws.take<float>(cb); float* dfr = ws.take<float>(fb);
-  cudaError_t e;
-  for (int i = 0; i < 5; ++i)
-    if ((e = cudaMemcpyAsync(dsrc[i], hsrc[i], tb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  if ((e = cudaMemcpyAsync(dlse, lse, sb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  if (p.A > 0) {
-    if ((e = cudaMemcpyAsync(dco, coords, cb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-    if ((e = cudaMemcpyAsync(dfr, freqs, fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_status(e);
-  }
-  strata_status_t s = strata_na3d_bwd(desc, dsrc[0], dsrc[1], dsrc[2], dsrc[3], dsrc[4], dlse, dco, dfr,
-                                      dout[0], dout[1], dout[2], ws.base + ws.off,
-                                      workspace_bytes - ws.off, stream);
-  if (s != STRATA_OK) return s;
-  void* hdst[3] = {dq, dk, dv};
-  for (int i = 0; i < 3; ++i)
-    if ((e = cudaMemcpyAsync(hdst[i], dout[i], tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_status(e);
-  return STRATA_OK;
+  const void* in[5] = {q, k, v, o, d_o};
+  void* out[3] = {dq, dk, dv};
+  return host_pipeline(desc, true, in, 5, out, 3, lse, nullptr, coords, freqs, workspace, workspace_bytes,
+                       reinterpret_cast<cudaStream_t>(stream));
 }
 
 int strata_na3d_last_launch_count(void) { return g_last_launches; }
@@ -432,6 +431,82 @@ const char* strata_status_string(strata_status_t s) {
   return "unknown status";
 }
 
-int strata_version(void) { return 100; }
+int strata_version(void) { return 200; }
 
 }  // extern "C"
+
+namespace {
+
+strata_status_t host_pipeline(const strata_na3d_desc_t* desc, bool backward, const void* const* h_in, int n_in,
+                              void* const* h_out, int n_out, const float* h_lse_in, float* h_lse_out,
+                              const float* h_coords, const float* h_freqs, void* workspace, size_t workspace_bytes,
+                              cudaStream_t st) {
+  Problem p; strata_status_t why;
+  if (!make_problem(desc, &p, &why)) return why;
+  if (p.A > 0 && (!h_coords || !h_freqs)) return STRATA_ERR_INVALID_ARG;
+  strata_na3d_desc_t d1 = *desc;
+  d1.batch = 1;
+  Problem p1;
+  if (!make_problem(&d1, &p1, &why)) return why;
+  const Path path = select_path(&d1, p1, backward);
+  if (path == PATH_NONE) return STRATA_ERR_UNSUPPORTED;
+  const HostLayout L = host_layout(p1, path, backward);
+  if (!workspace || workspace_bytes < L.total) return STRATA_ERR_WORKSPACE;
+  if (misaligned(workspace)) return STRATA_ERR_INVALID_ARG;
+  HostPipe* hp = host_pipe();
+  if (!hp) return STRATA_ERR_CUDA;
+  char* base = reinterpret_cast<char*>(workspace);
+  float* d_freqs = reinterpret_cast<float*>(base + 2 * L.slot);
+  char* inner = base + 2 * L.slot + L.freqs;
+  const size_t tb = tensor_bytes(p1), sb = stat_bytes(p1), cb = coords_bytes(p1), fb = freqs_bytes(p1);
+  // slot layout: inputs | outputs | lse | coords
+  auto slot_tensor = [&](int slot, int i) { return base + slot * L.slot + (size_t)i * L.tensor; };
+  auto slot_lse = [&](int slot) { return reinterpret_cast<float*>(base + slot * L.slot + (size_t)(n_in + n_out) * L.tensor); };
+  auto slot_coords = [&](int slot) { return reinterpret_cast<float*>(base + slot * L.slot + (size_t)(n_in + n_out) * L.tensor + L.stat); };
+
+  STRATA_CK(cudaEventRecord(hp->entry, st));                       // the copies start after what is already on `stream`
+  STRATA_CK(cudaStreamWaitEvent(hp->s_in, hp->entry, 0));
+  STRATA_CK(cudaStreamWaitEvent(hp->s_out, hp->entry, 0));
+  if (p.A > 0) STRATA_CK(cudaMemcpyAsync(d_freqs, h_freqs, fb, cudaMemcpyHostToDevice, hp->s_in));
+  int launches = 0;
+  for (int b = 0; b < p.B; ++b) {
+    const int s = b & 1;
+    // ---- copies in (slot s was last read by the kernels of sample b - 2)
+    if (b >= 2) STRATA_CK(cudaStreamWaitEvent(hp->s_in, hp->compute_done[s], 0));
+    for (int i = 0; i < n_in; ++i)
+      STRATA_CK(cudaMemcpyAsync(slot_tensor(s, i), static_cast<const char*>(h_in[i]) + (size_t)b * tb, tb,
+                                cudaMemcpyHostToDevice, hp->s_in));
+    if (h_lse_in) STRATA_CK(cudaMemcpyAsync(slot_lse(s), h_lse_in + (size_t)b * (sb / 4), sb, cudaMemcpyHostToDevice, hp->s_in));
+    if (p.A > 0) STRATA_CK(cudaMemcpyAsync(slot_coords(s), h_coords + (size_t)b * (cb / 4), cb, cudaMemcpyHostToDevice, hp->s_in));
+    STRATA_CK(cudaEventRecord(hp->in_ready[s], hp->s_in));
+    // ---- kernels of the sample on the caller's stream (its outputs of sample b - 2 must have left the slot)
+    STRATA_CK(cudaStreamWaitEvent(st, hp->in_ready[s], 0));
+    if (b >= 2) STRATA_CK(cudaStreamWaitEvent(st, hp->out_done[s], 0));
+    strata_status_t rc;
+    if (!backward)
+      rc = strata_na3d_fwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_coords(s), d_freqs,
+                           slot_tensor(s, n_in), slot_lse(s), inner, L.inner, st);
+    else
+      rc = strata_na3d_bwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_tensor(s, 3), slot_tensor(s, 4),
+                           slot_lse(s), slot_coords(s), d_freqs, slot_tensor(s, n_in), slot_tensor(s, n_in + 1),
+                           slot_tensor(s, n_in + 2), inner, L.inner, st);
+    if (rc != STRATA_OK) return rc;
+    launches += g_last_launches;
+    STRATA_CK(cudaEventRecord(hp->compute_done[s], st));
+    // ---- copies out
+    STRATA_CK(cudaStreamWaitEvent(hp->s_out, hp->compute_done[s], 0));
+    for (int i = 0; i < n_out; ++i)
+      STRATA_CK(cudaMemcpyAsync(static_cast<char*>(h_out[i]) + (size_t)b * tb, slot_tensor(s, n_in + i), tb,
+                                cudaMemcpyDeviceToHost, hp->s_out));
+    if (h_lse_out) STRATA_CK(cudaMemcpyAsync(h_lse_out + (size_t)b * (sb / 4), slot_lse(s), sb, cudaMemcpyDeviceToHost, hp->s_out));
+    STRATA_CK(cudaEventRecord(hp->out_done[s], hp->s_out));
+  }
+  // ---- join: the call is complete on `stream` when the last copies out are
+  for (int s = 0; s < 2 && s < p.B; ++s) STRATA_CK(cudaStreamWaitEvent(st, hp->out_done[s], 0));
+  STRATA_CK(cudaEventRecord(hp->entry, hp->s_in));
+  STRATA_CK(cudaStreamWaitEvent(st, hp->entry, 0));
+  g_last_launches = launches;
+  return STRATA_OK;
+}
+
+}  // namespace
