@@ -22,6 +22,7 @@ import numpy as np
 from . import build as _build
 from . import geometry  # noqa: F401
 from . import normgate as _normgate
+from . import stitch  # noqa: F401
 
 _LIB = None
 

@@ -509,3 +509,36 @@ def test_normgate_backward_vs_finite_differences(oracle_mod):
     # with eps = 0 the output does not depend on |q|: the gradient is orthogonal to q, row by row
     dq0, dk0, _, _ = oracle_mod.na3d_normgate_bwd(q, k, v, gate, d_o, coords, freqs, window, eps=0.0)
     assert np.max(np.abs(np.sum(dq0 * q, -1))) < 1e-12 and np.max(np.abs(np.sum(dk0 * k, -1))) < 1e-12
+
+
+# ------------------------------------------------------------------ tile stitching, eq. (5)
+def test_stitch_and_kbd_window(oracle_mod):
+    st = oracle_mod.stitch
+    w = st.kbd_window(32, 4.0)
+    # the defining property of a Kaiser-Bessel-DERIVED window (Princen-Bradley): w[j]^2 + w[j + n/2]^2 = 1; symmetric;
+    # rising over the first half; "tapers smoothly to zero at the edges"
+    assert np.max(np.abs(w[:16] ** 2 + w[16:] ** 2 - 1.0)) < 1e-14
+    assert np.array_equal(w, w[::-1]) and np.all(np.diff(w[:16]) > 0) and w[0] < 0.01 and abs(w[15] - 1.0) < 1e-2
+    # hand value, n = 2: k = (I0(0), I0(0)) -> w = sqrt(1/2)
+    assert np.allclose(st.kbd_window(2, 4.0), [math.sqrt(0.5)] * 2, atol=1e-15)
+    rng = np.random.default_rng(3)
+    th = tw = 16
+    origins = [(0, 0), (0, 12), (12, 0), (12, 12)]                     # stride 12: tiles share a border of 4 cells
+    gh = gw = 28
+    field = rng.normal(size=(3, gh, gw))
+    tiles = np.stack([field[:, y:y + th, x:x + tw] for y, x in origins])
+    wk = st.kbd_window(16, 4.0)
+    # (i) tiles cut from one field stitch back to it, whatever the (positive) window: S P = identity
+    assert np.max(np.abs(st.stitch(tiles, origins, wk, wk, gh, gw) - field)) < 1e-13
+    # (ii) "a 2D top-hat filter that is 1 in the interior and 0 in the halo ... reduces to simply a crop"
+    noisy = tiles + rng.normal(size=tiles.shape)                        # tile outputs that disagree in the overlaps
+    hat = np.zeros(16); hat[2:14] = 1.0                                 # halo of 2 on each side: interiors tile the field
+    got = st.stitch(noisy, origins, hat, hat, gh, gw)
+    for t, (y, x) in enumerate(origins):
+        assert np.array_equal(got[:, y + 2:y + 14, x + 2:x + 14], noisy[t][:, 2:14, 2:14])
+    assert np.all(got[:, :2, :] == 0.0)                                 # nobody's interior: weight 0, value 0
+    # (iii) a weighted AVERAGE: between the min and max of the contributing tiles, cell by cell; by hand in one cell
+    got = st.stitch(noisy, origins, wk, wk, gh, gw)
+    y, x = 5, 13                                                        # covered by tiles 0 (5, 13) and 1 (5, 1)
+    w0, w1 = wk[5] * wk[13], wk[5] * wk[1]
+    assert abs(got[1, y, x] - (w0 * noisy[0, 1, 5, 13] + w1 * noisy[1, 1, 5, 1]) / (w0 + w1)) < 1e-14
