@@ -196,6 +196,15 @@ strata_status_t strata_wind_to_tile_frame(const float* u, const float* v, const 
                                           long long n, double lat0, double lon0, float* u_loc, float* v_loc,
                                           void* stream);
 
+/* strata_tile_stitch: eq. (5), S = D^-1 P^T W: "each tile's output is weighted by a 2D ... window ...;
+ * the final value at each grid cell is the weighted average of all overlapping tile outputs".  tiles [T, C, th, tw]
+ * float32; origins [T, 2] int32 = (y0, x0) of each tile in the [C, gh, gw] field (tiles inside the field: P copies
+ * cells; cross-face interpolation is not modelled); wy [th], wx [tw]: the separable window (an input: the paper names a
+ * Kaiser-Bessel-derived window without parameters; a top-hat makes this a crop).  Cells no tile covers with a
+ * positive weight are set to 0.  All pointers DEVICE memory; asynchronous on `stream`. */
+strata_status_t strata_tile_stitch(const float* tiles, const int32_t* origins, int n_tiles, int channels, int th, int tw,
+                                   const float* wy, const float* wx, float* out, int gh, int gw, void* stream);
+
 const char* strata_status_string(strata_status_t status);
 int strata_version(void);
 

@@ -26,7 +26,7 @@ EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "s
            "strata_na3d_normgate_workspace_bytes", "strata_na3d_normgate_fwd", "strata_na3d_normgate_bwd",
            "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
            "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_stereo_coords",
-           "strata_wind_to_tile_frame", "strata_status_string", "strata_version")
+           "strata_wind_to_tile_frame", "strata_tile_stitch", "strata_status_string", "strata_version")
 
 
 class StrataError(RuntimeError):
@@ -120,6 +120,8 @@ def lib() -> ctypes.CDLL:
         L.strata_wind_to_tile_frame.restype = i32
         L.strata_wind_to_tile_frame.argtypes = [vp, vp, vp, vp, ctypes.c_longlong, ctypes.c_double, ctypes.c_double,
                                                 vp, vp, vp]
+        L.strata_tile_stitch.restype = i32
+        L.strata_tile_stitch.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, i32, i32, vp]
         L.strata_status_string.restype = ctypes.c_char_p
         L.strata_status_string.argtypes = [i32]
         L.strata_version.restype = i32
@@ -276,6 +278,18 @@ def strata_wind_to_tile_frame(u, v, lat, lon, lat0: float, lon0: float, u_loc, v
             raise TypeError("u, v, u_loc, v_loc: float32; lat, lon: float64; all of one size")
     _check(lib().strata_wind_to_tile_frame(_ptr(u), _ptr(v), _ptr(lat), _ptr(lon), n, float(lat0), float(lon0),
                                            _ptr(u_loc), _ptr(v_loc), _stream_handle(stream)), "strata_wind_to_tile_frame")
+
+
+def strata_tile_stitch(tiles, origins, wy, wx, out, stream=None):
+    """Eq. (5) on the device: tiles [T,C,th,tw] f32, origins [T,2] int32, windows wy [th], wx [tw], out [C,gh,gw] f32."""
+    T, C, th, tw = tiles.shape
+    if origins.dtype != torch.int32 or tuple(origins.shape) != (T, 2) or wy.numel() != th or wx.numel() != tw:
+        raise TypeError("origins: int32 [T, 2]; wy [th]; wx [tw]")
+    for t in (tiles, wy, wx, out):
+        if t.dtype != torch.float32:
+            raise TypeError("tiles, windows and out are float32")
+    _check(lib().strata_tile_stitch(_ptr(tiles), _ptr(origins), T, C, th, tw, _ptr(wy), _ptr(wx), _ptr(out), out.shape[1],
+                                    out.shape[2], _stream_handle(stream)), "strata_tile_stitch")
 
 
 # ------------------------------------------------------------------ convenience: allocate + call

@@ -1,4 +1,5 @@
-// geometry.cu -- the StereoRoPE inputs on the device: eq. (1) (tile-centred stereographic coordinates)
+// geometry.cu -- the field-level pieces around the attention on the device: tile stitching, eq. (5),
+// and the StereoRoPE inputs: eq. (1) (tile-centred stereographic coordinates)
 // and eq. (2) (winds in the tile centre's East-North frame).  Elementwise, HBM-bound (16 bytes of
 // lat / lon in per point); float64 arithmetic because the coordinates (up to ~1.5e3 in units of l_scale) are handed
 // to the attention kernels as float32 and must be correct to the last bit or two of that.
@@ -46,6 +47,26 @@ wind_frame_kernel(const float* __restrict__ u, const float* __restrict__ v, cons
   }
 }
 
+// eq. (5): out = D^-1 P^T W y for tiles that lie inside the field (P copies cells).  One thread per
+// cell of the [C, GH, GW] field; every tile that covers the cell contributes wy[dy] wx[dx] y_t[c, dy, dx].
+__global__ void __launch_bounds__(256)
+tile_stitch_kernel(const float* __restrict__ tiles, const int* __restrict__ origins, int T, int C, int th, int tw,
+                   const float* __restrict__ wy, const float* __restrict__ wx, float* __restrict__ out, int GH, int GW) {
+  const long long n = (long long)C * GH * GW;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int gx = (int)(i % GW), gy = (int)((i / GW) % GH), c = (int)(i / ((long long)GW * GH));
+    float num = 0.f, den = 0.f;
+    for (int t = 0; t < T; ++t) {
+      const int dy = gy - origins[2 * t], dx = gx - origins[2 * t + 1];
+      if (dy < 0 || dy >= th || dx < 0 || dx >= tw) continue;
+      const float w = wy[dy] * wx[dx];
+      num = fmaf(w, tiles[(((long long)t * C + c) * th + dy) * tw + dx], num);
+      den += w;
+    }
+    out[i] = den > 0.f ? num / den : 0.f;
+  }
+}
+
 unsigned grid_for(long long n) {
   const long long b = (n + 255) / 256;
   return (unsigned)(b < 1 ? 1 : b > 148 * 32 ? 148 * 32 : b);
@@ -77,6 +98,19 @@ strata_status_t strata_wind_to_tile_frame(const float* u, const float* v, const 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   strata::prof_begin("wind_to_tile_frame", st);
   strata::wind_frame_kernel<<<strata::grid_for(n), 256, 0, st>>>(u, v, lat, lon, n, sin(lat0), cos(lat0), sin(lon0), cos(lon0), u_loc, v_loc);
+  strata::prof_end(st);
+  if (cudaGetLastError() != cudaSuccess) return STRATA_ERR_CUDA;
+  return STRATA_OK;
+}
+
+strata_status_t strata_tile_stitch(const float* tiles, const int32_t* origins, int n_tiles, int channels, int th, int tw,
+                                   const float* wy, const float* wx, float* out, int gh, int gw, void* stream) {
+  if (!tiles || !origins || !wy || !wx || !out || n_tiles < 1 || channels < 1 || th < 1 || tw < 1 || gh < 1 || gw < 1)
+    return STRATA_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  strata::prof_begin("tile_stitch", st);
+  strata::tile_stitch_kernel<<<strata::grid_for((long long)channels * gh * gw), 256, 0, st>>>(tiles, origins, n_tiles, channels, th, tw,
+                                                                                       wy, wx, out, gh, gw);
   strata::prof_end(st);
   if (cudaGetLastError() != cudaSuccess) return STRATA_ERR_CUDA;
   return STRATA_OK;

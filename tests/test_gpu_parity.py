@@ -494,3 +494,21 @@ def lib_status_invalid():
     L = binding.lib()
     return L.strata_stereo_coords(None, None, 4, 0.0, 0.0, 1.0, None, 2, None) == 1 and \
         L.strata_wind_to_tile_frame(None, None, None, None, 4, 0.0, 0.0, None, None, None) == 1
+
+
+def test_tile_stitch_kernel(oracle_mod):
+    """strata_tile_stitch against oracle/stitch.py on config 3's tile layout of one face (2 x 2 tiles of 128 x 128 with
+    stride 112) at reduced channel count, Kaiser-Bessel-derived and top-hat windows."""
+    rng = np.random.default_rng(13)
+    T, C, th = 4, 5, 128
+    origins = np.array([(0, 0), (0, 112), (112, 0), (112, 112)], dtype=np.int32)
+    gh = gw = 240
+    tiles = rng.normal(size=(T, C, th, th)).astype(np.float32)
+    hat = np.zeros(th, np.float32); hat[8:120] = 1.0
+    for wy in (oracle_mod.stitch.kbd_window(th, 4.0).astype(np.float32), hat):
+        out = torch.full((C, gh, gw), 7.0, dtype=torch.float32, device="cuda")
+        binding.strata_tile_stitch(torch.from_numpy(tiles).cuda(), torch.from_numpy(origins).cuda(), torch.from_numpy(wy).cuda(),
+                                   torch.from_numpy(wy).cuda(), out)
+        ref = oracle_mod.stitch.stitch(tiles, origins, wy, wy, gh, gw)
+        err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
+        assert err.max() <= 1e-5, f"stitch: max abs err {err.max():.3e}"
