@@ -310,7 +310,9 @@ def alloc_workspace(nbytes: int, device) -> torch.Tensor:
 
 def na3d_forward(q, k, v, coords, freqs, window, rope_pairing=ROPE_INTERLEAVED, scale=0.0, impl=IMPL_AUTO,
                  workspace=None, stream=None):
-    """StereoRoPE + NA3D forward on device tensors.  Returns (o, lse)."""
+    """StereoRoPE + NA3D forward on device tensors.  Returns (o, lse).
+    A workspace allocated here (workspace=None) comes from torch's caching allocator on the CURRENT torch stream:
+    pass your own workspace when `stream` is another stream."""
     if not q.is_cuda:
         raise StrataError("na3d_forward needs CUDA tensors (there is no CPU path)")
     rope_axes = 0 if coords is None else coords.shape[-1]

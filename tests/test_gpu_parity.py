@@ -155,19 +155,21 @@ def test_qknorm_logits_bf16(oracle_mod):
 
 
 def test_large_logits_stay_close(oracle_mod):
-    """Unit-normal q, k with scale 0.5: logits of +-30 (the fused forward subtracts no maximum: e^30 is in range)."""
+    """Unit-normal q, k with scale 0.5: logits of +-20 (the fused forward subtracts no maximum: e^20 is in range)."""
     w = wl.small(name="hot", dtype="bf16", value_scale="unit", grid=(8, 16, 24), window=(3, 7, 7),
                  heads=2, head_dim=64)
     inp = wl.make_inputs(w)
     d, o, lse = run_fwd(w, inp, binding.IMPL_AUTO, 0.5)
     o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window, scale=0.5)
-    # logits of +-30 amplify the bf16 rounding of qrot / krot (2^-9 relative on each of the 64 products)
-    # into ~2e-2 on the logits, i.e. percent-level errors on P: outside north_star's tolerance by
-    # construction (the in-tolerance test of the same range is the exact-input one below).
+    # The rotated operands are rounded to bf16 (and the fused forward rotates in bf16x2 arithmetic): the error of a
+    # logit grows with its size, measured max-abs error on O 0.0085 / 0.028 / 0.060 / 0.092 at max |logit| 6 / 10 / 20 /
+    # 30 (DESIGN.md section 7).  At +-20 that is outside north_star's per-element bound by construction; held here: 1.5x
+    # the measured maximum, and the NORMAL relative-RMS bound (measured 7.5e-3).  The in-tolerance test of large logits
+    # is the exact-input one below.
     err = np.abs(to_f64(o) - o_ref)
-    assert np.isfinite(to_f64(o)).all() and err.max() < 0.15
-    assert np.sqrt(np.mean(err ** 2)) / np.sqrt(np.mean(o_ref ** 2)) < 3e-2
-    assert float(np.abs(to_f64(lse) - lse_ref).max()) < 0.15
+    assert np.isfinite(to_f64(o)).all() and err.max() < 0.09
+    assert np.sqrt(np.mean(err ** 2)) / np.sqrt(np.mean(o_ref ** 2)) < 1e-2
+    assert float(np.abs(to_f64(lse) - lse_ref).max()) < 0.075
 
 
 def _bf16_bits(x):
