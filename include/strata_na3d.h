@@ -67,7 +67,7 @@ typedef enum { STRATA_ROPE_INTERLEAVED = 0, STRATA_ROPE_HALF = 1 } strata_rope_p
 typedef enum {
   STRATA_IMPL_AUTO = 0,
   STRATA_IMPL_SIMT = 1,
-  STRATA_IMPL_TCGEN05 = 2,      /* tensor-core kernels; level-sweep kernel where it applies */
+  STRATA_IMPL_TCGEN05 = 2,      /* tensor-core kernels; the fused forward (na3d_fwd_plane.cu) where it applies */
   STRATA_IMPL_TCGEN05_TILE = 3  /* tensor-core kernel with one query tile per CTA (any covered shape) */
 } strata_impl_t;
 

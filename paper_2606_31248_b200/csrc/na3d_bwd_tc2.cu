@@ -1,15 +1,34 @@
-// na3d_bwd_tc2.cu -- persistent, double-buffered version of the tensor-core backward (na3d_bwd_tc.cu).
+// na3d_bwd_tc2.cu -- tcgen05 / TMEM / TMA backward kernels for 3D neighbourhood attention (sm_100a), bf16, head_dim 64.
 //
-// Same mathematics, modes and per-chunk MMAs as na3d_bwd_tc.cu (read that header first: MODE 0 = dQ,
-// query-stationary; MODE 1 = dK / dV, key-stationary over the inverse neighbourhood; B4 fused in the
-// epilogue).  What differs is the schedule.  A trace of na3d_bwd_tc.cu (profiles/r1_bwd_cfg4_and_tile_cfg2.md)
-// shows a chunk costing ~3100 cycles in a strictly serial chain -- S'/dP' MMAs, elementwise pass, gradient
-// MMAs -- that two co-resident CTAs only half fill.  Here ONE persistent CTA per SM runs the chain as a
-// pipeline:
+// Steps B2-B4 of DESIGN.md on pre-rotated bf16 operands (rope.cu rotates Q, K before; the transpose rotation B4 of
+// dQrot, dKrot is fused into the epilogues, from an fp32 cos / sin table; B1 is bwd_stat_kernel in na3d_bwd_tc.cu).
+// PAPER.md gives no backward; BASELINE.json config 4 and SURVEY.md section 8(a) rows B1-B4 define it:
+//   B2  p_ij   = exp(scale qrot_i . krot_j - lse_i),  dP_ij = dO_i . v_j,  dS_ij = p_ij (dP_ij - D_i)
+//       dqrot_i = scale sum_j dS_ij krot_j;  dkrot_j = scale sum_i dS_ij qrot_i;  dV_j = sum_i p_ij dO_i
+// ONE kernel template, two modes, both "a stationary tile of 128 rows against streamed chunks":
+//   MODE 0 (dQ, query-stationary)  rows = queries: A1 = Qrot, A2 = dO tile; chunks = the keys of the
+//       tile's window halo: B1 = Krot, B2 = V.            acc1 = dQrot = sum dS  B1
+//   MODE 1 (dK/dV, key-stationary) rows = keys:    A1 = Krot, A2 = V tile;  chunks = the queries of
+//       the tile's INVERSE halo (B3: the queries whose inward-clamped window holds a key of the tile --
+//       not symmetric at the borders): B1 = Qrot, B2 = dO.  acc1 = dKrot = sum dS^T B1,
+//       acc2 = dV = sum P^T B2.  Row statistics (lse, D) belong to the chunk's columns here: the
+//       elementwise threads fetch them one chunk ahead and publish them in shared memory.
+// Per chunk (CY rows x HX columns of one level plane = N <= 64 columns):
+//   S' = A1 B1^T and dP' = A2 B2^T on the tensor cores (M = 128, K = 64) -> TMEM;
+//   one row per thread: p = 2^(S' scale log2e - lse log2e) under the window mask, dS = p (dP' - D),
+//   written back to TMEM as bf16 over the buffers they came from;
+//   acc1 += dS B1 (and acc2 += P B2) with the bf16 matrix as the TMEM A operand and the SAME shared
+//   memory chunk re-read as an MN-major B operand.
+// No atomics: every output row is owned by exactly one thread; deterministic.
+//
+// Schedule: ONE persistent CTA per SM runs the chain S'/dP' MMAs -> elementwise pass -> gradient MMAs as a pipeline
+// (a one-tile-per-CTA version of round 1 cost ~3100 cycles per chunk in a strictly serial chain that two co-resident
+// CTAs only half filled, profiles/r1_bwd_cfg4_and_tile_cfg2.md):
 //   * S' / dP' have three buffers in TMEM and TWO elementwise warpgroups take alternate chunks, so the
 //     MMAs of chunks c + 1, c + 2 run under the elementwise pass of chunk c;
-//   * the stationary operand tiles are double buffered in shared memory (and the dQ accumulator in TMEM) and the chunk stream runs on across tiles, so the epilogue of tile t
-//     (TMEM -> un-rotate -> HBM) and the operand loads of tile t + 1 overlap the MMAs of tile t + 1.
+//   * the stationary operand tiles are double buffered in shared memory (and the dQ accumulator in TMEM) and the
+//     chunk stream runs on across tiles, so the epilogue of tile t (TMEM -> un-rotate -> HBM) and the operand loads
+//     of tile t + 1 overlap the MMAs of tile t + 1.
 // TMEM (512 columns): accumulators [0, 128) -- MODE 0: acc1 double buffered by tile parity, MODE 1: {acc1, acc2}
 // once -- | SD[buf] = {S' -> P, dP' -> dS} at 128 + 128 * buf, buf < 3 (chunk index mod 3).
 // Warps (352 threads): 0 TMA producer, 1 S'/dP' MMA issuer + TMEM owner, 2-5 elementwise group 0, 6-9 group 1,
