@@ -39,6 +39,9 @@ struct Cfg {
   // P (bf16 pairs) overlays the front of S: every S column of a chunk is in registers before P is stored
   static constexpr int TMEM_O = 0, TMEM_S = D, TMEM_P = D;
   static constexpr int TMEM_COLS = (D + NKEY <= 256) ? 256 : 512;
+  // Two S buffers where they fit the same allocation (d = 128: 128 + 2 x 64): Q K^T of chunk c + 1 runs under the
+  // softmax of chunk c.
+  static constexpr int NSBUF = (D + 2 * NKEY <= TMEM_COLS) ? 2 : 1;
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = 1024 + Q_BYTES + 2 * NSTAGE * STAGE_BYTES + BAR_BYTES;
   static constexpr int CTAS_PER_SM = (2 * SMEM_BYTES <= 227 * 1024 && TMEM_COLS == 256) ? 2 : 1;
@@ -77,10 +80,12 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   auto bar_kempty = [&](int s) { return bars + 8u * (1 + C::NSTAGE + s); };
   auto bar_vfull = [&](int s) { return bars + 8u * (1 + 2 * C::NSTAGE + s); };
   auto bar_vempty = [&](int s) { return bars + 8u * (1 + 3 * C::NSTAGE + s); };
-  const uint32_t bar_sfull = bars + 8u * (1 + 4 * C::NSTAGE);
-  const uint32_t bar_pfull = bar_sfull + 8;
-  const uint32_t bar_pvdone = bar_sfull + 16;
-  const uint32_t tmem_slot = bar_sfull + 24;
+  const uint32_t bar_sfull = bars + 8u * (1 + 4 * C::NSTAGE);      // [2] by S buffer
+  const uint32_t bar_pfull = bar_sfull + 16;                        // [2]
+  // [2] by chunk parity: a softmax warp can be two P V ahead of the last completed one when Q K^T runs a chunk ahead,
+  // and one barrier's parity cannot tell phase c - 1 from phase c - 3
+  const uint32_t bar_pvdone = bar_sfull + 32;
+  const uint32_t tmem_slot = bar_sfull + 48;
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -110,9 +115,9 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       mbar_init(bar_kfull(s), 1); mbar_init(bar_kempty(s), 1);
       mbar_init(bar_vfull(s), 1); mbar_init(bar_vempty(s), 1);
     }
-    mbar_init(bar_sfull, 1);
-    mbar_init(bar_pfull, 128);
-    mbar_init(bar_pvdone, 1);
+    mbar_init(bar_sfull, 1); mbar_init(bar_sfull + 8, 1);
+    mbar_init(bar_pfull, 128); mbar_init(bar_pfull + 8, 128);
+    mbar_init(bar_pvdone, 1); mbar_init(bar_pvdone + 8, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
@@ -160,8 +165,9 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
       mbar_wait(bar_q, 0);
       tc_fence_after();
-      for (int c = 0; c < nchunks; ++c) {
-        const int s = c % C::NSTAGE;
+      // chunk c uses S buffer c % NSBUF; barrier phases of a buffer count its uses
+      auto issue_qk = [&](int c) {
+        const int s = c % C::NSTAGE, sb = c % C::NSBUF;
         const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
         // ---- S = Qrot Krot^T  (M = 128, N = NKEY, K = D in steps of 16)
         mbar_wait(bar_kfull(s), ph);
@@ -171,12 +177,20 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
           const uint32_t off = (ks >> 2) * 1u, kin = (ks & 3) * 32u;      // sub-tile, byte offset in the row
           const uint64_t ad = smem_desc(q_smem + off * C::SUB_Q + kin);
           const uint64_t bd = smem_desc(k_smem + s * C::STAGE_BYTES + off * C::SUB_KV + kin);
-          umma_ss(tmem + C::TMEM_S, ad, bd, idesc_qk, ks > 0 ? 1u : 0u);
+          umma_ss(tmem + C::TMEM_S + sb * C::NKEY, ad, bd, idesc_qk, ks > 0 ? 1u : 0u);
         }
         umma_commit(bar_kempty(s));
-        umma_commit(bar_sfull);
+        umma_commit(bar_sfull + 8u * sb);
+      };
+      // With two buffers Q K^T runs one chunk ahead: buffer (c + 1) % 2 is free once P V of chunk c - 1 (which read
+      // its P) has been issued -- the tensor pipe executes in issue order.
+      if (nchunks > 0) issue_qk(0);
+      for (int c = 0; c < nchunks; ++c) {
+        const int s = c % C::NSTAGE, sb = c % C::NSBUF;
+        const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
+        if (C::NSBUF == 2 && c + 1 < nchunks) issue_qk(c + 1);
         // ---- O += P V  (M = 128, N = 64 per sub-tile, K = NKEY in steps of 16 keys)
-        mbar_wait(bar_pfull, (uint32_t)c & 1u);
+        mbar_wait(bar_pfull + 8u * sb, (uint32_t)(c / C::NSBUF) & 1u);
         mbar_wait(bar_vfull(s), ph);
         tc_fence_after();
 #pragma unroll
@@ -184,11 +198,12 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
 #pragma unroll
           for (int j = 0; j < C::DSUB; ++j) {
             const uint64_t bd = smem_desc(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
-            umma_ts(tmem + C::TMEM_O + 64 * j, tmem + C::TMEM_P + 8 * ks, bd, idesc_pv, (c > 0 || ks > 0) ? 1u : 0u);
+            umma_ts(tmem + C::TMEM_O + 64 * j, tmem + C::TMEM_P + sb * C::NKEY + 8 * ks, bd, idesc_pv, (c > 0 || ks > 0) ? 1u : 0u);
           }
         }
         umma_commit(bar_vempty(s));
-        umma_commit(bar_pvdone);
+        umma_commit(bar_pvdone + 8u * (c & 1));
+        if (C::NSBUF == 1 && c + 1 < nchunks) issue_qk(c + 1);
       }
     }
   } else {
@@ -217,7 +232,9 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       const bool plane_needed = pl >= wl_lo && pl < wl_hi;
       const bool plane_ok = pl >= lo_l && pl < lo_l + C::KL;
       for (int cy = 0; cy < ncy; ++cy, ++c) {
-        mbar_wait(bar_sfull, (uint32_t)c & 1u);
+        const int sb = c % C::NSBUF;
+        const uint32_t s_tm = tmem + lane_addr + C::TMEM_S + sb * C::NKEY;       // S of the chunk; P goes over its front
+        mbar_wait(bar_sfull + 8u * sb, (uint32_t)(c / C::NSBUF) & 1u);
         tc_fence_after();
         uint32_t pw[C::NKEY / 2];
         float csum = 0.f;
@@ -229,7 +246,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             const int py = cy * C::CY + r;
             if (plane_needed && py >= wy_lo && py < wy_hi) {
               float sv[16];
-              tmem_ld16(tmem + lane_addr + C::TMEM_S + r * C::HX, sv);
+              tmem_ld16(s_tm + r * C::HX, sv);
               tmem_wait_ld();
               const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
               float t[C::HX];
@@ -259,7 +276,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
           if (attempt == 0 && __any_sync(0xffffffffu, need)) {
             const float alpha = need ? ex2(m_ref - cmax) : 1.f;
             if (c > 0) {                                    // O holds chunks 0..c-1: rescale its rows
-              mbar_wait(bar_pvdone, (uint32_t)(c - 1) & 1u);
+              mbar_wait(bar_pvdone + 8u * ((c - 1) & 1), (uint32_t)((c - 1) >> 1) & 1u);
               tc_fence_after();
 #pragma unroll
               for (int j = 0; j < C::D; j += 16) {
@@ -282,14 +299,14 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         lsum += csum;
         // P (bf16 pairs) -> TMEM, then hand the chunk to MMA2
 #pragma unroll
-        for (int j = 0; j < C::NKEY / 2; j += 8) tmem_st8(tmem + lane_addr + C::TMEM_P + j, &pw[j]);
+        for (int j = 0; j < C::NKEY / 2; j += 8) tmem_st8(s_tm + j, &pw[j]);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar_pfull);
+        mbar_arrive(bar_pfull + 8u * sb);
       }
     }
     // ---- epilogue: O / l -> bf16 -> global, LSE
-    mbar_wait(bar_pvdone, (uint32_t)(nchunks - 1) & 1u);
+    mbar_wait(bar_pvdone + 8u * ((nchunks - 1) & 1), (uint32_t)((nchunks - 1) >> 1) & 1u);
     tc_fence_after();
     const float inv = 1.f / lsum;
     const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
