@@ -30,7 +30,7 @@ struct Cfg {
   static constexpr int D = D_, KL = KL_, KY = KY_, KX = KX_;
   static constexpr int TL = 2, TY = 8, TX = 8, M = 128;            // query tile
   static constexpr int HL = TL + KL - 1, HY = TY + KY - 1, HX = TX + KX - 1;   // halo box
-  static constexpr int CY = (D == 128) ? 4 : 8;                    // key rows per chunk (d = 128: small stages, two CTAs per SM)
+  static constexpr int CY = (D == 128 || HX == 16) ? 4 : 8;        // key rows per chunk (d = 128 / 16-wide halos: 64 keys, so that two S buffers and two CTAs per SM fit)
   static constexpr int NKEY = CY * HX;                             // keys per chunk (UMMA N of S)
   static constexpr int DSUB = D / 64;                              // 128-byte sub-tiles per row
   static constexpr int SUB_Q = M * 128, SUB_KV = NKEY * 128;       // bytes of one sub-tile
