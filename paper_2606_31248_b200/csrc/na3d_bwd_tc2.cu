@@ -11,8 +11,13 @@
 //   MODE 1 (dK/dV, key-stationary) rows = keys:    A1 = Krot, A2 = V tile;  chunks = the queries of
 //       the tile's INVERSE halo (B3: the queries whose inward-clamped window holds a key of the tile --
 //       not symmetric at the borders): B1 = Qrot, B2 = dO.  acc1 = dKrot = sum dS^T B1,
-//       acc2 = dV = sum P^T B2.  Row statistics (lse, D) belong to the chunk's columns here: the
-//       elementwise threads fetch them one chunk ahead and publish them in shared memory.
+//       acc2 = dV = sum P^T B2.  The statistics (lse, D) belong to the chunk's COLUMNS here, and a per-column
+//       bias is a rank-one term, so the tensor cores add it: S' and dP' get a fifth K step whose A operand is a
+//       constant tile of ones (three channels) and whose B operand holds, for column j, -lse_j / (scale log2 e)
+//       resp. -D_j split into three bf16 terms (24 significant bits, the sum is exact in the fp32 accumulator).
+//       The producer warp writes that small B tile next to the chunk it streams.  (Reading the statistics from
+//       shared memory in the elementwise loop instead cost 28 loads per chunk and thread, each waiting behind the
+//       tensor cores' own operand reads: profiles/r2_bwd_cfg4.md.)
 // Per chunk (CY rows x HX columns of one level plane = N <= 64 columns):
 //   S' = A1 B1^T and dP' = A2 B2^T on the tensor cores (M = 128, K = 64) -> TMEM;
 //   one row per thread: p = 2^(S' scale log2e - lse log2e) under the window mask, dS = p (dP' - D),
@@ -56,11 +61,11 @@ struct Bwd2Cfg {
   static constexpr int TILE_BYTES = M * 128, CHUNK_BYTES = N * 128;
   static constexpr int STAGE_BYTES = 2 * CHUNK_BYTES;              // B1 | B2
   static constexpr int NSTAGE = 4;
-  static constexpr int STAT_BYTES = CY * 128;                      // [CY][16 tokens] float2 (MODE 1)
+  static constexpr int XTRA_BYTES = TILE_BYTES + NSTAGE * CHUNK_BYTES;   // MODE 1: ones tile | per-stage bias tiles
   static constexpr int NBUF = 3;                                   // S'/dP' buffers in TMEM
   static constexpr int TMEM_ACC = 0, TMEM_SD = 128, TMEM_COLS = 512;
   static constexpr int NBARS = 4 + 2 * NSTAGE + 3 * NBUF + 4;
-  static constexpr int SMEM_BYTES = 1024 + 4 * TILE_BYTES + NSTAGE * STAGE_BYTES + 8 * NBARS + 16 + 128 + 4 * STAT_BYTES;
+  static constexpr int SMEM_BYTES = 1024 + 4 * TILE_BYTES + NSTAGE * STAGE_BYTES + XTRA_BYTES + 8 * NBARS + 16 + 128;
   static_assert(KL % 2 == 1 && KY % 2 == 1 && KX % 2 == 1, "odd windows only");
   static_assert(N <= 64 && HX <= 16 && HX % 2 == 0, "a chunk must fit 64 TMEM columns; column pairs share a row");
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
@@ -89,7 +94,9 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   const uint32_t base = (raw + 1023u) & ~1023u;
   auto a_smem = [&](int par, int which) { return base + (uint32_t)(2 * par + which) * C::TILE_BYTES; };
   const uint32_t st_smem = base + 4 * C::TILE_BYTES;                       // stages
-  const uint32_t bars = st_smem + C::NSTAGE * C::STAGE_BYTES;
+  const uint32_t xa_smem = st_smem + C::NSTAGE * C::STAGE_BYTES;           // MODE 1: A operand of the bias K step
+  auto xb_smem = [&](int s) { return xa_smem + C::TILE_BYTES + (uint32_t)s * C::CHUNK_BYTES; };   // its B operand
+  const uint32_t bars = xa_smem + C::XTRA_BYTES;
   auto bar_afull = [&](int par) { return bars + 8u * par; };               // TMA -> MMA: operand tiles of a tile
   auto bar_aempty = [&](int par) { return bars + 8u * (2 + par); };        // last S'/dP' MMA of the tile -> TMA
   auto bar_full = [&](int s) { return bars + 8u * (4 + s); };
@@ -102,7 +109,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   // accumulators: MODE 0 needs acc1 only and double buffers it by tile parity; MODE 1 has {acc1, acc2} once
   constexpr int NACC = MODE == 0 ? 2 : 1, ACC_STRIDE = 64;
   const uint32_t tmem_slot = bars + 8u * C::NBARS;
-  const uint32_t stat_base = (tmem_slot + 16 + 127u) & ~127u;              // [group][2] x STAT_BYTES
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - raw));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -135,7 +141,8 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
       mbar_init(bar_accdone(i), 1); mbar_init(bar_accfree(i), MODE == 1 ? 8 : 4);
     }
     for (int i = 0; i < C::NBUF; ++i) { mbar_init(bar_sfull(i), 1); mbar_init(bar_pfull(i), 4); mbar_init(bar_sdfree(i), 1); }
-    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
+    // MODE 1: a chunk is complete when its TMA bytes have landed AND its bias tile is written
+    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), MODE == 1 ? 2 : 1); mbar_init(bar_empty(s), 1); }
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
@@ -149,22 +156,65 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
       }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
+  if (MODE == 1) {
+    // bias K step: row r of the ones tile has 1, 1, 1 in channels 0-2 and 16-18 (16-byte chunks 0 and 2 of the
+    // 128-byte swizzled row); the bias tiles start as zeros and only chunks 0 and 2 of a row are ever rewritten
+    for (int u = threadIdx.x; u < C::XTRA_BYTES / 16; u += kBwd2Threads) {
+      const int r = u >> 3, ch = (u & 7) ^ (r & 7);
+      const bool one = u < C::TILE_BYTES / 16 && (ch == 0 || ch == 2);
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(xa_smem + u * 16), "r"(one ? 0x3F803F80u : 0u),
+                   "r"(one ? 0x00003F80u : 0u), "r"(0u) : "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot_ptr;
 
   if (warp == 0) {
-    // =========================== TMA producer ===========================
-    if (lane == 0) {
+    // =========================== TMA producer (MODE 1: and the bias tiles) ===========================
+    // MODE 1, all lanes: lane j owns columns j and j + 32 of a chunk.  Their statistics are loaded before the wait
+    // for the chunk's stage and turned into the bias tile at the start of the NEXT iteration, so the global load
+    // hides behind that wait; the chunk's `full` barrier takes one arrival from the TMA and one from here.
+    if (lane == 0 || MODE == 1) {
       int Tn = 0, Cn = 0;
+      float2 st0 = make_float2(0.f, 0.f), st1 = make_float2(0.f, 0.f);
+      int pend = -1;                                           // stage whose bias tile is still to be written
+      const float inv_cs = 1.f / p.scale_log2e;
+      auto split3 = [](float v, uint32_t& w01, uint32_t& w2) {
+        const __nv_bfloat16 h1 = __float2bfloat16_rn(v);
+        const float r1 = v - __bfloat162float(h1);
+        const __nv_bfloat16 h2 = __float2bfloat16_rn(r1);
+        const __nv_bfloat16 h3 = __float2bfloat16_rn(r1 - __bfloat162float(h2));
+        w01 = (uint32_t)__bfloat16_as_ushort(h1) | ((uint32_t)__bfloat16_as_ushort(h2) << 16);
+        w2 = (uint32_t)__bfloat16_as_ushort(h3);
+      };
+      auto write_col = [&](uint32_t xb, int j, float2 st) {
+        uint32_t a01, a2, d01, d2;
+        split3(-st.x * inv_cs, a01, a2);
+        split3(-st.y, d01, d2);
+        const uint32_t rowa = xb + j * 128;
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(rowa + ((0 ^ (j & 7)) << 4)), "r"(a01), "r"(a2), "r"(0u) : "memory");
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(rowa + ((2 ^ (j & 7)) << 4)), "r"(d01), "r"(d2), "r"(0u) : "memory");
+      };
+      auto flush = [&]() {
+        if (MODE != 1 || pend < 0) return;
+        write_col(xb_smem(pend), lane, st0);
+        if (lane + 32 < C::NCOL) write_col(xb_smem(pend), lane + 32, st1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_full(pend));
+      };
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const Tile2 T = tile_of(t);
         const int par = Tn & 1, bl = T.b * p.L;
-        mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
-        mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
-        tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
-        tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        if (lane == 0) {
+          mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
+          mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
+          tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+          tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        }
         for (int pl = T.bl0; pl < T.bl1; ++pl)
           for (int cy = 0; cy < T.ncy; ++cy)
             for (int cx = 0; cx < T.ncx; ++cx, ++Cn) {
@@ -172,12 +222,27 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
               const uint32_t ph = (uint32_t)(Cn / C::NSTAGE) & 1u;
               const uint32_t sb = st_smem + s * C::STAGE_BYTES;
               const int gx = T.bx0 + cx * C::HX, gy = T.by0 + cy * C::CY;
-              mbar_wait(bar_empty(s), ph ^ 1u);
-              mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128);
-              tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
-              tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              if (MODE == 1) {
+                flush();
+                const float2* srow = stat + ((long long)T.b * p.H + T.h) * p.N + (long long)pl * p.Y * p.X;
+                auto fetch = [&](int j) {
+                  const int qy = gy + j / C::HX, qx = gx + j % C::HX;
+                  return (j < C::NCOL && qy < p.Y && qx < p.X) ? __ldg(srow + (long long)qy * p.X + qx) : make_float2(0.f, 0.f);
+                };
+                st0 = fetch(lane);
+                st1 = fetch(lane + 32);
+                pend = s;
+              }
+              if (lane == 0) {
+                mbar_wait(bar_empty(s), ph ^ 1u);
+                mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128);
+                tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
+                tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              }
+              if (MODE == 1) __syncwarp();                   // the stage is free: its bias tile may be rewritten
             }
       }
+      flush();
     }
   } else if (warp == 1) {
     // =========================== S'/dP' issuer ===========================
@@ -198,10 +263,13 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
           const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
+          const uint64_t dxa = smem_desc(xa_smem), dxb = smem_desc(xb_smem(s));
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) umma_ss(sd, da1 + 2 * ks, db1 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
+          if (MODE == 1) umma_ss(sd, dxa, dxb, idesc_s, 1u);                       // S'  -= lse_j / (scale log2 e)
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
+          if (MODE == 1) umma_ss(sd + 64, dxa + 2, dxb + 2, idesc_s, 1u);          // dP' -= D_j
           umma_commit(bar_sfull(buf));
           if (c == n - 1) umma_commit(bar_aempty(par));           // the operand tiles are free after these MMAs
         }
@@ -239,36 +307,13 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
     const int g = (warp - 2) >> 2;                 // group: takes the chunks whose global index has parity g
     const int sp = warp & 3;                       // TMEM subpartition of this warp
     const int row = sp * 32 + lane;                // row of the stationary tile == TMEM lane
-    const int et = ((warp - 2) & 3) * 32 + lane;   // thread index inside the group (statistics fetch)
     const uint32_t tm = tmem + ((uint32_t)(sp * 32) << 16);
     const int rx = row & 7, ry = (row >> 3) & 7, rl = row >> 6;
     const float cs = p.scale_log2e;
-    const int sr = et / C::HX, sx = et % C::HX;
-    // MODE 1: statistics of chunk `cc` of tile T (they belong to the chunk's columns)
-    auto fetch_stat = [&](const Tile2& T, int cc) -> float2 {
-      if (MODE != 1 || et >= C::NCOL) return make_float2(0.f, 0.f);
-      const int ccx = cc % T.ncx, t2 = cc / T.ncx, ccy = t2 % T.ncy, cpl = T.bl0 + t2 / T.ncy;
-      const int gy = T.by0 + ccy * C::CY + sr, gx = T.bx0 + ccx * C::HX + sx;
-      if (gy >= p.Y || gx >= p.X) return make_float2(0.f, 0.f);
-      return __ldg(&stat[((long long)T.b * p.H + T.h) * p.N + ((long long)cpl * p.Y + gy) * p.X + gx]);
-    };
 
-    int Tn = 0, Cn = 0, kg = 0;                    // kg: chunks this group has processed (statistics buffer parity)
-    int t = blockIdx.x;
-    Tile2 T = tile_of(t < ntiles ? t : 0);
-    // first chunk of this group in the stream: global index g (every tile has at least three chunks... not
-    // assumed: walk tiles until the group's chunk is found)
-    float2 next_stat = make_float2(0.f, 0.f);
-    {
-      int tt = t, c0 = g;
-      Tile2 TT = T;
-      while (tt < ntiles && c0 >= TT.nchunks) { c0 -= TT.nchunks; tt += gridDim.x; if (tt < ntiles) TT = tile_of(tt); }
-      if (tt < ntiles) next_stat = fetch_stat(TT, c0);
-    }
-    for (; t < ntiles; t += gridDim.x, ++Tn) {
-      const int par = Tn & 1;
-      const int tn = t + gridDim.x;
-      const Tile2 TNx = tile_of(tn < ntiles ? tn : t);
+    int Tn = 0, Cn = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
+      const Tile2 T = tile_of(t);
       const int x0 = T.x0, y0 = T.y0, l0 = T.l0, b = T.b, h = T.h;
       const bool active = (x0 + rx < p.X) && (y0 + ry < p.Y) && (l0 + rl < p.L);
       const int ax = min(x0 + rx, p.X - 1), ay = min(y0 + ry, p.Y - 1), al = min(l0 + rl, p.L - 1);
@@ -309,16 +354,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
               xz2[x >> 1].x = ((xm >> x) & 1u) ? 0.f : -INFINITY;
               xz2[x >> 1].y = ((xm >> (x + 1)) & 1u) ? 0.f : -INFINITY;
             }
-            const uint32_t stat_smem = stat_base + (uint32_t)(2 * g + (kg & 1)) * C::STAT_BYTES;
-            if (MODE == 1) {
-              if (et < C::NCOL)
-                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(stat_smem + (sr * 16 + sx) * 8), "f"(next_stat.x), "f"(next_stat.y) : "memory");
-              // this group's next chunk: two further in the stream, possibly in the next tile
-              if (c + 2 < T.nchunks) next_stat = fetch_stat(T, c + 2);
-              else if (tn < ntiles && c + 2 - T.nchunks < TNx.nchunks) next_stat = fetch_stat(TNx, c + 2 - T.nchunks);
-              asm volatile("bar.sync %0, 128;" ::"r"(1 + g) : "memory");
-            }
-            ++kg;
             const int buf = Cn % C::NBUF;
             const uint32_t sd = tm + C::TMEM_SD + 128 * buf;
             mbar_wait(bar_sfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
@@ -338,14 +373,8 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
                   const int col = H0 + u;                            // compile-time
                   if (col < C::NCOL) {
                     const int r = col / C::HX, x = col % C::HX;     // x even: (x, x + 1) are in the same row
-                    F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
-                    if (MODE == 1) {
-                      float4 st;
-                      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                   : "=f"(st.x), "=f"(st.y), "=f"(st.z), "=f"(st.w) : "r"(stat_smem + (r * 32 + 2 * x) * 4));
-                      nb = ffma2(F2{st.x, st.z}, F2{-1.f, -1.f}, nb);
-                      dd = F2{-st.y, -st.w};
-                    }
+                    // MODE 1: the tensor cores have already subtracted the column statistics (bias K step)
+                    const F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
                     F2 tt = ffma2(F2{__uint_as_float(svw[u]), __uint_as_float(svw[u + 1])}, F2{cs, cs}, nb);
                     tt = fadd2(tt, xz2[x >> 1]);
                     const F2 e = {ex2(tt.x), ex2(tt.y)};
@@ -440,7 +469,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           }
         }
       }
-      T = TNx;
     }
   }
 
