@@ -1,7 +1,8 @@
 // na3d_bwd_tc.cu -- entry of the tcgen05 backward (bf16, head_dim 64): step B1 of DESIGN.md as a small streaming
 // kernel, then the two persistent kernels of na3d_bwd_tc2.cu (B2-B4).  PAPER.md gives no backward; BASELINE.json
 // config 4 and SURVEY.md section 8(a) rows B1-B4 define it:
-//   B1  D_i    = sum_c dO_ic O_ic                       (bwd_stat_kernel, stored with lse * log2 e)
+//   B1  D_i    = sum_c dO_ic O_ic                       (bwd_stat_kernel, stored with lse * log2 e, and a second
+//                                                         time as the bias rows of the dK/dV kernel)
 #include "tc_common.cuh"
 #include "bwd_common.cuh"
 
@@ -12,9 +13,12 @@ using namespace tc;
 
 // B1 (+ the row statistics in the form the kernels of na3d_bwd_tc2.cu consume): stat[b][h][t] = (lse * log2 e, D),
 // D = sum_c dO_c O_c.  8 lanes per (b, token, h) row of 64 channels, rows in memory order.
+// bias[b][token][h] = 8 bf16 {a1, a2, a3, d1, d2, d3, 0, 0}: a1 + a2 + a3 = -lse / scale and d1 + d2 + d3 = -D to 24
+// bits each.  The dK/dV kernel adds them to S' = q.k and dP' = dO.v on the tensor cores (na3d_bwd_tc2.cu, MODE 1).
 __global__ void __launch_bounds__(256)
 bwd_stat_kernel(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __restrict__ d_o,
-                const float* __restrict__ lse, float2* __restrict__ stat, long long rows, long long N, int H) {
+                const float* __restrict__ lse, float2* __restrict__ stat, uint4* __restrict__ bias, float inv_scale,
+                long long rows, long long N, int H) {
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long r = gid >> 3;
   const int sub = (int)(gid & 7);
@@ -36,13 +40,25 @@ bwd_stat_kernel(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __rest
     const int h = (int)(r % H);
     const long long bt = r / H, b = bt / N, t = bt - b * N;
     const long long idx = (b * H + h) * N + t;
-    stat[idx] = make_float2(lse[idx] * 1.4426950408889634f, part);
+    const float l = lse[idx];
+    stat[idx] = make_float2(l * 1.4426950408889634f, part);
+    auto split3 = [](float v, uint32_t& h1, uint32_t& h2, uint32_t& h3) {
+      const __nv_bfloat16 b1 = __float2bfloat16_rn(v);
+      const float r1 = v - __bfloat162float(b1);
+      const __nv_bfloat16 b2 = __float2bfloat16_rn(r1);
+      const __nv_bfloat16 b3 = __float2bfloat16_rn(r1 - __bfloat162float(b2));
+      h1 = __bfloat16_as_ushort(b1); h2 = __bfloat16_as_ushort(b2); h3 = __bfloat16_as_ushort(b3);
+    };
+    uint32_t a1, a2, a3, d1, d2, d3;
+    split3(-l * inv_scale, a1, a2, a3);
+    split3(-part, d1, d2, d3);
+    bias[r] = make_uint4(a1 | (a2 << 16), a3 | (d1 << 16), d2 | (d3 << 16), 0u);
   }
 }
 
 }  // namespace
 cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
-                                const void* stat, const void* rtab, void* dq, void* dk, void* dv,
+                                const void* stat, const void* bias, const void* rtab, void* dq, void* dk, void* dv,
                                 cudaStream_t stream, int* launches);
 // Shapes the tensor-core backward covers: bf16, head_dim 64, the windows below.
 #define STRATA_BWD_CONFIGS(X) \
@@ -68,12 +84,15 @@ cudaError_t launch_bwd_tc(const Problem& p, const void* qr, const void* kr, cons
   const long long rows = p.rows(), sgrid = (rows * 8 + 255) / 256;
   if (sgrid > 0x7fffffffLL) return cudaErrorInvalidValue;
   prof_begin("na3d_bwd_stat", stream);
-  bwd_stat_kernel<<<(unsigned)sgrid, 256, 0, stream>>>((const __nv_bfloat16*)o, (const __nv_bfloat16*)d_o, lse, (float2*)stat, rows, p.N, p.H);
+  // `stat` holds both arrays: float2 per row, then (256-byte aligned) the 16-byte bias rows
+  uint4* bias = reinterpret_cast<uint4*>(reinterpret_cast<char*>(stat) + (((size_t)rows * 8 + 255) & ~(size_t)255));
+  bwd_stat_kernel<<<(unsigned)sgrid, 256, 0, stream>>>((const __nv_bfloat16*)o, (const __nv_bfloat16*)d_o, lse, (float2*)stat, bias,
+                                                       1.f / p.scale, rows, p.N, p.H);
   prof_end(stream);
   if (launches) *launches += 1;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  return launch_bwd_tc2_main(p, qr, kr, v, d_o_main, (float2*)stat, rtab, dq, dk, dv, stream, launches);
+  return launch_bwd_tc2_main(p, qr, kr, v, d_o_main, (float2*)stat, bias, rtab, dq, dk, dv, stream, launches);
 }
 
 }  // namespace strata

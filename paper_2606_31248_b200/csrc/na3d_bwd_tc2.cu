@@ -13,11 +13,13 @@
 //       not symmetric at the borders): B1 = Qrot, B2 = dO.  acc1 = dKrot = sum dS^T B1,
 //       acc2 = dV = sum P^T B2.  The statistics (lse, D) belong to the chunk's COLUMNS here, and a per-column
 //       bias is a rank-one term, so the tensor cores add it: S' and dP' get a fifth K step whose A operand is a
-//       constant tile of ones (three channels) and whose B operand holds, for column j, -lse_j / (scale log2 e)
-//       resp. -D_j split into three bf16 terms (24 significant bits, the sum is exact in the fp32 accumulator).
-//       The producer warp writes that small B tile next to the chunk it streams.  (Reading the statistics from
-//       shared memory in the elementwise loop instead cost 28 loads per chunk and thread, each waiting behind the
-//       tensor cores' own operand reads: profiles/r2_bwd_cfg4.md.)
+//       constant tile (ones in three channels) and whose B operand holds, for column j, -lse_j / scale resp. -D_j
+//       split into three bf16 terms (24 significant bits, the sum is exact in the fp32 accumulator).  bwd_stat_kernel
+//       writes those 16-byte bias rows per (token, head); one more TMA box per chunk brings them in, unswizzled,
+//       which is the K-major core-matrix layout of an UMMA operand as it stands (8 rows x 16 bytes contiguous).
+//       (Reading the statistics from shared memory in the elementwise loop cost 28 loads per chunk and thread, each
+//       waiting behind the tensor cores' own operand reads; building the bias rows in the producer warp made that
+//       warp the bottleneck at ~190 dependent instructions per chunk: profiles/r2_bwd_cfg4.md.)
 // Per chunk (CY rows x HX columns of one level plane = N <= 64 columns):
 //   S' = A1 B1^T and dP' = A2 B2^T on the tensor cores (M = 128, K = 64) -> TMEM;
 //   one row per thread: p = 2^(S' scale log2e - lse log2e) under the window mask, dS = p (dP' - D),
@@ -36,10 +38,11 @@
 //     of tile t + 1 overlap the MMAs of tile t + 1.
 // TMEM (512 columns): accumulators [0, 128) -- MODE 0: acc1 double buffered by tile parity, MODE 1: {acc1, acc2}
 // once -- | SD[buf] = {S' -> P, dP' -> dS} at 128 + 128 * buf, buf < 3 (chunk index mod 3).
-// Warps (352 threads): 0 TMA producer, 1 S'/dP' MMA issuer + TMEM owner, 2-5 elementwise group 0, 6-9 group 1,
-// 10 gradient-MMA issuer.
-// Group g takes the chunks of global index parity g; in the epilogue group 0 writes acc1 (dQ or dK,
-// un-rotated), group 1 writes acc2 (dV, MODE 1 only).
+// Warps (512 threads): 0 TMA producer, 1 S'/dP' MMA issuer + TMEM owner, 2 gradient-MMA issuer, 3 idle,
+// 4-7 elementwise group 0, 8-11 group 1 (group g takes the chunks of global index parity g), 12-15 epilogue
+// (acc1 -> dQ or dK, un-rotated; acc2 -> dV in MODE 1).  The epilogue has warps of its own because its table loads
+// and stores take about as long as half a tile's elementwise work: done by an elementwise group, it held back that
+// group's chunks of the next tile, and with them the MMAs (profiles/r2_bwd_cfg4.md).
 #include <type_traits>
 
 #include "tc_common.cuh"
@@ -61,7 +64,9 @@ struct Bwd2Cfg {
   static constexpr int TILE_BYTES = M * 128, CHUNK_BYTES = N * 128;
   static constexpr int STAGE_BYTES = 2 * CHUNK_BYTES;              // B1 | B2
   static constexpr int NSTAGE = 4;
-  static constexpr int XTRA_BYTES = TILE_BYTES + NSTAGE * CHUNK_BYTES;   // MODE 1: ones tile | per-stage bias tiles
+  static constexpr int BIAS_BYTES = N * 16;                        // bias rows of a chunk: [N columns][8 bf16]
+  static constexpr int XTRA_BYTES = TILE_BYTES + NSTAGE * 1024 + 1024;   // MODE 1: ones tile | per-stage bias rows | zeros
+  static_assert(BIAS_BYTES <= 1024, "bias rows of a chunk");
   static constexpr int NBUF = 3;                                   // S'/dP' buffers in TMEM
   static constexpr int TMEM_ACC = 0, TMEM_SD = 128, TMEM_COLS = 512;
   static constexpr int NBARS = 4 + 2 * NSTAGE + 3 * NBUF + 4;
@@ -71,7 +76,7 @@ struct Bwd2Cfg {
   static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
-constexpr int kBwd2Threads = 352;
+constexpr int kBwd2Threads = 512;
 
 // Geometry of one stationary tile and of its streamed box.
 struct Tile2 {
@@ -86,7 +91,7 @@ template <class C, int MODE>
 __global__ void __launch_bounds__(kBwd2Threads, 1)
 na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_constant__ CUtensorMap tm_a2,
                     const __grid_constant__ CUtensorMap tm_b1, const __grid_constant__ CUtensorMap tm_b2,
-                    const float2* __restrict__ stat, const float4* __restrict__ rtab,
+                    const __grid_constant__ CUtensorMap tm_bias, const float2* __restrict__ stat, const float4* __restrict__ rtab,
                     __nv_bfloat16* __restrict__ out1, __nv_bfloat16* __restrict__ out2, const BwdParams p,
                     const int ntiles) {
   extern __shared__ uint8_t smem_raw[];
@@ -95,7 +100,8 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   auto a_smem = [&](int par, int which) { return base + (uint32_t)(2 * par + which) * C::TILE_BYTES; };
   const uint32_t st_smem = base + 4 * C::TILE_BYTES;                       // stages
   const uint32_t xa_smem = st_smem + C::NSTAGE * C::STAGE_BYTES;           // MODE 1: A operand of the bias K step
-  auto xb_smem = [&](int s) { return xa_smem + C::TILE_BYTES + (uint32_t)s * C::CHUNK_BYTES; };   // its B operand
+  auto xb_smem = [&](int s) { return xa_smem + C::TILE_BYTES + (uint32_t)s * 1024; };             // its B operand
+  const uint32_t xz_smem = xb_smem(C::NSTAGE);                             // zeros: channels 8-15 of every bias row
   const uint32_t bars = xa_smem + C::XTRA_BYTES;
   auto bar_afull = [&](int par) { return bars + 8u * par; };               // TMA -> MMA: operand tiles of a tile
   auto bar_aempty = [&](int par) { return bars + 8u * (2 + par); };        // last S'/dP' MMA of the tile -> TMA
@@ -136,13 +142,13 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   // ---- one-time setup
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tm_a1); tma_prefetch_desc(&tm_a2); tma_prefetch_desc(&tm_b1); tma_prefetch_desc(&tm_b2);
+    if (MODE == 1) tma_prefetch_desc(&tm_bias);
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_afull(i), 1); mbar_init(bar_aempty(i), 1);
-      mbar_init(bar_accdone(i), 1); mbar_init(bar_accfree(i), MODE == 1 ? 8 : 4);
+      mbar_init(bar_accdone(i), 1); mbar_init(bar_accfree(i), 4);
     }
     for (int i = 0; i < C::NBUF; ++i) { mbar_init(bar_sfull(i), 1); mbar_init(bar_pfull(i), 4); mbar_init(bar_sdfree(i), 1); }
-    // MODE 1: a chunk is complete when its TMA bytes have landed AND its bias tile is written
-    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), MODE == 1 ? 2 : 1); mbar_init(bar_empty(s), 1); }
+    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
@@ -157,13 +163,16 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   if (MODE == 1) {
-    // bias K step: row r of the ones tile has 1, 1, 1 in channels 0-2 and 16-18 (16-byte chunks 0 and 2 of the
-    // 128-byte swizzled row); the bias tiles start as zeros and only chunks 0 and 2 of a row are ever rewritten
+    // bias K step, A operand (128-byte swizzled rows like the other tiles): row r has ones in channels 0-2 (K step 0:
+    // picks the lse terms of a bias row) and in channels 16 + 3..5 (K step 1: picks the D terms); everything else,
+    // the zeros block and the pad rows of the bias stages start as zeros
     for (int u = threadIdx.x; u < C::XTRA_BYTES / 16; u += kBwd2Threads) {
       const int r = u >> 3, ch = (u & 7) ^ (r & 7);
-      const bool one = u < C::TILE_BYTES / 16 && (ch == 0 || ch == 2);
-      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(xa_smem + u * 16), "r"(one ? 0x3F803F80u : 0u),
-                   "r"(one ? 0x00003F80u : 0u), "r"(0u) : "memory");
+      const bool tile = u < C::TILE_BYTES / 16;
+      uint32_t w0 = 0u, w1 = 0u, w2 = 0u;
+      if (tile && ch == 0) { w0 = 0x3F803F80u; w1 = 0x00003F80u; }
+      if (tile && ch == 2) { w1 = 0x3F800000u; w2 = 0x3F803F80u; }
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(xa_smem + u * 16), "r"(w0), "r"(w1), "r"(w2), "r"(0u) : "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -171,50 +180,23 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot_ptr;
+  // registers: the kernel is compiled for 128 per thread (512 threads); the control warpgroup (72) hands the rest to
+  // the elementwise warpgroups (144) and the epilogue warpgroup (152)
+  // (each setmaxnreg sits at the head of its own branch: ptxas budgets the code a setmaxnreg dominates)
 
+  if (warp < 4) {
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
   if (warp == 0) {
-    // =========================== TMA producer (MODE 1: and the bias tiles) ===========================
-    // MODE 1, all lanes: lane j owns columns j and j + 32 of a chunk.  Their statistics are loaded before the wait
-    // for the chunk's stage and turned into the bias tile at the start of the NEXT iteration, so the global load
-    // hides behind that wait; the chunk's `full` barrier takes one arrival from the TMA and one from here.
-    if (lane == 0 || MODE == 1) {
+    // =========================== TMA producer ===========================
+    if (lane == 0) {
       int Tn = 0, Cn = 0;
-      float2 st0 = make_float2(0.f, 0.f), st1 = make_float2(0.f, 0.f);
-      int pend = -1;                                           // stage whose bias tile is still to be written
-      const float inv_cs = 1.f / p.scale_log2e;
-      auto split3 = [](float v, uint32_t& w01, uint32_t& w2) {
-        const __nv_bfloat16 h1 = __float2bfloat16_rn(v);
-        const float r1 = v - __bfloat162float(h1);
-        const __nv_bfloat16 h2 = __float2bfloat16_rn(r1);
-        const __nv_bfloat16 h3 = __float2bfloat16_rn(r1 - __bfloat162float(h2));
-        w01 = (uint32_t)__bfloat16_as_ushort(h1) | ((uint32_t)__bfloat16_as_ushort(h2) << 16);
-        w2 = (uint32_t)__bfloat16_as_ushort(h3);
-      };
-      auto write_col = [&](uint32_t xb, int j, float2 st) {
-        uint32_t a01, a2, d01, d2;
-        split3(-st.x * inv_cs, a01, a2);
-        split3(-st.y, d01, d2);
-        const uint32_t rowa = xb + j * 128;
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(rowa + ((0 ^ (j & 7)) << 4)), "r"(a01), "r"(a2), "r"(0u) : "memory");
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(rowa + ((2 ^ (j & 7)) << 4)), "r"(d01), "r"(d2), "r"(0u) : "memory");
-      };
-      auto flush = [&]() {
-        if (MODE != 1 || pend < 0) return;
-        write_col(xb_smem(pend), lane, st0);
-        if (lane + 32 < C::NCOL) write_col(xb_smem(pend), lane + 32, st1);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_full(pend));
-      };
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const Tile2 T = tile_of(t);
         const int par = Tn & 1, bl = T.b * p.L;
-        if (lane == 0) {
-          mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
-          mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
-          tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
-          tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
-        }
+        mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
+        mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
+        tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
         for (int pl = T.bl0; pl < T.bl1; ++pl)
           for (int cy = 0; cy < T.ncy; ++cy)
             for (int cx = 0; cx < T.ncx; ++cx, ++Cn) {
@@ -222,27 +204,13 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
               const uint32_t ph = (uint32_t)(Cn / C::NSTAGE) & 1u;
               const uint32_t sb = st_smem + s * C::STAGE_BYTES;
               const int gx = T.bx0 + cx * C::HX, gy = T.by0 + cy * C::CY;
-              if (MODE == 1) {
-                flush();
-                const float2* srow = stat + ((long long)T.b * p.H + T.h) * p.N + (long long)pl * p.Y * p.X;
-                auto fetch = [&](int j) {
-                  const int qy = gy + j / C::HX, qx = gx + j % C::HX;
-                  return (j < C::NCOL && qy < p.Y && qx < p.X) ? __ldg(srow + (long long)qy * p.X + qx) : make_float2(0.f, 0.f);
-                };
-                st0 = fetch(lane);
-                st1 = fetch(lane + 32);
-                pend = s;
-              }
-              if (lane == 0) {
-                mbar_wait(bar_empty(s), ph ^ 1u);
-                mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128);
-                tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
-                tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
-              }
-              if (MODE == 1) __syncwarp();                   // the stage is free: its bias tile may be rewritten
+              mbar_wait(bar_empty(s), ph ^ 1u);
+              mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128 + (MODE == 1 ? C::NCOL * 16 : 0));
+              tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              if (MODE == 1) tma_load_5d(xb_smem(s), &tm_bias, bar_full(s), 0, T.h, gx, gy, bl + pl);
             }
       }
-      flush();
     }
   } else if (warp == 1) {
     // =========================== S'/dP' issuer ===========================
@@ -263,19 +231,23 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
           const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
-          const uint64_t dxa = smem_desc(xa_smem), dxb = smem_desc(xb_smem(s));
+          // bias rows: unswizzled K-major operand -- 8 columns x 16 bytes per core matrix, the next 8 columns 128 bytes on
+          // (stride offset), channels 8-15 in the zeros block (leading offset)
+          const uint64_t dxa = smem_desc(xa_smem);
+          const uint64_t dxb = (uint64_t)((xb_smem(s) >> 4) & 0x3FFF) | ((uint64_t)((xz_smem - xb_smem(s)) >> 4) << 16) |
+                               ((uint64_t)(128 >> 4) << 32) | (1ull << 46);
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) umma_ss(sd, da1 + 2 * ks, db1 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
-          if (MODE == 1) umma_ss(sd, dxa, dxb, idesc_s, 1u);                       // S'  -= lse_j / (scale log2 e)
+          if (MODE == 1) umma_ss(sd, dxa, dxb, idesc_s, 1u);                       // S'  -= lse_j / scale
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
-          if (MODE == 1) umma_ss(sd + 64, dxa + 2, dxb + 2, idesc_s, 1u);          // dP' -= D_j
+          if (MODE == 1) umma_ss(sd + 64, dxa + 2, dxb, idesc_s, 1u);              // dP' -= D_j
           umma_commit(bar_sfull(buf));
           if (c == n - 1) umma_commit(bar_aempty(par));           // the operand tiles are free after these MMAs
         }
       }
     }
-  } else if (warp == 10) {
+  } else if (warp == 2) {
     // =========================== gradient-MMA issuer ===========================
     if (lane == 0) {
       constexpr uint32_t idesc_acc = instr_desc(C::M, 64, true);
@@ -302,9 +274,11 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
         }
       }
     }
-  } else {
-    // =========================== elementwise group g (one row per thread) + epilogue ===========================
-    const int g = (warp - 2) >> 2;                 // group: takes the chunks whose global index has parity g
+  }
+  } else if (warp < 12) {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 144;");
+    // =========================== elementwise group g (one row per thread) ===========================
+    const int g = (warp - 4) >> 2;                 // group: takes the chunks whose global index has parity g
     const int sp = warp & 3;                       // TMEM subpartition of this warp
     const int row = sp * 32 + lane;                // row of the stationary tile == TMEM lane
     const uint32_t tm = tmem + ((uint32_t)(sp * 32) << 16);
@@ -406,67 +380,76 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
             if (lane == 0) mbar_arrive(bar_pfull(buf));
           }
       }
-      // ---- epilogue of this tile (overlaps the next tile's chunks, which the other warps are already on):
-      // group 0: dx = R(-phi) (scale * acc1) -> bf16 (B4 fused); group 1 (MODE 1): acc2 -> bf16 dV
-      if (g == 0 || MODE == 1) {
-        const int ai = Tn % NACC, ak = Tn / NACC;
-        mbar_wait(bar_accdone(ai), (uint32_t)ak & 1u);
-        tc_fence_after();
-        const uint32_t acc = tm + C::TMEM_ACC + ACC_STRIDE * ai;
-        if (g == 0) {
-          __nv_bfloat16* r1 = out1 + (((long long)b * p.N + tok) * p.H + h) * C::D;
-          const float4* trow = rtab ? rtab + ((long long)b * p.N + tok) * (C::D / 4) : nullptr;   // 2 pairs per float4
-          float av[C::D];
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+    // =========================== epilogue warps (one row per thread) ===========================
+    // dx = R(-phi) (scale * acc1) -> bf16 (B4 fused); MODE 1 also acc2 -> bf16 dV.  The accumulators are given back
+    // as soon as they are in registers; the table loads and the stores of tile t run under the chunks of tile t + 1.
+    const int sp = warp & 3, row = sp * 32 + lane;
+    const uint32_t tm = tmem + ((uint32_t)(sp * 32) << 16);
+    const int rx = row & 7, ry = (row >> 3) & 7, rl = row >> 6;
+    int Tn = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
+      int bid = t;
+      const int x0 = (bid % p.ntx) * C::TX; bid /= p.ntx;
+      const int y0 = (bid % p.nty) * C::TY; bid /= p.nty;
+      const int l0 = (bid % p.ntl) * C::TL; bid /= p.ntl;
+      const int h = bid % p.H, b = bid / p.H;
+      const bool active = (x0 + rx < p.X) && (y0 + ry < p.Y) && (l0 + rl < p.L);
+      const int ax = min(x0 + rx, p.X - 1), ay = min(y0 + ry, p.Y - 1), al = min(l0 + rl, p.L - 1);
+      const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
+      const int ai = Tn % NACC, ak = Tn / NACC;
+      mbar_wait(bar_accdone(ai), (uint32_t)ak & 1u);
+      tc_fence_after();
+      const uint32_t acc = tm + C::TMEM_ACC + ACC_STRIDE * ai;
+      uint32_t vw[MODE == 1 ? C::D / 2 : 1];
+      if (MODE == 1) {
+        float av[C::D];
 #pragma unroll
-          for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + j, *reinterpret_cast<float(*)[16]>(&av[j]));
-          tmem_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_accfree(ai));            // acc1 is in registers
+        for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + 64 + j, *reinterpret_cast<float(*)[16]>(&av[j]));
+        tmem_wait_ld();
 #pragma unroll
-          for (int j = 0; j < C::D; ++j) av[j] *= p.scale;
-          if (active) {
-            if (trow) {
-              auto rot = [&](auto half_pairing) {
-                constexpr bool HP = decltype(half_pairing)::value;
+        for (int j = 0; j < C::D; j += 2) vw[j >> 1] = pack_bf16(av[j], av[j + 1]);
+      }
+      float av[C::D];
 #pragma unroll
-                for (int m = 0; m < C::D / 2; m += 2) {               // pairs m, m + 1
-                  const float4 tq = __ldg(trow + (m >> 1));           // (cos m, sin m, cos m+1, sin m+1)
-                  const int a0 = HP ? m : 2 * m, b0 = HP ? m + C::D / 2 : 2 * m + 1;
-                  const int a1 = HP ? m + 1 : 2 * m + 2, b1 = HP ? m + 1 + C::D / 2 : 2 * m + 3;
-                  const float xa0 = av[a0], xb0 = av[b0], xa1 = av[a1], xb1 = av[b1];
-                  av[a0] = fmaf(xb0, tq.y, xa0 * tq.x); av[b0] = fmaf(-xa0, tq.y, xb0 * tq.x);
-                  av[a1] = fmaf(xb1, tq.w, xa1 * tq.z); av[b1] = fmaf(-xa1, tq.w, xb1 * tq.z);
-                }
-              };
-              if (p.pairing) rot(std::true_type{}); else rot(std::false_type{});
+      for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + j, *reinterpret_cast<float(*)[16]>(&av[j]));
+      tmem_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_accfree(ai));              // the accumulators are in registers
+      if (MODE == 1 && active) {
+        uint4* r2 = reinterpret_cast<uint4*>(out2 + (((long long)b * p.N + tok) * p.H + h) * C::D);
+#pragma unroll
+        for (int j = 0; j < C::D / 8; ++j) r2[j] = make_uint4(vw[4 * j], vw[4 * j + 1], vw[4 * j + 2], vw[4 * j + 3]);
+      }
+      if (active) {
+        __nv_bfloat16* r1 = out1 + (((long long)b * p.N + tok) * p.H + h) * C::D;
+        const float4* trow = rtab ? rtab + ((long long)b * p.N + tok) * (C::D / 4) : nullptr;   // 2 pairs per float4
+#pragma unroll
+        for (int j = 0; j < C::D; ++j) av[j] *= p.scale;
+        if (trow) {
+          auto rot = [&](auto half_pairing) {
+            constexpr bool HP = decltype(half_pairing)::value;
+#pragma unroll
+            for (int m = 0; m < C::D / 2; m += 2) {               // pairs m, m + 1
+              const float4 tq = __ldg(trow + (m >> 1));           // (cos m, sin m, cos m+1, sin m+1)
+              const int a0 = HP ? m : 2 * m, b0 = HP ? m + C::D / 2 : 2 * m + 1;
+              const int a1 = HP ? m + 1 : 2 * m + 2, b1 = HP ? m + 1 + C::D / 2 : 2 * m + 3;
+              const float xa0 = av[a0], xb0 = av[b0], xa1 = av[a1], xb1 = av[b1];
+              av[a0] = fmaf(xb0, tq.y, xa0 * tq.x); av[b0] = fmaf(-xa0, tq.y, xb0 * tq.x);
+              av[a1] = fmaf(xb1, tq.w, xa1 * tq.z); av[b1] = fmaf(-xa1, tq.w, xb1 * tq.z);
             }
+          };
+          if (p.pairing) rot(std::true_type{}); else rot(std::false_type{});
+        }
 #pragma unroll
-            for (int j = 0; j < C::D; j += 8) {
-              uint4 w;
-              w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
-              w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
-              reinterpret_cast<uint4*>(r1)[j >> 3] = w;
-            }
-          }
-        } else {
-          __nv_bfloat16* r2 = out2 + (((long long)b * p.N + tok) * p.H + h) * C::D;
-          float av[C::D];
-#pragma unroll
-          for (int j = 0; j < C::D; j += 16) tmem_ld16(acc + 64 + j, *reinterpret_cast<float(*)[16]>(&av[j]));
-          tmem_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_accfree(ai));            // acc2 is in registers
-          if (active) {
-#pragma unroll
-            for (int j = 0; j < C::D; j += 8) {
-              uint4 w;
-              w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
-              w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
-              reinterpret_cast<uint4*>(r2)[j >> 3] = w;
-            }
-          }
+        for (int j = 0; j < C::D; j += 8) {
+          uint4 w;
+          w.x = pack_bf16(av[j], av[j + 1]);     w.y = pack_bf16(av[j + 2], av[j + 3]);
+          w.z = pack_bf16(av[j + 4], av[j + 5]); w.w = pack_bf16(av[j + 6], av[j + 7]);
+          reinterpret_cast<uint4*>(r1)[j >> 3] = w;
         }
       }
     }
@@ -486,8 +469,22 @@ std::mutex g_mu;
 
 template <class C>
 cudaError_t launch_bwd2_cfg(int slot, const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
-                            const float2* stat, const void* rtab, void* dq, void* dk, void* dv,
+                            const float2* stat, const void* bias, const void* rtab, void* dq, void* dk, void* dv,
                             cudaStream_t stream, int* launches) {
+  // bias rows [B*L, Y, X, H, 8] bf16, unswizzled boxes of one head x (HX, CY) tokens
+  CUtensorMap t_bias;
+  {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return cudaErrorInvalidValue;
+    const cuuint64_t dims[5] = {8, (cuuint64_t)p.H, (cuuint64_t)p.X, (cuuint64_t)p.Y, (cuuint64_t)p.B * (cuuint64_t)p.L};
+    const cuuint64_t strides[4] = {16, (cuuint64_t)p.H * 16, (cuuint64_t)p.X * p.H * 16, (cuuint64_t)p.Y * p.X * p.H * 16};
+    const cuuint32_t box[5] = {8, 1, (cuuint32_t)C::HX, (cuuint32_t)C::CY, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    if (fn(&t_bias, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(bias), dims, strides, box, estr,
+           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
   CUtensorMap tq_t, tdo_t, tk_c, tv_c, tk_t, tv_t, tq_c, tdo_c;
   if (!make_map(&tq_t, qr, p, C::TX, C::TY, C::TL) || !make_map(&tdo_t, d_o, p, C::TX, C::TY, C::TL) ||
       !make_map(&tk_c, kr, p, C::HX, C::CY, 1) || !make_map(&tv_c, v, p, C::HX, C::CY, 1) ||
@@ -507,11 +504,11 @@ cudaError_t launch_bwd2_cfg(int slot, const Problem& p, const void* qr, const vo
   if (e == cudaSuccess) e = ensure_smem_attr(ds, g_mu, 2 * slot + 1, na3d_bwd_tc2_kernel<C, 1>, C::SMEM_BYTES);
   if (e != cudaSuccess) return e;
   prof_begin("na3d_bwd_dq_tcgen05", stream);
-  na3d_bwd_tc2_kernel<C, 0><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, stat, (const float4*)rtab,
+  na3d_bwd_tc2_kernel<C, 0><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tq_t, tdo_t, tk_c, tv_c, t_bias, stat, (const float4*)rtab,
                                                                           (__nv_bfloat16*)dq, nullptr, bp, (int)ntiles);
   prof_end(stream);
   prof_begin("na3d_bwd_dkdv_tcgen05", stream);
-  na3d_bwd_tc2_kernel<C, 1><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tk_t, tv_t, tq_c, tdo_c, stat, (const float4*)rtab,
+  na3d_bwd_tc2_kernel<C, 1><<<grid, kBwd2Threads, C::SMEM_BYTES, stream>>>(tk_t, tv_t, tq_c, tdo_c, t_bias, stat, (const float4*)rtab,
                                                                           (__nv_bfloat16*)dk, (__nv_bfloat16*)dv, bp, (int)ntiles);
   prof_end(stream);
   if (launches) *launches += 2;
@@ -522,11 +519,11 @@ cudaError_t launch_bwd2_cfg(int slot, const Problem& p, const void* qr, const vo
 
 // The two main kernels of the backward in their persistent form; false if the window is not instantiated.
 cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr, const void* v, const void* d_o,
-                                const void* stat, const void* rtab, void* dq, void* dk, void* dv,
+                                const void* stat, const void* bias, const void* rtab, void* dq, void* dk, void* dv,
                                 cudaStream_t stream, int* launches) {
 #define X(I_, KL_, KY_, KX_)                                   \
   if (p.kL == KL_ && p.kY == KY_ && p.kX == KX_)                \
-    return launch_bwd2_cfg<Bwd2Cfg<KL_, KY_, KX_>>(I_, p, qr, kr, v, d_o, (const float2*)stat, rtab, dq, dk, dv, stream, launches);
+    return launch_bwd2_cfg<Bwd2Cfg<KL_, KY_, KX_>>(I_, p, qr, kr, v, d_o, (const float2*)stat, bias, rtab, dq, dk, dv, stream, launches);
   X(0, 3, 7, 7)
   X(1, 3, 5, 5)
   X(2, 3, 3, 3)

@@ -79,8 +79,8 @@ struct Carve {
 size_t ws_bytes(const Problem& p, Path path, bool backward) {
   const size_t e = (size_t)p.elems();
   const size_t stat = align_up((size_t)p.B * p.H * p.N * 4);
-  if (backward && path == PATH_TC_PREROT)                               // qr, kr (bf16), stat (float2), fp32 rotary table
-    return 2 * align_up(e * 2) + align_up(2 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
+  if (backward && path == PATH_TC_PREROT)               // qr, kr (bf16), stat (float2) + bias rows (16 B), fp32 rotary table
+    return 2 * align_up(e * 2) + align_up(6 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
   if (path == PATH_TC_PLANE || path == PATH_COLUMN) return align_up(strata::plane_fwd_workspace_bytes());
   if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
@@ -275,7 +275,7 @@ static strata_status_t bwd_impl(const strata_na3d_desc_t* desc, const void* q, c
   if (path == PATH_TC_PREROT) {
     void* qr = ws.take<char>(eb / 2);
     void* kr = ws.take<char>(eb / 2);
-    void* stat = ws.take<char>(2 * align_up(stat_bytes(p)));
+    void* stat = ws.take<char>(6 * align_up(stat_bytes(p)));
     void* rtab = ws.take<char>((size_t)p.B * p.N * (p.D / 2) * 8);
     e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
