@@ -53,6 +53,8 @@ cudaError_t launch_rope_rotate(const Problem& p, const void* x0, const void* x1,
                                const float* freqs, float sign, cudaStream_t stream, int* launches);
 
 // rope.cu: A1 as an fp32 table [B, L, Y, X, D/2] float2 (cos, sin), for the backward epilogues (B4).
+cudaError_t launch_rope_rotate_table(const Problem& p, const void* x0, const void* x1, void* y0, void* y1,
+                                     const void* table, float sign, cudaStream_t stream, int* launches);
 cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* coords, const float* freqs,
                                   cudaStream_t stream, int* launches);
 

@@ -147,7 +147,86 @@ rope_table_f32_kernel(float2* __restrict__ table, const float* __restrict__ coor
   table[gid] = make_float2(cs, sn);
 }
 
+// A2 from that table, bf16 -> bf16: one thread per ((token, head) row, group of 8 channels) and tensor pair, every access
+// 16 bytes and all of a thread's loads independent (the per-token loop over heads of rope_rotate_bf16_kernel keeps two
+// loads in flight per thread and ran at a fifth of the HBM rate).  The table rows of a token are re-read by its H
+// heads out of L1.  PAIR 0: group = pairs 4g .. 4g + 3.  PAIR 1: group = pairs 8g .. 8g + 7 (two 16-byte halves).
+template <int PAIR>
+__global__ void __launch_bounds__(256)
+rope_rotate_table_bf16_kernel(const __nv_bfloat16* __restrict__ x0, const __nv_bfloat16* __restrict__ x1,
+                              __nv_bfloat16* __restrict__ y0, __nv_bfloat16* __restrict__ y1,
+                              const float4* __restrict__ table, long long rows, int H, int D, float sign) {
+  constexpr int NP = PAIR ? 8 : 4;
+  const int half = D >> 1, groups = half / NP;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= rows * groups) return;
+  const long long r = gid / groups, t = r / H;
+  const int g = (int)(gid - r * groups);
+  const long long base = r * (long long)D;
+  const float4* trow = table + (t * half + NP * g) / 2;              // (cos, sin) x 2 per float4
+  float cs[NP], sn[NP];
+#pragma unroll
+  for (int u = 0; u < NP; u += 2) {
+    const float4 c = __ldg(trow + (u >> 1));
+    cs[u] = c.x; sn[u] = c.y * sign; cs[u + 1] = c.z; sn[u + 1] = c.w * sign;
+  }
+  uint4 va[2], vb[2];
+#pragma unroll
+  for (int which = 0; which < 2; ++which) {
+    const __nv_bfloat16* x = which ? x1 : x0;
+    if (x == nullptr) continue;
+    va[which] = *reinterpret_cast<const uint4*>(x + base + 8 * g);
+    if (PAIR) vb[which] = *reinterpret_cast<const uint4*>(x + base + half + 8 * g);
+  }
+#pragma unroll
+  for (int which = 0; which < 2; ++which) {
+    __nv_bfloat16* y = which ? y1 : y0;
+    if ((which ? x1 : x0) == nullptr) continue;
+    uint32_t wa[4] = {va[which].x, va[which].y, va[which].z, va[which].w};
+    if (PAIR == 0) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float2 ab = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[u]));
+        const __nv_bfloat162 r2 = __floats2bfloat162_rn(ab.x * cs[u] - ab.y * sn[u], ab.x * sn[u] + ab.y * cs[u]);
+        wa[u] = *reinterpret_cast<const uint32_t*>(&r2);
+      }
+      *reinterpret_cast<uint4*>(y + base + 8 * g) = make_uint4(wa[0], wa[1], wa[2], wa[3]);
+    } else {
+      uint32_t wb[4] = {vb[which].x, vb[which].y, vb[which].z, vb[which].w};
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[u]));
+        const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[u]));
+        const __nv_bfloat162 ra = __floats2bfloat162_rn(a2.x * cs[2 * u] - b2.x * sn[2 * u], a2.y * cs[2 * u + 1] - b2.y * sn[2 * u + 1]);
+        const __nv_bfloat162 rb = __floats2bfloat162_rn(a2.x * sn[2 * u] + b2.x * cs[2 * u], a2.y * sn[2 * u + 1] + b2.y * cs[2 * u + 1]);
+        wa[u] = *reinterpret_cast<const uint32_t*>(&ra);
+        wb[u] = *reinterpret_cast<const uint32_t*>(&rb);
+      }
+      *reinterpret_cast<uint4*>(y + base + 8 * g) = make_uint4(wa[0], wa[1], wa[2], wa[3]);
+      *reinterpret_cast<uint4*>(y + base + half + 8 * g) = make_uint4(wb[0], wb[1], wb[2], wb[3]);
+    }
+  }
+}
+
 }  // namespace
+
+// bf16 -> bf16 rotation of one or two tensors from the fp32 table of launch_rope_table_f32 (head_dim % 16 == 0).
+cudaError_t launch_rope_rotate_table(const Problem& p, const void* x0, const void* x1, void* y0, void* y1,
+                                     const void* table, float sign, cudaStream_t stream, int* launches) {
+  if (p.D % 16 != 0) return cudaErrorInvalidValue;
+  const long long rows = p.rows(), threads = rows * (p.D / 2 / (p.pairing ? 8 : 4)), grid = (threads + 255) / 256;
+  if (grid <= 0 || grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+  prof_begin(sign > 0 ? "rope_rotate" : "rope_unrotate", stream);
+  if (p.pairing)
+    rope_rotate_table_bf16_kernel<1><<<(unsigned)grid, 256, 0, stream>>>((const __nv_bfloat16*)x0, (const __nv_bfloat16*)x1,
+        (__nv_bfloat16*)y0, (__nv_bfloat16*)y1, (const float4*)table, rows, p.H, p.D, sign);
+  else
+    rope_rotate_table_bf16_kernel<0><<<(unsigned)grid, 256, 0, stream>>>((const __nv_bfloat16*)x0, (const __nv_bfloat16*)x1,
+        (__nv_bfloat16*)y0, (__nv_bfloat16*)y1, (const float4*)table, rows, p.H, p.D, sign);
+  prof_end(stream);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* coords, const float* freqs,
                                   cudaStream_t stream, int* launches) {

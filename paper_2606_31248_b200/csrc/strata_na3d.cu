@@ -277,12 +277,13 @@ static strata_status_t bwd_impl(const strata_na3d_desc_t* desc, const void* q, c
     void* kr = ws.take<char>(eb / 2);
     void* stat = ws.take<char>(6 * align_up(stat_bytes(p)));
     void* rtab = ws.take<char>((size_t)p.B * p.N * (p.D / 2) * 8);
-    e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
-    if (e != cudaSuccess) return cuda_status(e);
-    if (p.A > 0) {
+    if (p.A > 0) {                                          // the table serves A2 here and B4 in the epilogues
       e = strata::launch_rope_table_f32(p, rtab, coords, freqs, st, &launches);
-      if (e != cudaSuccess) return cuda_status(e);
+      if (e == cudaSuccess) e = strata::launch_rope_rotate_table(p, q, k, qr, kr, rtab, 1.f, st, &launches);
+    } else {
+      e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
     }
+    if (e != cudaSuccess) return cuda_status(e);
     e = strata::launch_bwd_tc(p, qr, kr, v, o, d_o, d_o_main, lse, stat, p.A > 0 ? rtab : nullptr, dq, dk, dv, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
     g_last_launches = launches;
