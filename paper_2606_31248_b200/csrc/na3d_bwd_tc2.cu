@@ -31,15 +31,17 @@
 // Schedule: ONE persistent CTA per SM runs the chain S'/dP' MMAs -> elementwise pass -> gradient MMAs as a pipeline
 // (a one-tile-per-CTA version of round 1 cost ~3100 cycles per chunk in a strictly serial chain that two co-resident
 // CTAs only half filled, profiles/r1_bwd_cfg4_and_tile_cfg2.md):
-//   * S' / dP' have three buffers in TMEM and TWO elementwise warpgroups take alternate chunks, so the
-//     MMAs of chunks c + 1, c + 2 run under the elementwise pass of chunk c;
+//   * S' / dP' have three buffers in TMEM and TWO elementwise warpgroups split every chunk by columns (the
+//     elementwise pass is the longest stage of the ring S' MMA -> elementwise -> gradient MMA: halving its latency
+//     shortens the ring; taking alternate chunks instead gave the same throughput bound at twice the latency),
+//     so the MMAs of chunks c + 1, c + 2 run under the elementwise pass of chunk c;
 //   * the stationary operand tiles are double buffered in shared memory (and the dQ accumulator in TMEM) and the
 //     chunk stream runs on across tiles, so the epilogue of tile t (TMEM -> un-rotate -> HBM) and the operand loads
 //     of tile t + 1 overlap the MMAs of tile t + 1.
 // TMEM (512 columns): accumulators [0, 128) -- MODE 0: acc1 double buffered by tile parity, MODE 1: {acc1, acc2}
 // once -- | SD[buf] = {S' -> P, dP' -> dS} at 128 + 128 * buf, buf < 3 (chunk index mod 3).
 // Warps (512 threads): 0 TMA producer, 1 S'/dP' MMA issuer + TMEM owner, 2 gradient-MMA issuer, 3 idle,
-// 4-7 elementwise group 0, 8-11 group 1 (group g takes the chunks of global index parity g), 12-15 epilogue
+// 4-7 elementwise group 0, 8-11 group 1 (group g takes columns [32 g, 32 g + 32) of every chunk), 12-15 epilogue
 // (acc1 -> dQ or dK, un-rotated; acc2 -> dV in MODE 1).  The epilogue has warps of its own because its table loads
 // and stores take about as long as half a tile's elementwise work: done by an elementwise group, it held back that
 // group's chunks of the next tile, and with them the MMAs (profiles/r2_bwd_cfg4.md).
@@ -147,7 +149,7 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
       mbar_init(bar_afull(i), 1); mbar_init(bar_aempty(i), 1);
       mbar_init(bar_accdone(i), 1); mbar_init(bar_accfree(i), 4);
     }
-    for (int i = 0; i < C::NBUF; ++i) { mbar_init(bar_sfull(i), 1); mbar_init(bar_pfull(i), 4); mbar_init(bar_sdfree(i), 1); }
+    for (int i = 0; i < C::NBUF; ++i) { mbar_init(bar_sfull(i), 1); mbar_init(bar_pfull(i), 8); mbar_init(bar_sdfree(i), 1); }
     for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
     fence_barrier_init();
   }
@@ -188,15 +190,22 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
   if (warp == 0) {
     // =========================== TMA producer ===========================
-    if (lane == 0) {
+    // The control warps walk their loops with all 32 lanes in uniform control flow and elect one lane for the TMA / MMA /
+    // commit instructions only: inside `if (lane == 0)` the compiler cannot prove any operand warp-uniform and wraps
+    // every tcgen05.mma in a ~10-instruction election / uniformisation sequence (~80 cycles per MMA of 32-48 tensor
+    // cycles: the S'/dP' issuer never waited on a barrier, it was the bottleneck).
+    {
       int Tn = 0, Cn = 0;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const Tile2 T = tile_of(t);
         const int par = Tn & 1, bl = T.b * p.L;
         mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
-        mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
-        tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
-        tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        if (elect_one()) {
+          mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
+          tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+          tma_load_5d(a_smem(par, 1), &tm_a2, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
+        }
+        __syncwarp();
         for (int pl = T.bl0; pl < T.bl1; ++pl)
           for (int cy = 0; cy < T.ncy; ++cy)
             for (int cx = 0; cx < T.ncx; ++cx, ++Cn) {
@@ -205,52 +214,62 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
               const uint32_t sb = st_smem + s * C::STAGE_BYTES;
               const int gx = T.bx0 + cx * C::HX, gy = T.by0 + cy * C::CY;
               mbar_wait(bar_empty(s), ph ^ 1u);
-              mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128 + (MODE == 1 ? C::NCOL * 16 : 0));
-              tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
-              tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
-              if (MODE == 1) tma_load_5d(xb_smem(s), &tm_bias, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              if (elect_one()) {
+                mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128 + (MODE == 1 ? C::NCOL * 16 : 0));
+                tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
+                tma_load_5d(sb + C::CHUNK_BYTES, &tm_b2, bar_full(s), 0, T.h, gx, gy, bl + pl);
+                if (MODE == 1) tma_load_5d(xb_smem(s), &tm_bias, bar_full(s), 0, T.h, gx, gy, bl + pl);
+              }
+              __syncwarp();
             }
       }
     }
   } else if (warp == 1) {
     // =========================== S'/dP' issuer ===========================
-    // Issuing one tcgen05.mma costs its thread ~70 cycles whatever the shape (measured: 8 MMAs of 32 tensor-pipe
-    // cycles each take ~560 cycles to issue), so the two kinds of MMA have an issuer warp each.
-    if (lane == 0) {
+    {
       constexpr uint32_t idesc_s = instr_desc(C::M, C::N, false);
+      constexpr uint32_t kDescHi = 0x40004040u;            // 8-row groups 1024 bytes apart, version 1, 128-byte swizzle
+      auto dlo = [](uint32_t addr) { return ((addr >> 4) & 0x3FFFu) | (1u << 16); };
+      auto dsc = [](uint32_t lo) { return ((uint64_t)kDescHi << 32) | lo; };
+      const uint32_t lxa = dlo(xa_smem);
       int Tn = 0, Cn = 0;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const int n = tile_of(t).nchunks;
         const int par = Tn & 1;
         mbar_wait<false>(bar_afull(par), (uint32_t)(Tn >> 1) & 1u);
-        const uint64_t da1 = smem_desc(a_smem(par, 0)), da2 = smem_desc(a_smem(par, 1));
+        const uint32_t la1 = dlo(a_smem(par, 0)), la2 = dlo(a_smem(par, 1));
         for (int c = 0; c < n; ++c, ++Cn) {
           const int s = Cn % C::NSTAGE, buf = Cn % C::NBUF;
           mbar_wait<false>(bar_full(s), (uint32_t)(Cn / C::NSTAGE) & 1u);
           mbar_wait<false>(bar_sdfree(buf), ((uint32_t)(Cn / C::NBUF) & 1u) ^ 1u);    // gradient MMAs of chunk Cn - NBUF are done
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
-          const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
+          const uint32_t lb1 = dlo(sb), lb2 = dlo(sb + C::CHUNK_BYTES);
           // bias rows: unswizzled K-major operand -- 8 columns x 16 bytes per core matrix, the next 8 columns 128 bytes on
           // (stride offset), channels 8-15 in the zeros block (leading offset)
-          const uint64_t dxa = smem_desc(xa_smem);
           const uint64_t dxb = (uint64_t)((xb_smem(s) >> 4) & 0x3FFF) | ((uint64_t)((xz_smem - xb_smem(s)) >> 4) << 16) |
                                ((uint64_t)(128 >> 4) << 32) | (1ull << 46);
+          if (elect_one()) {
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks) umma_ss(sd, da1 + 2 * ks, db1 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
-          if (MODE == 1) umma_ss(sd, dxa, dxb, idesc_s, 1u);                       // S'  -= lse_j / scale
+            for (int ks = 0; ks < 4; ++ks) umma_ss(sd, dsc(la1 + 2 * ks), dsc(lb1 + 2 * ks), idesc_s, ks > 0 ? 1u : 0u);
+            if (MODE == 1) umma_ss(sd, dsc(lxa), dxb, idesc_s, 1u);                     // S'  -= lse_j / scale
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, da2 + 2 * ks, db2 + 2 * ks, idesc_s, ks > 0 ? 1u : 0u);
-          if (MODE == 1) umma_ss(sd + 64, dxa + 2, dxb, idesc_s, 1u);              // dP' -= D_j
-          umma_commit(bar_sfull(buf));
-          if (c == n - 1) umma_commit(bar_aempty(par));           // the operand tiles are free after these MMAs
+            for (int ks = 0; ks < 4; ++ks) umma_ss(sd + 64, dsc(la2 + 2 * ks), dsc(lb2 + 2 * ks), idesc_s, ks > 0 ? 1u : 0u);
+            if (MODE == 1) umma_ss(sd + 64, dsc(lxa + 2), dxb, idesc_s, 1u);            // dP' -= D_j
+            umma_commit(bar_sfull(buf));
+            if (c == n - 1) umma_commit(bar_aempty(par));         // the operand tiles are free after these MMAs
+          }
+          __syncwarp();
         }
       }
     }
   } else if (warp == 2) {
     // =========================== gradient-MMA issuer ===========================
-    if (lane == 0) {
+    {
       constexpr uint32_t idesc_acc = instr_desc(C::M, 64, true);
+      constexpr uint32_t kDescHi = 0x40004040u;
+      auto dlo = [](uint32_t addr) { return ((addr >> 4) & 0x3FFFu) | (1u << 16); };
+      auto dsc = [](uint32_t lo) { return ((uint64_t)kDescHi << 32) | lo; };
       int Tn = 0, Cn = 0;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const int n = tile_of(t).nchunks;
@@ -262,15 +281,21 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
           if (c == 0) mbar_wait<false>(bar_accfree(ai), ((uint32_t)ak & 1u) ^ 1u);   // epilogue of the last tile on this accumulator
           tc_fence_after();
           const uint32_t sb = st_smem + s * C::STAGE_BYTES, sd = tmem + C::TMEM_SD + 128 * buf;
-          const uint64_t db1 = smem_desc(sb), db2 = smem_desc(sb + C::CHUNK_BYTES);
+          const uint32_t lb1 = dlo(sb), lb2 = dlo(sb + C::CHUNK_BYTES);
+          const uint32_t acc_on = c > 0 ? 1u : 0u;
+          if (elect_one()) {
 #pragma unroll
-          for (int ks = 0; ks < C::N / 16; ++ks) {
-            umma_ts(acc, sd + 64 + 8 * ks, db1 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
-            if (MODE == 1) umma_ts(acc + 64, sd + 8 * ks, db2 + 128 * ks, idesc_acc, (c > 0 || ks > 0) ? 1u : 0u);
+            for (int ks = 0; ks < C::N / 16; ++ks) {
+              // the packed P / dS of key columns [16 ks, 16 ks + 16): written by elementwise group ks / 2 into its own half
+              const uint32_t pa = 32u * (ks >> 1) + 8u * (ks & 1);
+              umma_ts(acc, sd + 64 + pa, dsc(lb1 + 128 * ks), idesc_acc, ks > 0 ? 1u : acc_on);
+              if (MODE == 1) umma_ts(acc + 64, sd + pa, dsc(lb2 + 128 * ks), idesc_acc, ks > 0 ? 1u : acc_on);
+            }
+            umma_commit(bar_empty(s));
+            umma_commit(bar_sdfree(buf));
+            if (c == n - 1) umma_commit(bar_accdone(ai));
           }
-          umma_commit(bar_empty(s));
-          umma_commit(bar_sdfree(buf));
-          if (c == n - 1) umma_commit(bar_accdone(ai));
+          __syncwarp();
         }
       }
     }
@@ -278,7 +303,7 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
   } else if (warp < 12) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 144;");
     // =========================== elementwise group g (one row per thread) ===========================
-    const int g = (warp - 4) >> 2;                 // group: takes the chunks whose global index has parity g
+    const int g = (warp - 4) >> 2;                 // group: takes columns [32 g, 32 g + 32) of every chunk
     const int sp = warp & 3;                       // TMEM subpartition of this warp
     const int row = sp * 32 + lane;                // row of the stationary tile == TMEM lane
     const uint32_t tm = tmem + ((uint32_t)(sp * 32) << 16);
@@ -309,7 +334,6 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
         const bool plane_ok = pl >= il0 && pl < il1;
         for (int cy = 0; cy < T.ncy; ++cy)
           for (int cx = 0; cx < T.ncx; ++cx, ++c, ++Cn) {
-            if ((Cn & 1) != g) continue;
             // validity of this row over the chunk's columns: bit mask (skip test) and additive biases
             const int xa = max(ix0 - cx * C::HX, 0), xb = min(ix1 - cx * C::HX, C::HX);
             const uint32_t xm = xb > xa ? ((1u << xb) - 1u) & ~((1u << xa) - 1u) : 0u;
@@ -333,45 +357,58 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
             mbar_wait(bar_sfull(buf), (uint32_t)(Cn / C::NBUF) & 1u);
             tc_fence_after();
             if (__any_sync(0xffffffffu, anyrow && xm != 0u)) {
-              auto batch = [&](auto h0c, auto nbc) {
-                constexpr int H0 = decltype(h0c)::value, NB = decltype(nbc)::value;
-                uint32_t svw[NB], dpw[NB];
-                tmem_ld_issue_n<NB>(sd + H0, svw);
-                tmem_ld_issue_n<NB>(sd + 64 + H0, dpw);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                reg_fence_n<NB>(svw);
-                reg_fence_n<NB>(dpw);
-                uint32_t pw[NB / 2], dw[NB / 2];
+              // this group's half of the columns, 16 at a time, software pipelined: the TMEM load of batch k + 1 is issued
+              // before the arithmetic of batch k (tcgen05.wait::ld waits for every outstanding load: one batch in flight)
+              auto half = [&](auto gc) {
+                constexpr int NB = 16, KB0 = 2 * decltype(gc)::value, KB1 = (KB0 + 2 < C::N / NB) ? KB0 + 2 : C::N / NB;
+                uint32_t svw[2][NB], dpw[2][NB];
+                tmem_ld_issue_n<NB>(sd + KB0 * NB, svw[0]);
+                tmem_ld_issue_n<NB>(sd + 64 + KB0 * NB, dpw[0]);
 #pragma unroll
-                for (int u = 0; u < NB; u += 2) {
-                  const int col = H0 + u;                            // compile-time
-                  if (col < C::NCOL) {
-                    const int r = col / C::HX, x = col % C::HX;     // x even: (x, x + 1) are in the same row
-                    // MODE 1: the tensor cores have already subtracted the column statistics (bias K step)
-                    const F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
-                    F2 tt = ffma2(F2{__uint_as_float(svw[u]), __uint_as_float(svw[u + 1])}, F2{cs, cs}, nb);
-                    tt = fadd2(tt, xz2[x >> 1]);
-                    const F2 e = {ex2(tt.x), ex2(tt.y)};
-                    const F2 gq = fmul2(e, fadd2(F2{__uint_as_float(dpw[u]), __uint_as_float(dpw[u + 1])}, dd));
-                    pw[u >> 1] = pack_bf16(e.x, e.y);
-                    dw[u >> 1] = pack_bf16(gq.x, gq.y);
-                  } else {
-                    pw[u >> 1] = 0u; dw[u >> 1] = 0u;
+                for (int kb = KB0; kb < KB1; ++kb) {
+                  const int H0 = kb * NB, cur = (kb - KB0) & 1;
+                  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                  reg_fence_n<NB>(svw[cur]);
+                  reg_fence_n<NB>(dpw[cur]);
+                  if (kb + 1 < KB1) {
+                    tmem_ld_issue_n<NB>(sd + H0 + NB, svw[cur ^ 1]);
+                    tmem_ld_issue_n<NB>(sd + 64 + H0 + NB, dpw[cur ^ 1]);
                   }
+                  uint32_t pw[NB / 2], dw[NB / 2];
+#pragma unroll
+                  for (int u = 0; u < NB; u += 2) {
+                    const int col = H0 + u;                            // compile-time
+                    if (col < C::NCOL) {
+                      const int r = col / C::HX, x = col % C::HX;     // x even: (x, x + 1) are in the same row
+                      // MODE 1: the tensor cores have already subtracted the column statistics (bias K step)
+                      const F2 nb = {nbr[r], nbr[r]}, dd = {-my_d, -my_d};
+                      F2 tt = ffma2(F2{__uint_as_float(svw[cur][u]), __uint_as_float(svw[cur][u + 1])}, F2{cs, cs}, nb);
+                      tt = fadd2(tt, xz2[x >> 1]);
+                      const F2 e = {ex2(tt.x), ex2(tt.y)};
+                      const F2 gq = fmul2(e, fadd2(F2{__uint_as_float(dpw[cur][u]), __uint_as_float(dpw[cur][u + 1])}, dd));
+                      pw[u >> 1] = pack_bf16(e.x, e.y);
+                      dw[u >> 1] = pack_bf16(gq.x, gq.y);
+                    } else {
+                      pw[u >> 1] = 0u; dw[u >> 1] = 0u;
+                    }
+                  }
+                  // packed bf16 results go into this group's own half of the buffer (the other half is still being read)
+                  constexpr int PK = 32 * (KB0 / 2);
+                  if (MODE == 1) tmem_st_n<NB / 2>(sd + PK + (H0 - PK) / 2, pw);
+                  tmem_st_n<NB / 2>(sd + 64 + PK + (H0 - PK) / 2, dw);
                 }
-                if (MODE == 1) tmem_st_n<NB / 2>(sd + H0 / 2, pw);
-                tmem_st_n<NB / 2>(sd + 64 + H0 / 2, dw);
               };
-              batch(std::integral_constant<int, 0>{}, std::integral_constant<int, (C::N < 32 ? C::N : 32)>{});
-              if constexpr (C::N > 32) batch(std::integral_constant<int, 32>{}, std::integral_constant<int, C::N - 32>{});
+              if (g == 0) half(std::integral_constant<int, 0>{}); else half(std::integral_constant<int, 1>{});
             } else {
               uint32_t z[8];
 #pragma unroll
               for (int u = 0; u < 8; ++u) z[u] = 0u;
 #pragma unroll
-              for (int j0 = 0; j0 < C::N / 2; j0 += 8) {
-                if (MODE == 1) tmem_st8(sd + j0, z);
-                tmem_st8(sd + 64 + j0, z);
+              for (int j0 = 0; j0 < 16; j0 += 8) {                 // this group's half: 32 columns = 16 packed
+                if (32 * g + 2 * j0 < C::N) {
+                  if (MODE == 1) tmem_st8(sd + 32 * g + j0, z);
+                  tmem_st8(sd + 64 + 32 * g + j0, z);
+                }
               }
             }
             tmem_wait_st();
