@@ -128,20 +128,29 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
 
   if (warp == 0) {
     // =========================== TMA producer ===========================
-    if (lane == 0) {
+    // Both control warps run their loops with all 32 lanes in uniform control flow and elect one lane for the TMA /
+    // MMA / commit instructions: under `if (lane == 0)` the compiler cannot prove the operands warp-uniform and wraps
+    // every tcgen05.mma in an election / uniformisation sequence of ~10 instructions.
+    {
       const int bl = b * p.L;
-      mbar_expect_tx(bar_q, C::Q_BYTES);
-      for (int j = 0; j < C::DSUB; ++j) tma_load_5d(q_smem + j * C::SUB_Q, &tm_q, bar_q, 64 * j, h, x0, y0, bl + l0);
+      if (elect_one()) {
+        mbar_expect_tx(bar_q, C::Q_BYTES);
+        for (int j = 0; j < C::DSUB; ++j) tma_load_5d(q_smem + j * C::SUB_Q, &tm_q, bar_q, 64 * j, h, x0, y0, bl + l0);
+      }
+      __syncwarp();
       // K loads run one chunk ahead of the V loads: a K stage is released by the QK^T MMA, a V stage only by
       // the PV MMA after the softmax; waiting for V first would hold back the next K chunk
       auto load_v = [&](int c, int pl, int cy) {
         const int s = c % C::NSTAGE;
         const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
         mbar_wait(bar_vempty(s), ph ^ 1u);
-        mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
-        for (int j = 0; j < C::DSUB; ++j)
-          tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_v, bar_vfull(s), 64 * j, h, hs_x,
-                      hs_y + cy * C::CY, bl + hs_l + pl);
+        if (elect_one()) {
+          mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
+          for (int j = 0; j < C::DSUB; ++j)
+            tma_load_5d(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_v, bar_vfull(s), 64 * j, h, hs_x,
+                        hs_y + cy * C::CY, bl + hs_l + pl);
+        }
+        __syncwarp();
       };
       int c = 0, ppl = -1, pcy = 0;
       for (int pl = 0; pl < hl; ++pl)
@@ -149,10 +158,13 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
           const int s = c % C::NSTAGE;
           const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
           mbar_wait(bar_kempty(s), ph ^ 1u);
-          mbar_expect_tx(bar_kfull(s), C::STAGE_BYTES);
-          for (int j = 0; j < C::DSUB; ++j)
-            tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_k, bar_kfull(s), 64 * j, h, hs_x,
-                        hs_y + cy * C::CY, bl + hs_l + pl);
+          if (elect_one()) {
+            mbar_expect_tx(bar_kfull(s), C::STAGE_BYTES);
+            for (int j = 0; j < C::DSUB; ++j)
+              tma_load_5d(k_smem + s * C::STAGE_BYTES + j * C::SUB_KV, &tm_k, bar_kfull(s), 64 * j, h, hs_x,
+                          hs_y + cy * C::CY, bl + hs_l + pl);
+          }
+          __syncwarp();
           if (ppl >= 0) load_v(c - 1, ppl, pcy);
           ppl = pl; pcy = cy;
         }
@@ -160,7 +172,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     }
   } else if (warp == 1) {
     // =========================== MMA issuer ===========================
-    if (lane == 0) {
+    {
       constexpr uint32_t idesc_qk = instr_desc(C::M, C::NKEY, false);
       constexpr uint32_t idesc_pv = instr_desc(C::M, 64, true);
       mbar_wait(bar_q, 0);
@@ -172,15 +184,18 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         // ---- S = Qrot Krot^T  (M = 128, N = NKEY, K = D in steps of 16)
         mbar_wait(bar_kfull(s), ph);
         tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
-        for (int ks = 0; ks < C::D / 16; ++ks) {
-          const uint32_t off = (ks >> 2) * 1u, kin = (ks & 3) * 32u;      // sub-tile, byte offset in the row
-          const uint64_t ad = smem_desc(q_smem + off * C::SUB_Q + kin);
-          const uint64_t bd = smem_desc(k_smem + s * C::STAGE_BYTES + off * C::SUB_KV + kin);
-          umma_ss(tmem + C::TMEM_S + sb * C::NKEY, ad, bd, idesc_qk, ks > 0 ? 1u : 0u);
+          for (int ks = 0; ks < C::D / 16; ++ks) {
+            const uint32_t off = (ks >> 2) * 1u, kin = (ks & 3) * 32u;      // sub-tile, byte offset in the row
+            const uint64_t ad = smem_desc(q_smem + off * C::SUB_Q + kin);
+            const uint64_t bd = smem_desc(k_smem + s * C::STAGE_BYTES + off * C::SUB_KV + kin);
+            umma_ss(tmem + C::TMEM_S + sb * C::NKEY, ad, bd, idesc_qk, ks > 0 ? 1u : 0u);
+          }
+          umma_commit(bar_kempty(s));
+          umma_commit(bar_sfull + 8u * sb);
         }
-        umma_commit(bar_kempty(s));
-        umma_commit(bar_sfull + 8u * sb);
+        __syncwarp();
       };
       // With two buffers Q K^T runs one chunk ahead: buffer (c + 1) % 2 is free once P V of chunk c - 1 (which read
       // its P) has been issued -- the tensor pipe executes in issue order.
@@ -193,16 +208,19 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         mbar_wait(bar_pfull + 8u * sb, (uint32_t)(c / C::NSBUF) & 1u);
         mbar_wait(bar_vfull(s), ph);
         tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
-        for (int ks = 0; ks < C::NKEY / 16; ++ks) {
+          for (int ks = 0; ks < C::NKEY / 16; ++ks) {
 #pragma unroll
-          for (int j = 0; j < C::DSUB; ++j) {
-            const uint64_t bd = smem_desc(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
-            umma_ts(tmem + C::TMEM_O + 64 * j, tmem + C::TMEM_P + sb * C::NKEY + 8 * ks, bd, idesc_pv, (c > 0 || ks > 0) ? 1u : 0u);
+            for (int j = 0; j < C::DSUB; ++j) {
+              const uint64_t bd = smem_desc(v_smem + s * C::STAGE_BYTES + j * C::SUB_KV + ks * 16 * 128);
+              umma_ts(tmem + C::TMEM_O + 64 * j, tmem + C::TMEM_P + sb * C::NKEY + 8 * ks, bd, idesc_pv, (c > 0 || ks > 0) ? 1u : 0u);
+            }
           }
+          umma_commit(bar_vempty(s));
+          umma_commit(bar_pvdone + 8u * (c & 1));
         }
-        umma_commit(bar_vempty(s));
-        umma_commit(bar_pvdone + 8u * (c & 1));
+        __syncwarp();
         if (C::NSBUF == 1 && c + 1 < nchunks) issue_qk(c + 1);
       }
     }
