@@ -60,6 +60,10 @@ cudaError_t launch_rope_table_f32(const Problem& p, void* table, const float* co
 
 // na3d_fwd_plane.cu: tcgen05 forward (head_dim 64, k_L = 3), everything (A1-A6) in one kernel; whole key planes per
 // softmax hand-off, Q~ in TMEM.  `fix` is plane_fwd_workspace_bytes() of device scratch (rows for the fix-up kernel).
+// The fix-up list: [0] number of listed rows, [1] != 0: every row, [2 ...] up to kFixCap row ids ((b * H + h) * N + token).
+// A forward kernel that exponentiates without a reference lists the rows whose sum left [kRowSumMin, kRowSumMax].
+constexpr unsigned int kFixCap = 65535;
+constexpr float kRowSumMax = 1.2676506e30f, kRowSumMin = 8.2718061e-25f;   // 2^100, 2^-80
 bool plane_fwd_supported(const Problem& p);
 size_t plane_fwd_workspace_bytes();
 cudaError_t launch_fwd_plane(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
@@ -96,9 +100,9 @@ cudaError_t launch_rmsnorm_bwd_rows(const Problem& p, const void* x, void* dx, f
 cudaError_t launch_dgate_rows(const Problem& p, const void* d_o, const void* o, const float* gate, float* dgate,
                               cudaStream_t st, int* launches);
 
-// na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands.
+// na3d_tc_fwd.cu: tcgen05 forward on pre-rotated bf16 operands; lists rows for launch_fix_rows in `fix` (cleared here).
 bool tc_fwd_supported(const Problem& p);
 cudaError_t launch_fwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
-                          float* lse, cudaStream_t stream, int* launches);
+                          float* lse, void* fix, cudaStream_t stream, int* launches);
 
 }  // namespace strata

@@ -106,7 +106,6 @@ constexpr int kWarpAux = 16, kWarpTma = 20, kWarpMma = 21, kWarpTmaV = 22;
 constexpr int kBarPair = 1;               // named barriers 1-8: the two warps of a (pair, subpartition), 64 threads
 constexpr int kBarAux = 13;               // the aux warpgroup, 128 threads
 constexpr int kMaxLevels = 256;
-constexpr float kRowSumMax = 1.2676506e30f, kRowSumMin = 8.2718061e-25f;   // 2^100, 2^-80: row sums outside go to the fix-up kernel
 
 // ------------------------------------------------------------------------------------------------
 // small device helpers
@@ -836,31 +835,41 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
 }
 
 // ------------------------------------------------------------------------------------------------
-// Fix-up: the rows whose sum overflowed, recomputed with a true two-pass softmax (one warp per row, lane j owns
-// the rotary pair j of the 64 channels; fp64 angle).  Rare by construction; correctness over speed.
+// Fix-up: the listed rows recomputed with a true two-pass softmax from the RAW Q, K (one warp per row, lane j owns the
+// rotary pairs j, j + 32, ... of the D / 2; fp64 angle).  Rare by construction; correctness over speed.
 // ------------------------------------------------------------------------------------------------
+template <int D>
 __global__ void __launch_bounds__(128)
 na3d_fix_rows_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k,
                      const __nv_bfloat16* __restrict__ v, const float* __restrict__ coords,
                      const float* __restrict__ freqs, __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                      const unsigned long long* __restrict__ fix, unsigned int cap, Problem p) {
+  constexpr int NP = D / 64;                                        // rotary pairs per lane
   const unsigned long long listed = fix[0];
   const bool all = listed > cap || fix[1] != 0;                     // the list overflowed / level-dependent coordinates: every row
   if (listed == 0 && !all) return;
   const unsigned long long total = all ? (unsigned long long)p.rows() : listed;
   const int lane = threadIdx.x & 31;
   const unsigned long long w0 = (unsigned long long)blockIdx.x * 4 + (threadIdx.x >> 5), nw = (unsigned long long)gridDim.x * 4;
-  const int c0 = p.pairing ? lane : 2 * lane, c1 = p.pairing ? lane + 32 : 2 * lane + 1;
-  float f[3] = {0.f, 0.f, 0.f};
-  for (int a = 0; a < p.A && a < 3; ++a) f[a] = freqs[a * 32 + lane];
-  auto rotated = [&](const __nv_bfloat16* x, long long b, long long tok, int h, float& ra, float& rb) {
-    const __nv_bfloat16* src = x + ((b * p.N + tok) * p.H + h) * 64;
-    const float a_ = __bfloat162float(src[c0]), b_ = __bfloat162float(src[c1]);
-    double phi = 0.0;
-    for (int a = 0; a < p.A && a < 3; ++a) phi += (double)coords[(b * p.N + tok) * p.A + a] * (double)f[a];
-    double sn, cs;
-    sincos(phi, &sn, &cs);
-    ra = (float)(a_ * cs - b_ * sn); rb = (float)(a_ * sn + b_ * cs);
+  int c0[NP], c1[NP];
+  float f[NP][3];
+#pragma unroll
+  for (int u = 0; u < NP; ++u) {
+    const int j = lane + 32 * u;
+    c0[u] = p.pairing ? j : 2 * j; c1[u] = p.pairing ? j + D / 2 : 2 * j + 1;
+    for (int a = 0; a < 3; ++a) f[u][a] = (a < p.A) ? freqs[a * (D / 2) + j] : 0.f;
+  }
+  auto rotated = [&](const __nv_bfloat16* x, long long b, long long tok, int h, float (&ra)[NP], float (&rb)[NP]) {
+    const __nv_bfloat16* src = x + ((b * p.N + tok) * p.H + h) * D;
+#pragma unroll
+    for (int u = 0; u < NP; ++u) {
+      const float a_ = __bfloat162float(src[c0[u]]), b_ = __bfloat162float(src[c1[u]]);
+      double phi = 0.0;
+      for (int a = 0; a < p.A && a < 3; ++a) phi += (double)coords[(b * p.N + tok) * p.A + a] * (double)f[u][a];
+      double sn, cs;
+      sincos(phi, &sn, &cs);
+      ra[u] = (float)(a_ * cs - b_ * sn); rb[u] = (float)(a_ * sn + b_ * cs);
+    }
   };
   for (unsigned long long i = w0; i < total; i += nw) {
     const unsigned long long rid = all ? i : fix[2 + i];          // (b * H + h) * N + token
@@ -869,29 +878,36 @@ na3d_fix_rows_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
     const long long b = (long long)(rid / (unsigned long long)p.N / (unsigned long long)p.H);
     const int x = (int)(tok % p.X), y = (int)((tok / p.X) % p.Y), l = (int)(tok / ((long long)p.X * p.Y));
     const int sl = window_start(l, p.kL, p.L), sy = window_start(y, p.kY, p.Y), sx = window_start(x, p.kX, p.X);
-    float qa, qb;
+    float qa[NP], qb[NP];
     rotated(q, b, tok, h, qa, qb);
     float mx = -INFINITY;
     for (int pass = 0; pass < 2; ++pass) {
-      float sum = 0.f, oa = 0.f, ob = 0.f;
+      float sum = 0.f, oa[NP], ob[NP];
+#pragma unroll
+      for (int u = 0; u < NP; ++u) { oa[u] = 0.f; ob[u] = 0.f; }
       for (int dl = 0; dl < p.kL; ++dl)
         for (int dy = 0; dy < p.kY; ++dy)
           for (int dx = 0; dx < p.kX; ++dx) {
             const long long kt = ((long long)(sl + dl) * p.Y + sy + dy) * p.X + sx + dx;
-            float ka, kb;
+            float ka[NP], kb[NP];
             rotated(k, b, kt, h, ka, kb);
-            float s = qa * ka + qb * kb;
+            float s = 0.f;
+#pragma unroll
+            for (int u = 0; u < NP; ++u) s += qa[u] * ka[u] + qb[u] * kb[u];
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
             s *= p.scale;
             if (pass == 0) { mx = fmaxf(mx, s); continue; }
             const float pr = expf(s - mx);
-            const __nv_bfloat16* vs = v + ((b * p.N + kt) * p.H + h) * 64;
-            sum += pr; oa += pr * __bfloat162float(vs[c0]); ob += pr * __bfloat162float(vs[c1]);
+            const __nv_bfloat16* vs = v + ((b * p.N + kt) * p.H + h) * D;
+            sum += pr;
+#pragma unroll
+            for (int u = 0; u < NP; ++u) { oa[u] += pr * __bfloat162float(vs[c0[u]]); ob[u] += pr * __bfloat162float(vs[c1[u]]); }
           }
       if (pass == 1) {
-        __nv_bfloat16* dst = o + ((b * p.N + tok) * p.H + h) * 64;
-        dst[c0] = __float2bfloat16_rn(oa / sum); dst[c1] = __float2bfloat16_rn(ob / sum);
+        __nv_bfloat16* dst = o + ((b * p.N + tok) * p.H + h) * D;
+#pragma unroll
+        for (int u = 0; u < NP; ++u) { dst[c0[u]] = __float2bfloat16_rn(oa[u] / sum); dst[c1[u]] = __float2bfloat16_rn(ob[u] / sum); }
         if (lane == 0) lse[rid] = mx + logf(sum);
       }
     }
@@ -901,7 +917,6 @@ na3d_fix_rows_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
 // ------------------------------------------------------------------------------------------------
 // Host side
 // ------------------------------------------------------------------------------------------------
-constexpr unsigned int kFixCap = 65535;
 
 template <class C>
 bool plane_shape_ok(const Problem& p) {
@@ -972,13 +987,14 @@ cudaError_t launch_plane(const Problem& p, int cfg_index, const void* q, const v
 size_t plane_fwd_workspace_bytes() { return 16 + 8 * (size_t)kFixCap; }
 
 // The rows listed in `fix` (plane_fwd_workspace_bytes() of device memory: [0] count, [1] != 0: every row, [2 ...] row
-// ids), recomputed with the two-pass SIMT softmax.  head_dim 64, bf16.
+// ids), recomputed with the two-pass SIMT softmax.  head_dim 64 or 128, bf16.
 cudaError_t launch_fix_rows(const Problem& p, const void* q, const void* k, const void* v, const float* coords,
                             const float* freqs, void* o, float* lse, void* fix, cudaStream_t stream, int* launches) {
+  if (p.D != 64 && p.D != 128) return cudaErrorInvalidValue;
   prof_begin("na3d_fix_rows", stream);
-  na3d_fix_rows_kernel<<<148, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v,
-                                                coords, freqs, (__nv_bfloat16*)o, lse,
-                                                reinterpret_cast<const unsigned long long*>(fix), kFixCap, p);
+  auto kernel = p.D == 64 ? na3d_fix_rows_kernel<64> : na3d_fix_rows_kernel<128>;
+  kernel<<<148, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, coords, freqs,
+                                  (__nv_bfloat16*)o, lse, reinterpret_cast<const unsigned long long*>(fix), kFixCap, p);
   prof_end(stream);
   if (launches) ++*launches;
   return cudaGetLastError();

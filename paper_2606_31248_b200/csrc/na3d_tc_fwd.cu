@@ -6,13 +6,16 @@
 //   trimmed to what the inward-clamped windows (R1) really reach -- is
 //   streamed through shared memory by TMA in chunks of CY = 8 key rows of one level plane;
 //   S = Qrot Krot^T and O += P V run on the 5th-gen tensor cores (tcgen05.mma, M = 128,
-//   accumulators in TMEM); the softmax is online, one query row per thread, with the window mask
-//   applied as an additive -inf bias and whole key rows / planes skipped per warp.
+//   accumulators in TMEM); one query row per thread, the window mask applied as an additive -inf bias and whole key
+//   rows / planes skipped per warp.  As in the fused forward there is no running maximum and no rescale of O
+//   (R19): P = 2^(s scale log2 e); a row whose sum leaves 2^-80 .. 2^100 is listed in `fix` and recomputed
+//   by na3d_fix_rows_kernel (two-pass softmax from the raw Q, K) right after this kernel.  Dropping the maximum, the
+//   optimistic-pass / redo logic and the O rescale took 6 % off config 2 and 12 % off the 9 x 9 x 9 shape.
 //
 // Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner,
 // warps 2-5 = softmax + epilogue (TMEM subpartition = warp index mod 4).
 // Pipelines (mbarriers): K/V stage full/empty (TMA <-> MMA), s_full (MMA1 -> softmax),
-// p_full (softmax -> MMA2), pv_done (MMA2 -> O rescale / epilogue).
+// p_full (softmax -> MMA2), pv_done (MMA2 -> epilogue).
 //
 // TMEM columns: O [0, D) fp32 | S [D, D+NKEY) fp32, overwritten by P (bf16x2, A operand of MMA2).
 #include "tc_common.cuh"
@@ -55,10 +58,10 @@ struct TcParams {
   int ntl, nty, ntx;
   long long N;
   float scale_log2e;
+  unsigned long long* fix;   // fix-up list (common.cuh): rows whose sum left the safe range
 };
 
 constexpr int kThreads = 192;
-constexpr float kRescaleThreshold = 8.f;   // log2 units: P stays below 2^8 between rescales
 
 // ------------------------------------------------------------------------------------------------
 // Kernel
@@ -243,7 +246,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     const int wy_lo = __reduce_min_sync(0xffffffffu, lo_y), wy_hi = __reduce_max_sync(0xffffffffu, lo_y + C::KY);
     const int wl_lo = __reduce_min_sync(0xffffffffu, lo_l), wl_hi = __reduce_max_sync(0xffffffffu, lo_l + C::KL);
 
-    float m_ref = -INFINITY, lsum = 0.f;
+    float lsum = 0.f;
     const float cs = p.scale_log2e;
     int c = 0;
     for (int pl = 0; pl < hl; ++pl) {
@@ -256,63 +259,29 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         tc_fence_after();
         uint32_t pw[C::NKEY / 2];
         float csum = 0.f;
-        for (int attempt = 0; attempt < 2; ++attempt) {
-          float cmax = -INFINITY;
-          csum = 0.f;
+        // No running maximum and no rescale of O: P = 2^(s scale log2 e) as in the fused forward (R19).  The epilogue
+        // checks the row sum and lists the row for the two-pass fix-up kernel if it left the safe range.
 #pragma unroll
-          for (int r = 0; r < C::CY; ++r) {
-            const int py = cy * C::CY + r;
-            if (plane_needed && py >= wy_lo && py < wy_hi) {
-              float sv[16];
-              tmem_ld16(s_tm + r * C::HX, sv);
-              tmem_wait_ld();
-              const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
-              float t[C::HX];
-              float rmax = -INFINITY;
+        for (int r = 0; r < C::CY; ++r) {
+          const int py = cy * C::CY + r;
+          if (plane_needed && py >= wy_lo && py < wy_hi) {
+            float sv[16];
+            tmem_ld16(s_tm + r * C::HX, sv);
+            tmem_wait_ld();
+            const bool rowok = plane_ok && py >= lo_y && py < lo_y + C::KY;
+            const float nb = rowok ? 0.f : -INFINITY;
+            float rsum = 0.f;
 #pragma unroll
-              for (int j = 0; j < C::HX; ++j) { t[j] = fmaf(sv[j], cs, xbias[j]); rmax = fmaxf(rmax, t[j]); }
-              if (rowok) {
-                if (m_ref == -INFINITY) m_ref = rmax;     // first key row of this query: no rescale needed
-                cmax = fmaxf(cmax, rmax);
-              }
-              const float nb = rowok ? -m_ref : -INFINITY;
-              float rsum = 0.f;
-#pragma unroll
-              for (int j = 0; j < C::HX; j += 2) {
-                const float p0 = ex2(t[j] + nb), p1 = ex2(t[j + 1] + nb);
-                rsum += p0 + p1;
-                pw[(r * C::HX + j) >> 1] = pack_bf16(p0, p1);
-              }
-              csum += rsum;
-            } else {
-#pragma unroll
-              for (int j = 0; j < C::HX; j += 2) pw[(r * C::HX + j) >> 1] = 0u;
+            for (int j = 0; j < C::HX; j += 2) {
+              const float p0 = ex2(fmaf(sv[j], cs, xbias[j]) + nb), p1 = ex2(fmaf(sv[j + 1], cs, xbias[j + 1]) + nb);
+              rsum += p0 + p1;
+              pw[(r * C::HX + j) >> 1] = pack_bf16(p0, p1);
             }
-          }
-          // optimistic pass used the old reference maximum; redo the chunk if it was too small
-          const bool need = cmax > m_ref + kRescaleThreshold;
-          if (attempt == 0 && __any_sync(0xffffffffu, need)) {
-            const float alpha = need ? ex2(m_ref - cmax) : 1.f;
-            if (c > 0) {                                    // O holds chunks 0..c-1: rescale its rows
-              mbar_wait(bar_pvdone + 8u * ((c - 1) & 1), (uint32_t)((c - 1) >> 1) & 1u);
-              tc_fence_after();
+            csum += rsum;
+          } else {
 #pragma unroll
-              for (int j = 0; j < C::D; j += 16) {
-                float ov[16];
-                tmem_ld16(tmem + lane_addr + C::TMEM_O + j, ov);
-                tmem_wait_ld();
-                uint32_t ow[16];
-#pragma unroll
-                for (int u = 0; u < 16; ++u) ow[u] = __float_as_uint(ov[u] * alpha);
-                tmem_st16(tmem + lane_addr + C::TMEM_O + j, ow);
-              }
-              tmem_wait_st();
-            }
-            lsum *= alpha;
-            if (need) m_ref = cmax;
-            continue;
+            for (int j = 0; j < C::HX; j += 2) pw[(r * C::HX + j) >> 1] = 0u;
           }
-          break;
         }
         lsum += csum;
         // P (bf16 pairs) -> TMEM, then hand the chunk to MMA2
@@ -344,7 +313,14 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         reinterpret_cast<uint4*>(orow + j)[1] = w1;
       }
     }
-    if (active) lse[((long long)b * p.H + h) * p.N + tok] = (m_ref + log2f(lsum)) * 0.69314718055994531f;
+    if (active) {
+      const long long rid = ((long long)b * p.H + h) * p.N + tok;
+      lse[rid] = log2f(lsum) * 0.69314718055994531f;
+      if (!(lsum < kRowSumMax && lsum > kRowSumMin)) {        // out of the safe range (or NaN): the fix-up kernel recomputes the row
+        const unsigned long long idx = atomicAdd(p.fix, 1ull);
+        if (idx < kFixCap) p.fix[2 + idx] = (unsigned long long)rid;
+      }
+    }
   }
 
   // ---- teardown
@@ -364,7 +340,7 @@ std::mutex g_mu;
 
 template <class C>
 cudaError_t launch_cfg(int slot, const Problem& p, const void* qr, const void* kr, const void* v, void* o, float* lse,
-                       cudaStream_t stream, int* launches) {
+                       void* fix, cudaStream_t stream, int* launches) {
   CUtensorMap tq, tk, tv;
   if (!make_map(&tq, qr, p, C::TX, C::TY, C::TL) || !make_map(&tk, kr, p, C::HX, C::CY, 1) ||
       !make_map(&tv, v, p, C::HX, C::CY, 1))
@@ -373,11 +349,14 @@ cudaError_t launch_cfg(int slot, const Problem& p, const void* qr, const void* k
   tp.B = p.B; tp.H = p.H; tp.L = p.L; tp.Y = p.Y; tp.X = p.X; tp.N = p.N;
   tp.ntl = (p.L + C::TL - 1) / C::TL; tp.nty = (p.Y + C::TY - 1) / C::TY; tp.ntx = (p.X + C::TX - 1) / C::TX;
   tp.scale_log2e = p.scale * 1.4426950408889634f;
+  tp.fix = reinterpret_cast<unsigned long long*>(fix);
   const long long grid = (long long)p.B * p.H * tp.ntl * tp.nty * tp.ntx;
   if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
   DeviceState* ds = device_state(g_states, g_mu);
   if (!ds) return cudaErrorInvalidDevice;
   cudaError_t e = ensure_smem_attr(ds, g_mu, slot, na3d_fwd_tc_kernel<C>, C::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(fix, 0, 16, stream);
   if (e != cudaSuccess) return e;
   prof_begin("na3d_fwd_tcgen05", stream);
   na3d_fwd_tc_kernel<C><<<(unsigned)grid, kThreads, C::SMEM_BYTES, stream>>>(tq, tk, tv, (__nv_bfloat16*)o, lse, tp);
@@ -406,10 +385,10 @@ bool tc_fwd_supported(const Problem& p) {
 }
 
 cudaError_t launch_fwd_tc(const Problem& p, const void* qr, const void* kr, const void* v, void* o,
-                          float* lse, cudaStream_t stream, int* launches) {
+                          float* lse, void* fix, cudaStream_t stream, int* launches) {
 #define X(I_, D_, KL_, KY_, KX_)                                           \
   if (p.D == D_ && p.kL == KL_ && p.kY == KY_ && p.kX == KX_)               \
-    return launch_cfg<Cfg<D_, KL_, KY_, KX_>>(I_, p, qr, kr, v, o, lse, stream, launches);
+    return launch_cfg<Cfg<D_, KL_, KY_, KX_>>(I_, p, qr, kr, v, o, lse, fix, stream, launches);
   STRATA_TC_CONFIGS(X)
 #undef X
   return cudaErrorNotSupported;

@@ -83,7 +83,7 @@ size_t ws_bytes(const Problem& p, Path path, bool backward) {
     return 2 * align_up(e * 2) + align_up(6 * stat) + align_up((size_t)p.B * p.N * (p.D / 2) * 8);
   if (backward) return 4 * align_up(e * 4) + stat;                       // qr, kr, dqr, dkr, delta
   if (path == PATH_TC_PLANE || path == PATH_COLUMN) return align_up(strata::plane_fwd_workspace_bytes());
-  if (path == PATH_TC_PREROT) return 2 * align_up(e * 2);                // qr, kr (bf16)
+  if (path == PATH_TC_PREROT) return align_up(strata::plane_fwd_workspace_bytes()) + 2 * align_up(e * 2);   // fix list, qr, kr (bf16)
   return 2 * align_up(e * 4);                                            // qr, kr (f32)
 }
 
@@ -235,11 +235,14 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
     void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
     e = strata::launch_fwd_column(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);
   } else if (path == PATH_TC_PREROT) {
+    void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
     void* qr = ws.take<char>((size_t)p.elems() * 2);
     void* kr = ws.take<char>((size_t)p.elems() * 2);
     e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
-    e = strata::launch_fwd_tc(p, qr, kr, v, o, lse, st, &launches);
+    e = strata::launch_fwd_tc(p, qr, kr, v, o, lse, fix, st, &launches);
+    if (e != cudaSuccess) return cuda_status(e);
+    e = strata::launch_fix_rows(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);   // rows the kernel listed (usually none)
   } else {
     float* qr = ws.take<float>((size_t)p.elems() * 4);
     float* kr = ws.take<float>((size_t)p.elems() * 4);

@@ -211,10 +211,15 @@ def _exact_inputs(w, rng):
     return q, k, v
 
 
-def test_rows_outside_the_exponent_range_take_the_fixup_kernel(oracle_mod):
-    """The fused forward exponentiates without a reference; a row whose sum leaves 2^-80 .. 2^100 is listed and
+@pytest.mark.parametrize("case", [dict(impl=binding.IMPL_AUTO, window=(3, 7, 7), head_dim=64),            # fused forward
+                                  dict(impl=binding.IMPL_TCGEN05_TILE, window=(3, 7, 7), head_dim=64),    # tile kernel
+                                  dict(impl=binding.IMPL_AUTO, window=(5, 9, 9), head_dim=128)],          # tile kernel, d = 128
+                         ids=["fused", "tile", "tile_d128"])
+def test_rows_outside_the_exponent_range_take_the_fixup_kernel(oracle_mod, case):
+    """The tensor-core forwards exponentiate without a reference; a row whose sum leaves 2^-80 .. 2^100 is listed and
     recomputed by na3d_fix_rows_kernel with a two-pass softmax.  Inputs exact in bf16: normal tolerances apply."""
-    w = wl.small(name="fixup", dtype="bf16", grid=(6, 17, 19), window=(3, 7, 7), heads=2, head_dim=64, rope_axes=0)
+    w = wl.small(name="fixup", dtype="bf16", grid=(6, 17, 19), window=case["window"], heads=2, head_dim=case["head_dim"],
+                 rope_axes=0)
     rng = np.random.default_rng(77)
     q, k, v = _exact_inputs(w, rng)
     k[..., 1] = -40.0                                  # every key: a large component that normal queries hardly see
@@ -229,13 +234,13 @@ def test_rows_outside_the_exponent_range_take_the_fixup_kernel(oracle_mod):
     inp = {"q": _bf16_bits(q), "k": _bf16_bits(k), "v": _bf16_bits(v), "coords": np.zeros((w.batch,) + w.grid + (0,), np.float32),
            "freqs": np.zeros((0, w.head_dim // 2), np.float32)}
     dev = device_inputs(w, inp)
-    desc = desc_of(w, binding.IMPL_AUTO, 0.125)
+    desc = desc_of(w, case["impl"], 0.125)
     o = torch.empty_like(dev["q"])
     lse = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
     ws = binding.alloc_workspace(binding.strata_na3d_workspace_bytes(desc, False), "cuda")
     binding.strata_na3d_fwd(desc, dev["q"], dev["k"], dev["v"], None, None, o, lse, ws)
     torch.cuda.synchronize()
-    listed = int(ws.view(torch.int64)[0].item())       # (white box: the head of the fix-up list)
+    listed = int(ws.view(torch.int64)[0].item())       # (white box: the fix-up list is the head of the workspace)
     assert listed >= len(hot), f"fix-up list holds {listed} rows"
     o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window, scale=0.125)
     assert_parity(to_f64(o), o_ref, "bf16", "fixup O")
