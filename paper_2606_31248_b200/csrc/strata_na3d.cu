@@ -238,9 +238,13 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc, const void* q, c
     void* fix = ws.take<char>(strata::plane_fwd_workspace_bytes());
     void* qr = ws.take<char>((size_t)p.elems() * 2);
     void* kr = ws.take<char>((size_t)p.elems() * 2);
-    e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
-    if (e != cudaSuccess) return cuda_status(e);
-    e = strata::launch_fwd_tc(p, qr, kr, v, o, lse, fix, st, &launches);
+    const void *qin = q, *kin = k;
+    if (p.A > 0) {                                          // (no rotary axes: the kernel reads Q, K as they are)
+      e = strata::launch_rope_rotate(p, q, k, p.dtype, qr, kr, 1, coords, freqs, 1.f, st, &launches);
+      if (e != cudaSuccess) return cuda_status(e);
+      qin = qr; kin = kr;
+    }
+    e = strata::launch_fwd_tc(p, qin, kin, v, o, lse, fix, st, &launches);
     if (e != cudaSuccess) return cuda_status(e);
     e = strata::launch_fix_rows(p, q, k, v, coords, freqs, o, lse, fix, st, &launches);   // rows the kernel listed (usually none)
   } else {
