@@ -54,7 +54,8 @@ typedef enum {
   STRATA_ERR_INVALID_ARG = 1,
   STRATA_ERR_UNSUPPORTED = 2,
   STRATA_ERR_WORKSPACE = 3,
-  STRATA_ERR_CUDA = 4
+  STRATA_ERR_CUDA = 4,
+  STRATA_ERR_STATIC_SCRATCH = 5 /* strata_na3d_fwd_static only: needs more than STRATA_STATIC_SCRATCH_BYTES */
 } strata_status_t;
 
 typedef enum { STRATA_DTYPE_F32 = 0, STRATA_DTYPE_BF16 = 1 } strata_dtype_t;
@@ -152,6 +153,38 @@ strata_status_t strata_na3d_bwd_host(const strata_na3d_desc_t* desc,
                                      const float* coords, const float* freqs,
                                      void* dq, void* dk, void* dv,
                                      void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- forward for callers that have no device memory to hand over ---------------------------------------------------
+ * strata_na3d_fwd wants a `workspace` that the caller allocated.  Some callers cannot get one: a plug-in running
+ * inside a host application whose memory pool has already claimed the whole GPU (a cudaMalloc there fails, or takes
+ * memory the host has promised elsewhere), code that is called inside a latency-critical loop where the implicit
+ * device synchronisation of cudaMalloc / cudaFree is not acceptable, and code that runs where the allocator may not be
+ * called at all (between the host's "no more allocations" point and shutdown).  For them this one call runs the same
+ * forward (same kernels, same results, same argument meaning as strata_na3d_fwd) with the scratch taken from a
+ * fixed array of STRATA_STATIC_SCRATCH_BYTES that is part of the library image: every GPU on which the library is
+ * loaded holds that 1 MiB from load until the process exits, used or not.
+ *   - The call allocates nothing: no cudaMalloc, no cudaFree, no allocating library routine, on any call.  (Keep
+ *     strata_na3d_set_profiling off around it: the profiler creates CUDA events.)
+ *   - Limit: the problem's scratch need, strata_na3d_workspace_bytes(desc, 0), must be <= STRATA_STATIC_SCRATCH_BYTES,
+ *     else STRATA_ERR_STATIC_SCRATCH is returned and nothing is enqueued.  The fused bf16 forward (head_dim 64,
+ *     k_L = 3: configs 1 and 3) and the column-wise forward need 524 544 bytes at ANY batch and grid size; the fp32
+ *     kernels and the bf16 tile kernel keep rotated copies of Q and K in scratch and fit up to B * L * Y * X * H * d
+ *     = 131 072 elements (config 0 has 65 536).  There is no such variant of the backward.
+ *   - The first call on each device (with that device current) looks up the array's address on that device; every
+ *     later call on it reuses the address.  Make that first call before starting any stream capture.
+ *   - All calls on a device share the one array, and it keeps what the previous call left in it.  The only part that
+ *     has to start at zero -- the 16-byte header (row count, take-all flag) of the list of rows for the fix-up kernel
+ *     -- is cleared on `stream` by every call before its kernels; the rest is written before it is read.  Two calls
+ *     that can overlap on the GPU (different streams without an event between them, or different host threads on the
+ *     same device) race on the array and give wrong results: order them on one stream or with events.  A call that
+ *     uses strata_na3d_fwd with its own workspace never touches the array.
+ *   - The sentence on CUDA graphs in the conventions at the top of this header was written for the calls that take a
+ *     workspace; nothing is stated here, either way, about capturing this call. */
+#define STRATA_STATIC_SCRATCH_BYTES 1048576
+strata_status_t strata_na3d_fwd_static(const strata_na3d_desc_t* desc,
+                                       const void* q, const void* k, const void* v,
+                                       const float* coords, const float* freqs,
+                                       void* o, float* lse, void* stream);
 
 /* Number of kernel launches the last successful call on this thread enqueued (for bench.py's
  * `gpu_launches`; memcpy nodes are not counted). */

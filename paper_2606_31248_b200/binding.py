@@ -17,12 +17,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libstrata_na3d.so")
 
 STRATA_OK = 0
+STRATA_ERR_STATIC_SCRATCH = 5
+STATIC_SCRATCH_BYTES = 1 << 20          # STRATA_STATIC_SCRATCH_BYTES of include/strata_na3d.h
 DTYPE_F32, DTYPE_BF16 = 0, 1
 ROPE_INTERLEAVED, ROPE_HALF = 0, 1
 IMPL_AUTO, IMPL_SIMT, IMPL_TCGEN05, IMPL_TCGEN05_TILE = 0, 1, 2, 3
 
 EXPORTS = ("strata_na3d_workspace_bytes", "strata_na3d_host_workspace_bytes", "strata_na3d_impl_selected",
            "strata_na3d_fwd", "strata_na3d_bwd", "strata_na3d_fwd_host", "strata_na3d_bwd_host",
+           "strata_na3d_fwd_static",
            "strata_na3d_normgate_workspace_bytes", "strata_na3d_normgate_fwd", "strata_na3d_normgate_bwd",
            "strata_na3d_last_launch_count", "strata_na3d_set_profiling", "strata_na3d_profile_read",
            "strata_na3d_window_start", "strata_na3d_inverse_window", "strata_stereo_coords",
@@ -99,6 +102,8 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, name)
             f.restype = i32
             f.argtypes = [dp] + [vp] * 12 + [sz, vp]
+        L.strata_na3d_fwd_static.restype = i32
+        L.strata_na3d_fwd_static.argtypes = [dp] + [vp] * 7 + [vp]
         L.strata_na3d_normgate_workspace_bytes.restype = sz
         L.strata_na3d_normgate_workspace_bytes.argtypes = [dp, i32]
         L.strata_na3d_normgate_fwd.restype = i32
@@ -219,6 +224,20 @@ def strata_na3d_bwd_status(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv
 
 def strata_na3d_fwd(desc, q, k, v, coords, freqs, o, lse, workspace, stream=None):
     _check(strata_na3d_fwd_status(desc, q, k, v, coords, freqs, o, lse, workspace, stream), "strata_na3d_fwd")
+
+
+def strata_na3d_fwd_static_status(desc, q, k, v, coords, freqs, o, lse, stream=None) -> int:
+    """Raw status of strata_na3d_fwd_static (no workspace argument: the library's own fixed array is the scratch)."""
+    return int(lib().strata_na3d_fwd_static(ctypes.byref(desc.c()), _ptr(q), _ptr(k), _ptr(v), _ptr(coords), _ptr(freqs),
+                                            _ptr(o), _ptr(lse), _stream_handle(stream)))
+
+
+def strata_na3d_fwd_static(desc, q, k, v, coords, freqs, o, lse, stream=None):
+    """The forward for a caller that cannot allocate device memory (it lives inside a host whose pool owns the GPU, or
+    may not disturb a running loop with cudaMalloc's synchronisation): same kernels and results as strata_na3d_fwd,
+    scratch in a 1 MiB array inside the library.  Raises StrataError (status 5) when the problem needs more than
+    STATIC_SCRATCH_BYTES of scratch; calls that may overlap on one GPU race on the array -- keep them on one stream."""
+    _check(strata_na3d_fwd_static_status(desc, q, k, v, coords, freqs, o, lse, stream), "strata_na3d_fwd_static")
 
 
 def strata_na3d_bwd(desc, q, k, v, o, d_o, lse, coords, freqs, dq, dk, dv, workspace, stream=None):

@@ -435,6 +435,7 @@ const char* strata_status_string(strata_status_t s) {
     case STRATA_ERR_UNSUPPORTED: return "unsupported configuration";
     case STRATA_ERR_WORKSPACE: return "workspace missing or too small";
     case STRATA_ERR_CUDA: return "CUDA error";
+    case STRATA_ERR_STATIC_SCRATCH: return "problem needs more scratch than the library's static array holds (STRATA_STATIC_SCRATCH_BYTES)";
   }
   return "unknown status";
 }
