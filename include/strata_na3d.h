@@ -102,6 +102,18 @@ strata_status_t strata_na3d_fwd(const strata_na3d_desc_t* desc,
                                 void* o, float* lse,
                                 void* workspace, size_t workspace_bytes, void* stream);
 
+/* Exponent range of the tensor-core forwards, and what leaving it costs.  The bf16 tensor-core kernels
+ * (strata_na3d_impl_selected == STRATA_IMPL_TCGEN05) exponentiate scale * q~ . k~ without subtracting a row maximum.
+ * A row whose sum of exponentials leaves [2^-80, 2^100] (|logit| beyond ~55..69: "logits reach +-100..1000 without
+ * QK-norm", App. B.5) is listed in the workspace and recomputed exactly, one warp per row, by a second kernel
+ * that every such call enqueues: a few listed rows cost microseconds.  But when more than 65 535 rows are listed, or
+ * when (fused head_dim-64 forward, column kernel) the rotary coordinates of a (y, x) column differ between levels,
+ * EVERY row is recomputed that way: still exact, about two orders of magnitude slower, and not predictable from the
+ * descriptor.  To see it, read the first 16 bytes of `workspace` after the stream has completed the call: two
+ * uint64, [0] = rows listed (counts past 65 535 too), [1] != 0 = every row was recomputed.  With QK-RMSNorm
+ * (|logit| <= sqrt(head_dim)) and the paper's level-independent coordinates neither happens.  Only the row SUM is
+ * checked: inputs with |v| near the bf16 maximum can still overflow the fp32 output accumulator. */
+
 /* Backward: B1-B4 of DESIGN.md.  o and lse are the forward's outputs for the same inputs.
  * Writes dq, dk, dv (same layout and dtype as q). */
 strata_status_t strata_na3d_bwd(const strata_na3d_desc_t* desc,

@@ -323,6 +323,13 @@ def desc_for(q: torch.Tensor, window: Sequence[int], rope_axes: int, rope_pairin
                     DTYPE_F32 if q.dtype == torch.float32 else DTYPE_BF16, impl, float(scale))
 
 
+def fixup_stats(workspace: torch.Tensor):
+    """(rows listed for the exact fix-up kernel, take-all flag) that the last tensor-core FORWARD left at the head of
+    `workspace` (include/strata_na3d.h, "exponent range"); synchronises.  Meaningless after a SIMT call."""
+    head = workspace[:16].view(torch.int64).cpu()
+    return int(head[0]), bool(head[1] != 0)
+
+
 def alloc_workspace(nbytes: int, device) -> torch.Tensor:
     return torch.empty(max(int(nbytes), 16), dtype=torch.uint8, device=device)
 

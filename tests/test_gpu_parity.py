@@ -240,8 +240,8 @@ def test_rows_outside_the_exponent_range_take_the_fixup_kernel(oracle_mod, case)
     ws = binding.alloc_workspace(binding.strata_na3d_workspace_bytes(desc, False), "cuda")
     binding.strata_na3d_fwd(desc, dev["q"], dev["k"], dev["v"], None, None, o, lse, ws)
     torch.cuda.synchronize()
-    listed = int(ws.view(torch.int64)[0].item())       # (white box: the fix-up list is the head of the workspace)
-    assert listed >= len(hot), f"fix-up list holds {listed} rows"
+    listed, take_all = binding.fixup_stats(ws)          # (documented in strata_na3d.h: head of the workspace)
+    assert listed >= len(hot) and not take_all, f"fix-up list holds {listed} rows, take-all {take_all}"
     o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window, scale=0.125)
     assert_parity(to_f64(o), o_ref, "bf16", "fixup O")
     assert float(np.abs(to_f64(lse) - lse_ref).max()) < 1e-3, "fixup LSE"
@@ -255,7 +255,14 @@ def test_level_dependent_coordinates_take_the_fixup_kernel(oracle_mod):
     coords = inp["coords"].copy()
     coords[:, 1:, ..., 0] += 3.0 * np.arange(1, w.grid[0], dtype=np.float32)[None, :, None, None]
     inp["coords"] = coords
-    d, o, lse = run_fwd(w, inp)
+    d = device_inputs(w, inp)
+    desc = desc_of(w)
+    o = torch.empty_like(d["q"])
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
+    ws = binding.alloc_workspace(binding.strata_na3d_workspace_bytes(desc, False), "cuda")
+    binding.strata_na3d_fwd(desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], o, lse, ws)
+    torch.cuda.synchronize()
+    assert binding.fixup_stats(ws)[1], "the take-all flag the header documents is not set"
     o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], coords, inp["freqs"], w.window)
     assert_parity(to_f64(o), o_ref, "bf16", "level-dependent coords O")
     assert_parity(to_f64(lse), lse_ref, "bf16", "level-dependent coords LSE", rms_bound=1e-2)
@@ -295,6 +302,58 @@ def test_host_entry_points(oracle_mod):
     ref = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
     for got, r, nm in zip((dq, dk, dv), ref, ("dQ", "dK", "dV")):
         assert_parity(to_f64(got), r, "bf16", f"host {nm}", rms_bound=2e-2)
+
+
+def test_host_entry_points_reuse_their_staging_slots(oracle_mod):
+    """Batch 5 through the per-sample host pipeline (strata_na3d.cu host_pipeline): both staging slots are reused
+    (samples 2, 3, 4 wait for the kernels and the copies out of samples 0, 1, 2) and the final join covers an uneven
+    tail.  The result must equal the device-pointer call on the same inputs bit for bit, forward and backward, and
+    match the oracle.  Second pass: on a side stream with work queued ahead of the call -- a delay, then the copy that
+    fills the pinned Q buffer -- which the pipeline's copy streams have to wait for."""
+    w = wl.small(name="host5", dtype="bf16", value_scale="rsqrt_d", grid=(4, 9, 10), window=(3, 5, 5), heads=2,
+                 head_dim=64, batch=5)
+    inp = wl.make_inputs(w, with_do=True)
+    dev = device_inputs(w, inp)
+    h = {n: (t.pin_memory() if t is not None else None) for n, t in device_inputs(w, inp, device="cpu").items()}
+    desc = desc_of(w)
+    # device-pointer calls (the whole batch in one call)
+    o_d = torch.empty_like(dev["q"])
+    lse_d = torch.empty(desc.lse_shape, dtype=torch.float32, device="cuda")
+    ws = binding.alloc_workspace(max(binding.strata_na3d_workspace_bytes(desc, False),
+                                     binding.strata_na3d_workspace_bytes(desc, True)), "cuda")
+    binding.strata_na3d_fwd(desc, dev["q"], dev["k"], dev["v"], dev["coords"], dev["freqs"], o_d, lse_d, ws)
+    g_d = [torch.empty_like(dev["q"]) for _ in range(3)]
+    binding.strata_na3d_bwd(desc, dev["q"], dev["k"], dev["v"], o_d, dev["do"], lse_d, dev["coords"], dev["freqs"], *g_d, ws)
+    torch.cuda.synchronize()
+    o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window)
+    assert_parity(to_f64(o_d), o_ref, "bf16", "host5 device O")
+
+    ws_f = binding.alloc_workspace(binding.strata_na3d_host_workspace_bytes(desc, False), "cuda")
+    ws_b = binding.alloc_workspace(binding.strata_na3d_host_workspace_bytes(desc, True), "cuda")
+    side = torch.cuda.Stream()
+    for stream in (None, side):
+        o = torch.zeros_like(h["q"]).pin_memory()
+        lse = torch.zeros(desc.lse_shape, dtype=torch.float32).pin_memory()
+        g = [torch.zeros_like(h["q"]).pin_memory() for _ in range(3)]
+        hq = h["q"]
+        if stream is not None:
+            hq = torch.zeros_like(h["q"]).pin_memory()                  # filled by work queued on `stream` before the call
+            with torch.cuda.stream(stream):
+                torch.cuda._sleep(40_000_000)                            # ~20 ms: the call below returns long before this ends
+                hq.copy_(dev["q"], non_blocking=True)
+        binding.strata_na3d_fwd_host(desc, hq, h["k"], h["v"], h["coords"], h["freqs"], o, lse, ws_f, stream=stream)
+        binding.strata_na3d_bwd_host(desc, hq, h["k"], h["v"], o, h["do"], lse, h["coords"], h["freqs"], *g, ws_b,
+                                     stream=stream)
+        (stream or torch.cuda.current_stream()).synchronize()
+        tag = "default stream" if stream is None else "side stream"
+        assert torch.equal(o, o_d.cpu()) and torch.equal(lse, lse_d.cpu()), f"host forward differs ({tag})"
+        for got, ref, nm in zip(g, g_d, ("dQ", "dK", "dV")):
+            assert torch.equal(got, ref.cpu()), f"host {nm} differs ({tag})"
+        assert_parity(to_f64(o), o_ref, "bf16", f"host5 O ({tag})")
+        assert_parity(to_f64(lse), lse_ref, "bf16", f"host5 LSE ({tag})")
+    ref = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
+    for got, r, nm in zip(g, ref, ("dQ", "dK", "dV")):
+        assert_parity(to_f64(got), r, "bf16", f"host5 {nm}", rms_bound=2e-2)
 
 
 def test_device_error_paths_and_stream():
@@ -421,7 +480,31 @@ def test_column_attention(oracle_mod, case):
     kw.update(case)
     w = wl.small(**kw)
     w = dataclasses.replace(w, window=(w.grid[0], 1, 1))
-    check_full(oracle_mod, w, binding.IMPL_AUTO, backward=False)
+    check_full(oracle_mod, w, binding.IMPL_AUTO, backward=True)       # (the (L, 1, 1) backward: CUDA-core kernels)
+
+
+def test_column_window_through_the_host_backward(oracle_mod):
+    """Window (24, 1, 1) (the column-wise blocks) through strata_na3d_fwd_host / _bwd_host, three samples
+    (the third reuses a staging slot)."""
+    w = wl.small(name="colhost", dtype="bf16", value_scale="qknorm", grid=(24, 5, 6), window=(24, 1, 1), heads=2,
+                 head_dim=64, batch=3)
+    inp = wl.make_inputs(w, with_do=True)
+    h = {n: (t.pin_memory() if t is not None else None) for n, t in device_inputs(w, inp, device="cpu").items()}
+    desc = desc_of(w)
+    o = torch.empty_like(h["q"]).pin_memory()
+    lse = torch.empty(desc.lse_shape, dtype=torch.float32).pin_memory()
+    ws = binding.alloc_workspace(max(binding.strata_na3d_host_workspace_bytes(desc, False),
+                                     binding.strata_na3d_host_workspace_bytes(desc, True)), "cuda")
+    binding.strata_na3d_fwd_host(desc, h["q"], h["k"], h["v"], h["coords"], h["freqs"], o, lse, ws)
+    g = [torch.empty_like(h["q"]).pin_memory() for _ in range(3)]
+    binding.strata_na3d_bwd_host(desc, h["q"], h["k"], h["v"], o, h["do"], lse, h["coords"], h["freqs"], *g, ws)
+    torch.cuda.synchronize()
+    o_ref, lse_ref = oracle_mod.na3d_fwd(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window)
+    assert_parity(to_f64(o), o_ref, "bf16", "column host O")
+    assert_parity(to_f64(lse), lse_ref, "bf16", "column host LSE", rms_bound=1e-2)
+    ref = oracle_mod.na3d_bwd(inp["q"], inp["k"], inp["v"], inp["do"], inp["coords"], inp["freqs"], w.window)
+    for got, r, nm in zip(g, ref, ("dQ", "dK", "dV")):
+        assert_parity(to_f64(got), r, "bf16", f"column host {nm}", rms_bound=2e-2)
 
 
 def test_column_attention_with_level_dependent_coordinates(oracle_mod):
