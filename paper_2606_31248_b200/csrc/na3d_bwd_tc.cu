@@ -89,6 +89,9 @@ cudaError_t launch_bwd_tc2_main(const Problem& p, const void* qr, const void* kr
 
 bool tc_bwd_supported(const Problem& p) {
   if (p.dtype != 1 || p.D != 64) return false;
+  // bwd_stat_kernel transposes 2 x kStatTokens x (H + 1) floats through (non-opt-in) shared memory: beyond 191 heads
+  // AUTO takes the CUDA-core backward instead of failing at the launch
+  if ((size_t)2 * kStatTokens * (p.H + 1) * sizeof(float) > 48 * 1024) return false;
 #define X(KL_, KY_, KX_) \
   if (p.kL == KL_ && p.kY == KY_ && p.kX == KX_) return true;
   STRATA_BWD_CONFIGS(X)

@@ -333,8 +333,13 @@ strata_status_t strata_na3d_normgate_fwd(const strata_na3d_desc_t* desc, const v
                                          void* o, float* lse, void* workspace, size_t workspace_bytes, void* stream) {
   Problem p; strata_status_t why;
   if (!make_problem(desc, &p, &why)) return why;
-  if (!q || !k || !o || !(eps >= 0.f)) return STRATA_ERR_INVALID_ARG;
-  if (misaligned(q) || misaligned(k) || misaligned(gate) || misaligned(workspace)) return STRATA_ERR_INVALID_ARG;
+  // every argument is checked before the first kernel is enqueued (the inner strata_na3d_fwd would only see v, lse,
+  // coords, freqs after the two normalisation kernels are already on the stream)
+  if (!q || !k || !v || !o || !lse || !(eps >= 0.f)) return STRATA_ERR_INVALID_ARG;
+  if (p.A > 0 && (!coords || !freqs)) return STRATA_ERR_INVALID_ARG;
+  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(coords) ||
+      misaligned(freqs) || misaligned(gate) || misaligned(workspace))
+    return STRATA_ERR_INVALID_ARG;
   const size_t need = strata_na3d_normgate_workspace_bytes(desc, 0);
   if (need == 0) return STRATA_ERR_UNSUPPORTED;
   if (!workspace || workspace_bytes < need) return STRATA_ERR_WORKSPACE;
@@ -363,8 +368,12 @@ strata_status_t strata_na3d_normgate_bwd(const strata_na3d_desc_t* desc, const v
                                          float* dgate, void* workspace, size_t workspace_bytes, void* stream) {
   Problem p; strata_status_t why;
   if (!make_problem(desc, &p, &why)) return why;
-  if (!q || !k || !o || !d_o || !dq || !dk || !(eps >= 0.f) || (gate && !dgate)) return STRATA_ERR_INVALID_ARG;
-  if (misaligned(q) || misaligned(k) || misaligned(gate) || misaligned(dgate) || misaligned(workspace))
+  if (!q || !k || !v || !o || !d_o || !lse || !dq || !dk || !dv || !(eps >= 0.f) || (gate && !dgate))
+    return STRATA_ERR_INVALID_ARG;                                  // (all of it before the first enqueue, as in the forward)
+  if (p.A > 0 && (!coords || !freqs)) return STRATA_ERR_INVALID_ARG;
+  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(d_o) || misaligned(lse) ||
+      misaligned(coords) || misaligned(freqs) || misaligned(dq) || misaligned(dk) || misaligned(dv) || misaligned(gate) ||
+      misaligned(dgate) || misaligned(workspace))
     return STRATA_ERR_INVALID_ARG;
   const size_t need = strata_na3d_normgate_workspace_bytes(desc, 1);
   if (need == 0) return STRATA_ERR_UNSUPPORTED;
@@ -478,42 +487,54 @@ strata_status_t host_pipeline(const strata_na3d_desc_t* desc, bool backward, con
   STRATA_CK(cudaStreamWaitEvent(hp->s_out, hp->entry, 0));
   if (p.A > 0) STRATA_CK(cudaMemcpyAsync(d_freqs, h_freqs, fb, cudaMemcpyHostToDevice, hp->s_in));
   int launches = 0;
-  for (int b = 0; b < p.B; ++b) {
-    const int s = b & 1;
-    // ---- copies in (slot s was last read by the kernels of sample b - 2)
-    if (b >= 2) STRATA_CK(cudaStreamWaitEvent(hp->s_in, hp->compute_done[s], 0));
-    for (int i = 0; i < n_in; ++i)
-      STRATA_CK(cudaMemcpyAsync(slot_tensor(s, i), static_cast<const char*>(h_in[i]) + (size_t)b * tb, tb,
-                                cudaMemcpyHostToDevice, hp->s_in));
-    if (h_lse_in) STRATA_CK(cudaMemcpyAsync(slot_lse(s), h_lse_in + (size_t)b * (sb / 4), sb, cudaMemcpyHostToDevice, hp->s_in));
-    if (p.A > 0) STRATA_CK(cudaMemcpyAsync(slot_coords(s), h_coords + (size_t)b * (cb / 4), cb, cudaMemcpyHostToDevice, hp->s_in));
-    STRATA_CK(cudaEventRecord(hp->in_ready[s], hp->s_in));
-    // ---- kernels of the sample on the caller's stream (its outputs of sample b - 2 must have left the slot)
-    STRATA_CK(cudaStreamWaitEvent(st, hp->in_ready[s], 0));
-    if (b >= 2) STRATA_CK(cudaStreamWaitEvent(st, hp->out_done[s], 0));
-    strata_status_t rc;
-    if (!backward)
-      rc = strata_na3d_fwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_coords(s), d_freqs,
-                           slot_tensor(s, n_in), slot_lse(s), inner, L.inner, st);
-    else
-      rc = strata_na3d_bwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_tensor(s, 3), slot_tensor(s, 4),
-                           slot_lse(s), slot_coords(s), d_freqs, slot_tensor(s, n_in), slot_tensor(s, n_in + 1),
-                           slot_tensor(s, n_in + 2), inner, L.inner, st);
-    if (rc != STRATA_OK) return rc;
-    launches += g_last_launches;
-    STRATA_CK(cudaEventRecord(hp->compute_done[s], st));
-    // ---- copies out
-    STRATA_CK(cudaStreamWaitEvent(hp->s_out, hp->compute_done[s], 0));
-    for (int i = 0; i < n_out; ++i)
-      STRATA_CK(cudaMemcpyAsync(static_cast<char*>(h_out[i]) + (size_t)b * tb, slot_tensor(s, n_in + i), tb,
-                                cudaMemcpyDeviceToHost, hp->s_out));
-    if (h_lse_out) STRATA_CK(cudaMemcpyAsync(h_lse_out + (size_t)b * (sb / 4), slot_lse(s), sb, cudaMemcpyDeviceToHost, hp->s_out));
-    STRATA_CK(cudaEventRecord(hp->out_done[s], hp->s_out));
-  }
-  // ---- join: the call is complete on `stream` when the last copies out are
-  for (int s = 0; s < 2 && s < p.B; ++s) STRATA_CK(cudaStreamWaitEvent(st, hp->out_done[s], 0));
-  STRATA_CK(cudaEventRecord(hp->entry, hp->s_in));
-  STRATA_CK(cudaStreamWaitEvent(st, hp->entry, 0));
+  // From here on work may sit on the two internal streams: whatever happens, they are joined back into `stream`
+  // before the call returns, so that an error half-way leaves no copy running behind the caller's back.
+  auto enqueue = [&]() -> strata_status_t {
+    for (int b = 0; b < p.B; ++b) {
+      const int s = b & 1;
+      // ---- copies in (slot s was last read by the kernels of sample b - 2)
+      if (b >= 2) STRATA_CK(cudaStreamWaitEvent(hp->s_in, hp->compute_done[s], 0));
+      for (int i = 0; i < n_in; ++i)
+        STRATA_CK(cudaMemcpyAsync(slot_tensor(s, i), static_cast<const char*>(h_in[i]) + (size_t)b * tb, tb,
+                                  cudaMemcpyHostToDevice, hp->s_in));
+      if (h_lse_in) STRATA_CK(cudaMemcpyAsync(slot_lse(s), h_lse_in + (size_t)b * (sb / 4), sb, cudaMemcpyHostToDevice, hp->s_in));
+      if (p.A > 0) STRATA_CK(cudaMemcpyAsync(slot_coords(s), h_coords + (size_t)b * (cb / 4), cb, cudaMemcpyHostToDevice, hp->s_in));
+      STRATA_CK(cudaEventRecord(hp->in_ready[s], hp->s_in));
+      // ---- kernels of the sample on the caller's stream (its outputs of sample b - 2 must have left the slot)
+      STRATA_CK(cudaStreamWaitEvent(st, hp->in_ready[s], 0));
+      if (b >= 2) STRATA_CK(cudaStreamWaitEvent(st, hp->out_done[s], 0));
+      strata_status_t rc;
+      if (!backward)
+        rc = strata_na3d_fwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_coords(s), d_freqs,
+                             slot_tensor(s, n_in), slot_lse(s), inner, L.inner, st);
+      else
+        rc = strata_na3d_bwd(&d1, slot_tensor(s, 0), slot_tensor(s, 1), slot_tensor(s, 2), slot_tensor(s, 3), slot_tensor(s, 4),
+                             slot_lse(s), slot_coords(s), d_freqs, slot_tensor(s, n_in), slot_tensor(s, n_in + 1),
+                             slot_tensor(s, n_in + 2), inner, L.inner, st);
+      if (rc != STRATA_OK) return rc;
+      launches += g_last_launches;
+      STRATA_CK(cudaEventRecord(hp->compute_done[s], st));
+      // ---- copies out
+      STRATA_CK(cudaStreamWaitEvent(hp->s_out, hp->compute_done[s], 0));
+      for (int i = 0; i < n_out; ++i)
+        STRATA_CK(cudaMemcpyAsync(static_cast<char*>(h_out[i]) + (size_t)b * tb, slot_tensor(s, n_in + i), tb,
+                                  cudaMemcpyDeviceToHost, hp->s_out));
+      if (h_lse_out) STRATA_CK(cudaMemcpyAsync(h_lse_out + (size_t)b * (sb / 4), slot_lse(s), sb, cudaMemcpyDeviceToHost, hp->s_out));
+      STRATA_CK(cudaEventRecord(hp->out_done[s], hp->s_out));
+    }
+    return STRATA_OK;
+  };
+  auto join = [&]() -> strata_status_t {                             // `stream` waits for everything on s_out and s_in
+    STRATA_CK(cudaEventRecord(hp->entry, hp->s_out));
+    STRATA_CK(cudaStreamWaitEvent(st, hp->entry, 0));
+    STRATA_CK(cudaEventRecord(hp->entry, hp->s_in));
+    STRATA_CK(cudaStreamWaitEvent(st, hp->entry, 0));
+    return STRATA_OK;
+  };
+  const strata_status_t rc_enqueue = enqueue();
+  const strata_status_t rc_join = join();
+  if (rc_enqueue != STRATA_OK) return rc_enqueue;
+  if (rc_join != STRATA_OK) return rc_join;
   g_last_launches = launches;
   return STRATA_OK;
 }

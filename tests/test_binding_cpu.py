@@ -66,6 +66,37 @@ def test_status_codes_without_touching_the_gpu(L):
     assert bw(d, ok11[:9] + [None, vp(0x1000)], vp(0x1000), 1 << 30) == 1
 
 
+def test_normgate_calls_validate_everything_before_enqueuing(L):
+    """strata_na3d_normgate_fwd / _bwd: a null or misaligned v, lse, o, dv ... is refused on the host, before the
+    normalisation kernels go on the stream (no GPU here: reaching a launch would return CUDA, not INVALID_ARG)."""
+    d = _desc()
+    vp = ctypes.c_void_p
+    a = vp(0x1000)
+    fwd = lambda q, k, v, co, fr, g, o, lse: L.strata_na3d_normgate_fwd(ctypes.byref(d.c()), q, k, v, co, fr, g, 1e-6, o, lse,
+                                                                       a, 1 << 30, None)
+    assert fwd(a, a, None, a, a, None, a, a) == 1                        # null v
+    assert fwd(a, a, a, a, a, None, a, None) == 1                        # null lse
+    assert fwd(a, a, vp(0x1004), a, a, None, a, a) == 1                  # misaligned v
+    assert fwd(a, a, a, None, a, None, a, a) == 1                        # rope_axes = 2 without coords
+    assert fwd(a, a, a, a, a, None, vp(0x1008), a) == 1                  # misaligned o
+    bwd = lambda v, lse, dv: L.strata_na3d_normgate_bwd(ctypes.byref(d.c()), a, a, v, a, a, lse, a, a, None, 1e-6, a, a, dv,
+                                                        None, a, 1 << 30, None)
+    assert bwd(None, a, a) == 1 and bwd(a, None, a) == 1 and bwd(a, a, None) == 1 and bwd(a, a, vp(0x1002)) == 1
+
+
+def test_backward_family_respects_the_head_limit_of_the_statistics_kernel(L):
+    """The tcgen05 backward's statistics pass stages 2 x 32 x (H + 1) floats in 48 KiB of shared memory: up to 191
+    heads.  Past that AUTO must resolve to the CUDA-core backward (and an explicit TCGEN05 request is UNSUPPORTED)
+    instead of failing at the launch."""
+    bf = lambda heads, impl=binding.IMPL_AUTO: _desc(dtype=binding.DTYPE_BF16, head_dim=64, window=(3, 7, 7),
+                                                     grid=(4, 16, 16), heads=heads, impl=impl)
+    assert binding.strata_na3d_impl_selected(bf(191), True) == binding.IMPL_TCGEN05
+    assert binding.strata_na3d_impl_selected(bf(192), True) == binding.IMPL_SIMT
+    assert binding.strata_na3d_impl_selected(bf(192, binding.IMPL_TCGEN05), True) == -1
+    assert binding.strata_na3d_workspace_bytes(bf(192), True) >= 4 * 1024 * 192 * 64 * 4      # fp32 rotated copies + grads
+    assert binding.strata_na3d_impl_selected(bf(192), False) == binding.IMPL_TCGEN05           # the forward has no such limit
+
+
 def test_window_and_inverse_window_against_brute_force(L):
     """A3 / B3 as the kernels compute them (csrc/common.cuh) against the definition by enumeration:
     "centre the window on the query, then shift it inward until it fits" (PAPER.md:79 + reading R1),
