@@ -36,8 +36,7 @@ def _compile(src: str) -> str:
     hdr_m = _deps_mtime()
     if os.path.exists(obj) and os.path.getmtime(obj) >= hdr_m:
         return obj
-    extra = os.environ.get("STRATA_NVCC_EXTRA", "").split()          # e.g. -DSTRATA_TRACE (debug builds)
-    r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", obj], capture_output=True, text=True)
+    r = subprocess.run(["nvcc"] + NVCC_FLAGS + ["-c", src, "-o", obj], capture_output=True, text=True)
     with open(log, "w") as f:
         f.write(r.stdout + r.stderr)
     if r.returncode != 0:

@@ -199,7 +199,7 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++Tn) {
         const Tile2 T = tile_of(t);
         const int par = Tn & 1, bl = T.b * p.L;
-        mbar_wait(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
+        mbar_wait_bounded(bar_aempty(par), ((uint32_t)(Tn >> 1) & 1u) ^ 1u);
         if (elect_one()) {
           mbar_expect_tx(bar_afull(par), 2 * C::TILE_BYTES);
           tma_load_5d(a_smem(par, 0), &tm_a1, bar_afull(par), 0, T.h, T.x0, T.y0, bl + T.l0);
@@ -213,7 +213,7 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
               const uint32_t ph = (uint32_t)(Cn / C::NSTAGE) & 1u;
               const uint32_t sb = st_smem + s * C::STAGE_BYTES;
               const int gx = T.bx0 + cx * C::HX, gy = T.by0 + cy * C::CY;
-              mbar_wait(bar_empty(s), ph ^ 1u);
+              mbar_wait_bounded(bar_empty(s), ph ^ 1u);
               if (elect_one()) {
                 mbar_expect_tx(bar_full(s), 2 * C::NCOL * 128 + (MODE == 1 ? C::NCOL * 16 : 0));
                 tma_load_5d(sb, &tm_b1, bar_full(s), 0, T.h, gx, gy, bl + pl);
@@ -437,7 +437,7 @@ na3d_bwd_tc2_kernel(const __grid_constant__ CUtensorMap tm_a1, const __grid_cons
       const int ax = min(x0 + rx, p.X - 1), ay = min(y0 + ry, p.Y - 1), al = min(l0 + rl, p.L - 1);
       const long long tok = ((long long)al * p.Y + ay) * p.X + ax;
       const int ai = Tn % NACC, ak = Tn / NACC;
-      mbar_wait(bar_accdone(ai), (uint32_t)ak & 1u);
+      mbar_wait_bounded(bar_accdone(ai), (uint32_t)ak & 1u);
       tc_fence_after();
       const uint32_t acc = tm + C::TMEM_ACC + ACC_STRIDE * ai;
       uint32_t vw[MODE == 1 ? C::D / 2 : 1];

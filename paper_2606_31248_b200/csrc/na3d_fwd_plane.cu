@@ -335,7 +335,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
         const int li = it.cl * p.L + plane, s = li % ns;
         const uint32_t ph = (uint32_t)(li / ns) & 1u;
         const uint32_t full = isv ? bar_vfull(s) : bar_kfull(s);
-        mbar_wait(isv ? bar_vempty(s) : bar_kempty(s), ph ^ 1u);
+        mbar_wait_bounded(isv ? bar_vempty(s) : bar_kempty(s), ph ^ 1u);
         if (elect_one()) {
           mbar_expect_tx(full, (uint32_t)(C::NTOK * 128));
           tma_load_5d(stage0 + s * C::STAGE, map, full, 0, c.h, c.hs_x, c.hs_y, c.b * p.L + plane);
@@ -788,7 +788,7 @@ na3d_fwd_plane_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_con
             // ---- this pair handled the last plane of the tile: its epilogue (O / l -> bf16 -> global, LSE), in the
             // shadow of the P V and Q K^T the pair waits for anyway.  Each of the two warps of a subpartition takes
             // half of the O row.
-            mbar_wait(bar_pvdone, (uint32_t)T & 1u);
+            mbar_wait_bounded(bar_pvdone, (uint32_t)T & 1u);
             tc_fence_after();
             const uint32_t la = ls_row + (uint32_t)(T & 1) * 2048u;      // (read before O is released: tile T + 2 reuses the slots)
             const float ltot = (lds32(la) + lds32(la + 512)) + (lds32(la + 1024) + lds32(la + 1536));

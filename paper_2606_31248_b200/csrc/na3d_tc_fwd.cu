@@ -146,7 +146,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       auto load_v = [&](int c, int pl, int cy) {
         const int s = c % C::NSTAGE;
         const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
-        mbar_wait(bar_vempty(s), ph ^ 1u);
+        mbar_wait_bounded(bar_vempty(s), ph ^ 1u);
         if (elect_one()) {
           mbar_expect_tx(bar_vfull(s), C::STAGE_BYTES);
           for (int j = 0; j < C::DSUB; ++j)
@@ -160,7 +160,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         for (int cy = 0; cy < ncy; ++cy, ++c) {
           const int s = c % C::NSTAGE;
           const uint32_t ph = (uint32_t)(c / C::NSTAGE) & 1u;
-          mbar_wait(bar_kempty(s), ph ^ 1u);
+          mbar_wait_bounded(bar_kempty(s), ph ^ 1u);
           if (elect_one()) {
             mbar_expect_tx(bar_kfull(s), C::STAGE_BYTES);
             for (int j = 0; j < C::DSUB; ++j)
@@ -293,7 +293,7 @@ na3d_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       }
     }
     // ---- epilogue: O / l -> bf16 -> global, LSE
-    mbar_wait(bar_pvdone + 8u * ((nchunks - 1) & 1), (uint32_t)((nchunks - 1) >> 1) & 1u);
+    mbar_wait_bounded(bar_pvdone + 8u * ((nchunks - 1) & 1), (uint32_t)((nchunks - 1) >> 1) & 1u);
     tc_fence_after();
     const float inv = 1.f / lsum;
     const long long tok = ((long long)al * p.Y + ay) * p.X + ax;

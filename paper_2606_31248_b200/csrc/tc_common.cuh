@@ -4,9 +4,6 @@
 #include <cuda.h>
 
 #include <mutex>
-#ifdef STRATA_DEBUG_SYNC
-#include <cstdio>
-#endif
 
 #include "common.cuh"
 
@@ -32,11 +29,24 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 // sixteen warps of a CTA sit in such loops, and every extra instruction per poll is taken from the issue slots
 // of the working warps (a suspend-time hint, a nanosleep or a poll counter cost more than they save: the sleeps
 // return after a few nanoseconds while other warps signal barriers).
-// STRATA_DEBUG_SYNC: bounded wait, a protocol bug becomes a trap after ~1 s instead of a hung GPU.
 template <bool SLEEP = true>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-#ifdef STRATA_DEBUG_SYNC
-  uint32_t spins = 0;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@!p bra WAIT_LOOP;\n\t}"
+      :: "r"(bar), "r"(parity) : "memory");
+}
+// The same wait with a bound, for the waiters that are off the critical path (TMA producers, epilogues): every
+// 65 536 failed polls (a millisecond or more) it looks at the global timer and traps once the wait has lasted more
+// than kWaitBoundNs.  A protocol or parity bug normally stalls every role of a CTA, the producers and epilogues
+// among them, so it ends as a failed launch (cudaErrorLaunchFailure) after a few seconds instead of a GPU that hangs
+// until the process is killed.  No kernel of this library runs longer than tens of milliseconds.
+constexpr unsigned long long kWaitBoundNs = 4000000000ull;
+__device__ __forceinline__ void mbar_wait_bounded(uint32_t bar, uint32_t parity) {
+  uint32_t polls = 0;
+  unsigned long long t0 = 0;
   for (;;) {
     uint32_t ok;
     asm volatile(
@@ -44,20 +54,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (ok) break;
-    if (++spins > 20000000u) {
-      printf("mbar timeout: block %d thread %d bar 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
-      __trap();
+    if (ok) return;
+    if ((++polls & 0xffffu) == 0) {
+      unsigned long long now;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > kWaitBoundNs) __trap();
     }
   }
-#else
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@!p bra WAIT_LOOP;\n\t}"
-      :: "r"(bar), "r"(parity) : "memory");
-#endif
 }
 // One lane of a converged warp (all 32 lanes must execute this).
 __device__ __forceinline__ bool elect_one() {
@@ -202,7 +206,25 @@ inline cudaError_t ensure_smem_attr(DeviceState* ds, std::mutex& mu, int slot, K
 
 // Tensor [B*L, Y, X, H, D] bf16 as a rank-5 map (fastest first: d, h, x, y, b*l); box = 64 channels of
 // one head x (bx, by, bl) tokens, 128-byte swizzle, out-of-bounds reads return zero.
+// Encoding a map costs a driver call (~1 us); callers pass the same tensors step after step, so the last few maps
+// are kept per host thread, keyed by everything the encoding depends on (base pointer, tensor shape, box).
 inline bool make_map(CUtensorMap* map, const void* ptr, const Problem& p, int bx, int by, int bl) {
+  struct Entry {
+    const void* ptr = nullptr;
+    long long bl_rows = 0;
+    int D = 0, H = 0, X = 0, Y = 0, bx = 0, by = 0, bl = 0;
+    CUtensorMap map;
+  };
+  constexpr int kEntries = 16;
+  thread_local Entry cache[kEntries];
+  thread_local int next = 0;
+  const long long bl_rows = (long long)p.B * p.L;
+  for (const Entry& c : cache)
+    if (c.ptr == ptr && ptr && c.bl_rows == bl_rows && c.D == p.D && c.H == p.H && c.X == p.X && c.Y == p.Y && c.bx == bx &&
+        c.by == by && c.bl == bl) {
+      *map = c.map;
+      return true;
+    }
   EncodeTiledFn fn = encode_fn();
   if (!fn) return false;
   const cuuint64_t dims[5] = {(cuuint64_t)p.D, (cuuint64_t)p.H, (cuuint64_t)p.X, (cuuint64_t)p.Y,
@@ -212,9 +234,15 @@ inline bool make_map(CUtensorMap* map, const void* ptr, const Problem& p, int bx
                                  (cuuint64_t)p.Y * p.X * p.H * p.D * e};
   const cuuint32_t box[5] = {64, 1, (cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bl};
   const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-  return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(ptr), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  if (fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(ptr), dims, strides, box, estr,
+         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return false;
+  Entry& slot = cache[next];
+  next = (next + 1) % kEntries;
+  slot.ptr = ptr; slot.bl_rows = bl_rows; slot.D = p.D; slot.H = p.H; slot.X = p.X; slot.Y = p.Y;
+  slot.bx = bx; slot.by = by; slot.bl = bl; slot.map = *map;
+  return true;
 }
 
 
