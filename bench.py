@@ -301,7 +301,49 @@ def cpu_baseline(w: wl.Workload, sess: Session, seconds: float = 12.0):
             "tokens_per_s": (n / w.heads) / dt}
 
 
-def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=True):
+def measure_streaming(peaks, w: wl.Workload, steps: int = 20):
+    """The elementwise kernels around the attention (NEXT rows of SURVEY.md §8(f)) as HBM streams: bytes each must
+    move / time / measured copy bandwidth.  Sizes follow config 3 (24 tiles of 128 x 128 patches, stride 112, 8 levels),
+    scaled so that every working set exceeds the 126 MB L2 (no flush needed); inputs are seeded torch.rand."""
+    import torch
+    from paper_2606_31248_b200 import binding
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev); g.manual_seed(wl.BASE_SEED + 7)
+    out = {}
+
+    def run(name, fn, nbytes, note):
+        for _ in range(3):
+            fn()
+        ms = time_steps(torch, fn, steps)
+        gbs = nbytes / (ms * 1e-3) / 1e9
+        out[name] = {"ms": ms, "bytes": int(nbytes), "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peaks["hbm_gbs"], "size": note}
+
+    n = 4 * w.batch * w.tokens                                        # eq. (1) / eq. (2): points
+    lat = (torch.rand(n, generator=g, device=dev, dtype=torch.float64) - 0.5) * 0.4 + 0.3
+    lon = (torch.rand(n, generator=g, device=dev, dtype=torch.float64) - 0.5) * 0.4 + 1.0
+    coords = torch.empty(n, 2, device=dev)
+    run("stereo_coords", lambda: binding.strata_stereo_coords(lat, lon, 0.3, 1.0, float(wl.N_TOTAL), coords), n * 24,
+        f"{n} points (4 x config 3's tokens): 16 B in, 8 B out")
+    u, v = torch.rand(n, generator=g, device=dev), torch.rand(n, generator=g, device=dev)
+    ul, vl = torch.empty_like(u), torch.empty_like(v)
+    run("wind_to_tile_frame", lambda: binding.strata_wind_to_tile_frame(u, v, lat, lon, 0.3, 1.0, ul, vl), n * 32,
+        f"{n} points: 8 + 16 B in, 8 B out")
+    del lat, lon, coords, u, v, ul, vl
+    T, C, th, st = 24, 128, 128, 112                                  # eq. (5): six faces of 2 x 2 tiles side by side
+    origins = torch.tensor([(ty * st, f * (th + st) + tx * st) for f in range(6) for ty in range(2) for tx in range(2)],
+                           dtype=torch.int32, device=dev)
+    gh, gw = th + st, 6 * (th + st)
+    tiles = torch.rand(T, C, th, th, generator=g, device=dev)
+    win = torch.sin(torch.arange(th, device=dev, dtype=torch.float32).add(0.5).mul(3.141592653589793 / th))
+    field = torch.empty(C, gh, gw, device=dev)
+    run("tile_stitch", lambda: binding.strata_tile_stitch(tiles, origins, win, win, field),
+        tiles.numel() * 4 + field.numel() * 4, f"{T} tiles x {C} channels x {th} x {th}, stride {st} -> [{C}, {gh}, {gw}]")
+    del tiles, field
+    torch.cuda.empty_cache()
+    return out
+
+
+def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=True, with_normgate=False):
     import torch
     from paper_2606_31248_b200 import binding
     dev = torch.device("cuda", torch.cuda.current_device())
@@ -312,11 +354,13 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
     launches_per_step = binding.strata_na3d_last_launch_count()
     sampler = ClockSampler(torch.cuda.current_device())
     sampler.start()
+    ms = time_steps(torch, sess.step, args.steps, dist)          # the headline: nothing but the library's own launches
+    clocks = sampler.stop()
+    # per-kernel times come from a loop of their own (two event records per kernel would sit in the timed region)
     binding.strata_na3d_set_profiling(True)
-    ms = time_steps(torch, sess.step, args.steps, dist)
+    time_steps(torch, sess.step, args.steps, None)
     prof = binding.strata_na3d_profile_read()
     binding.strata_na3d_set_profiling(False)
-    clocks = sampler.stop()
     per_kernel = {}
     for name, t in prof:
         per_kernel.setdefault(name, []).append(t)
@@ -340,6 +384,29 @@ def measure(w: wl.Workload, args, dist, rank, peaks, with_e2e=True, with_cpu=Tru
     out = {"ms_per_step": ms, "tflops": tflops, "tokens_per_s": tok_s, "launches_per_step": launches_per_step,
            "roofline": roofline, "clocks": clocks,
            "impl": {0: "auto", 1: "simt", 2: "tcgen05"}.get(binding.strata_na3d_impl_selected(sess.desc, w.backward))}
+    if with_normgate and not w.backward:
+        # PAPER.md:390 around the same forward: QK-RMSNorm + head gate.  A fused version would move the same bytes as the
+        # plain forward plus 4 B of gate logit per (token, head); today three streaming kernels surround the attention.
+        gate = torch.zeros((w.batch,) + tuple(w.grid) + (w.heads,), dtype=torch.float32, device=dev)
+        ws_ng = binding.alloc_workspace(binding.strata_na3d_normgate_workspace_bytes(sess.desc, False), dev)
+        d = sess.dev
+        ng = lambda: binding.strata_na3d_normgate_fwd(sess.desc, d["q"], d["k"], d["v"], d["coords"], d["freqs"], gate, 1e-6,
+                                                      sess.o, sess.lse, ws_ng)
+        for _ in range(3):
+            ng()
+        k_ng = max(3, min(args.steps, 10))
+        ms_ng = time_steps(torch, ng, k_ng, None)
+        binding.strata_na3d_set_profiling(True)
+        ng(); torch.cuda.synchronize()
+        ng_kernels = {}
+        for name, t in binding.strata_na3d_profile_read():
+            ng_kernels[name] = ng_kernels.get(name, 0.0) + t
+        binding.strata_na3d_set_profiling(False)
+        ideal = (bytes_ + gate.numel() * 4) / (peaks["hbm_gbs"] * 1e9) * 1e3
+        out["normgate_fwd"] = {"ms_per_step": ms_ng, "steps": k_ng, "vs_plain_forward": ms_ng / ms,
+                               "launches_per_step": binding.strata_na3d_last_launch_count(),
+                               "frac_of_roofline": ideal / ms_ng, "kernels_ms": ng_kernels}
+        del gate, ws_ng
     if with_e2e:
         n_in, n_out = sess.setup_e2e()
         sess.step_e2e(); torch.cuda.synchronize()
@@ -384,7 +451,7 @@ def main():
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist = dist_mod
     peaks = load_peaks()
-    main_res = measure(w, args, dist, rank, peaks)
+    main_res = measure(w, args, dist, rank, peaks, with_normgate=(world == 1 and bool(args.extras)))
     others = {}
     if args.extras and world == 1:
         short = argparse.Namespace(**{**vars(args), "steps": max(3, min(args.steps, 10)), "e2e_steps": 1})
@@ -393,6 +460,9 @@ def main():
             others[name] = {"ms_per_step": r["ms_per_step"], "tflops": r["tflops"], "tokens_per_s": r["tokens_per_s"],
                             "frac_of_roofline": r["roofline"]["step_frac_of_roofline"], "impl": r["impl"],
                             "kernels_ms": r["roofline"]["kernels_ms"]}
+        if "normgate_fwd" in main_res:
+            others["normgate_fwd_" + args.workload] = main_res["normgate_fwd"]
+        others["streaming_kernels"] = measure_streaming(peaks, w, steps=max(3, min(args.steps, 20)))
     if rank == 0:
         line = {"metric": METRIC, "value": main_res["tflops"], "unit": "TFLOP/s", "n_gpus": args.gpus,
                 "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": main_res["ms_per_step"],

@@ -47,10 +47,11 @@ wind_frame_kernel(const float* __restrict__ u, const float* __restrict__ v, cons
   }
 }
 
-// eq. (5): out = D^-1 P^T W y for tiles that lie inside the field (P copies cells).  One thread per
-// cell of the [C, GH, GW] field; every tile that covers the cell contributes wy[dy] wx[dx] y_t[c, dy, dx].
+// eq. (5): out = D^-1 P^T W y for tiles that lie inside the field (P copies cells).  Generic form, one
+// thread per cell of the [C, GH, GW] field looking at every tile: kept for layouts the row kernel below does not take
+// (more than kStitchMaxTiles tiles, more than 65 535 rows).  Both kernels add the tiles in ascending order: same bits.
 __global__ void __launch_bounds__(256)
-tile_stitch_kernel(const float* __restrict__ tiles, const int* __restrict__ origins, int T, int C, int th, int tw,
+tile_stitch_generic_kernel(const float* __restrict__ tiles, const int* __restrict__ origins, int T, int C, int th, int tw,
                    const float* __restrict__ wy, const float* __restrict__ wx, float* __restrict__ out, int GH, int GW) {
   const long long n = (long long)C * GH * GW;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
@@ -64,6 +65,82 @@ tile_stitch_kernel(const float* __restrict__ tiles, const int* __restrict__ orig
       den += w;
     }
     out[i] = den > 0.f ? num / den : 0.f;
+  }
+}
+
+// The same sum as a stream (HBM-bound: every tile cell is read once, every field cell written once).  A block owns 256
+// consecutive cells of one field row for a group of channels.  Warp 0 lists, in ascending order, the tiles that touch
+// that row segment (a handful out of T); every thread turns the list into the (weight, offset) pairs of its own cell
+// once -- up to kStitchLocal of them in registers -- and then walks the channels with coalesced loads and stores.
+constexpr int kStitchMaxTiles = 1024, kStitchLocal = 8;
+__global__ void __launch_bounds__(256)
+tile_stitch_rows_kernel(const float* __restrict__ tiles, const int* __restrict__ origins, int T, int C, int th, int tw,
+                        const float* __restrict__ wy, const float* __restrict__ wx, float* __restrict__ out, int GH, int GW,
+                        int c_per_block) {
+  __shared__ int s_list[kStitchMaxTiles];
+  __shared__ int s_cnt;
+  const int gy = blockIdx.y, x0 = blockIdx.x * 256, gx = x0 + threadIdx.x;
+  if (threadIdx.x < 32) {
+    int cnt = 0;
+    for (int base = 0; base < T; base += 32) {
+      const int t = base + threadIdx.x;
+      bool hit = false;
+      if (t < T) {
+        const int oy = origins[2 * t], ox = origins[2 * t + 1];
+        hit = gy >= oy && gy < oy + th && ox < x0 + 256 && ox + tw > x0;
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, hit);
+      if (hit) s_list[cnt + __popc(m & ((1u << threadIdx.x) - 1u))] = t;
+      cnt += __popc(m);
+    }
+    if (threadIdx.x == 0) s_cnt = cnt;
+  }
+  __syncthreads();
+  if (gx >= GW) return;
+  const int cnt = s_cnt;
+  const long long plane = (long long)th * tw;
+  const int c0 = blockIdx.z * c_per_block, c1 = min(C, c0 + c_per_block);
+  float w[kStitchLocal];
+  long long off[kStitchLocal];
+  int mine = 0;                                     // tiles that cover this cell (ascending), first kStitchLocal in registers
+  float den = 0.f;
+  bool overflow = false;
+  for (int k = 0; k < cnt; ++k) {
+    const int t = s_list[k];
+    const int dy = gy - origins[2 * t], dx = gx - origins[2 * t + 1];
+    if (dx < 0 || dx >= tw) continue;
+    const float wk = wy[dy] * wx[dx];
+    den += wk;
+    if (mine < kStitchLocal) {
+#pragma unroll
+      for (int u = 0; u < kStitchLocal; ++u)
+        if (u == mine) { w[u] = wk; off[u] = (long long)t * C * plane + (long long)dy * tw + dx; }
+    } else {
+      overflow = true;
+    }
+    ++mine;
+  }
+  const float inv_ok = den > 0.f ? 1.f : 0.f;
+  if (!overflow) {
+#pragma unroll 4
+    for (int c = c0; c < c1; ++c) {
+      float num = 0.f;
+#pragma unroll
+      for (int u = 0; u < kStitchLocal; ++u)
+        if (u < mine) num = fmaf(w[u], tiles[off[u] + c * plane], num);
+      out[((long long)c * GH + gy) * GW + gx] = inv_ok != 0.f ? num / den : 0.f;
+    }
+  } else {                                          // more than kStitchLocal tiles over one cell: walk the list per channel
+    for (int c = c0; c < c1; ++c) {
+      float num = 0.f;
+      for (int k = 0; k < cnt; ++k) {
+        const int t = s_list[k];
+        const int dy = gy - origins[2 * t], dx = gx - origins[2 * t + 1];
+        if (dx < 0 || dx >= tw) continue;
+        num = fmaf(wy[dy] * wx[dx], tiles[(((long long)t * C + c) * th + dy) * tw + dx], num);
+      }
+      out[((long long)c * GH + gy) * GW + gx] = inv_ok != 0.f ? num / den : 0.f;
+    }
   }
 }
 
@@ -109,8 +186,18 @@ strata_status_t strata_tile_stitch(const float* tiles, const int32_t* origins, i
     return STRATA_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   strata::prof_begin("tile_stitch", st);
-  strata::tile_stitch_kernel<<<strata::grid_for((long long)channels * gh * gw), 256, 0, st>>>(tiles, origins, n_tiles, channels, th, tw,
-                                                                                       wy, wx, out, gh, gw);
+  const long long xy_blocks = (long long)gh * ((gw + 255) / 256);
+  if (n_tiles <= strata::kStitchMaxTiles && gh <= 65535) {
+    // channel groups: enough blocks to fill the GPU several times over, at most one group per channel
+    long long groups = (148LL * 16 + xy_blocks - 1) / xy_blocks;
+    groups = groups < 1 ? 1 : groups > channels ? channels : groups > 65535 ? 65535 : groups;
+    const int c_per_block = (int)((channels + groups - 1) / groups);
+    const dim3 grid((unsigned)((gw + 255) / 256), (unsigned)gh, (unsigned)((channels + c_per_block - 1) / c_per_block));
+    strata::tile_stitch_rows_kernel<<<grid, 256, 0, st>>>(tiles, origins, n_tiles, channels, th, tw, wy, wx, out, gh, gw, c_per_block);
+  } else {
+    strata::tile_stitch_generic_kernel<<<strata::grid_for((long long)channels * gh * gw), 256, 0, st>>>(tiles, origins, n_tiles, channels,
+                                                                                               th, tw, wy, wx, out, gh, gw);
+  }
   strata::prof_end(st);
   if (cudaGetLastError() != cudaSuccess) return STRATA_ERR_CUDA;
   return STRATA_OK;

@@ -624,3 +624,27 @@ def test_tile_stitch_kernel(oracle_mod):
         ref = oracle_mod.stitch.stitch(tiles, origins, wy, wy, gh, gw)
         err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
         assert err.max() <= 1e-5, f"stitch: max abs err {err.max():.3e}"
+
+
+@pytest.mark.parametrize("case", ["twelve_deep", "many_tiles"])
+def test_tile_stitch_kernel_other_layouts(oracle_mod, case):
+    """eq. (5) where the row kernel leaves its fast path: twelve tiles over the same cells (more than the eight it keeps
+    in registers) and 1100 small tiles (more than its list holds: the generic kernel).  Tiles overlap at random, some
+    cells are covered by none (-> 0)."""
+    rng = np.random.default_rng(29)
+    if case == "twelve_deep":
+        T, C, th, tw, gh, gw = 12, 3, 16, 16, 40, 300
+        origins = np.array([(i, i) for i in range(T)], dtype=np.int32)      # cells (11..15, 11..15) lie under all twelve
+    else:
+        T, C, th, tw, gh, gw = 1100, 2, 3, 5, 64, 70
+        origins = np.stack([rng.integers(0, gh - th + 1, T), rng.integers(0, gw - tw + 1, T)], axis=1).astype(np.int32)
+    tiles = rng.normal(size=(T, C, th, tw)).astype(np.float32)
+    wy = rng.uniform(0.1, 1.0, th).astype(np.float32)
+    wx = rng.uniform(0.1, 1.0, tw).astype(np.float32)
+    out = torch.full((C, gh, gw), 7.0, dtype=torch.float32, device="cuda")
+    binding.strata_tile_stitch(torch.from_numpy(tiles).cuda(), torch.from_numpy(origins).cuda(), torch.from_numpy(wy).cuda(),
+                               torch.from_numpy(wx).cuda(), out)
+    ref = oracle_mod.stitch.stitch(tiles, origins, wy, wx, gh, gw)
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
+    assert err.max() <= 1e-5 * max(1.0, np.abs(ref).max()), f"stitch {case}: max abs err {err.max():.3e}"
+    assert (ref == 0).any() and (ref != 0).any()
