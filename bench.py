@@ -33,7 +33,7 @@ from paper_2606_31248_b200 import workloads as wl  # noqa: E402
 
 WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4,
              # not BASELINE.json configs: the paper's own attention shapes (workloads.production), as extras
-             "prod16": "prod16", "prod32": "prod32", "col16": "col16", "col32": "col32"}
+             "prod16": "prod16", "prod32": "prod32", "col16": "col16", "col32": "col32", "dec64": "dec64"}
 
 
 def workload_of(key: str) -> wl.Workload:
@@ -431,7 +431,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--extras", default="cfg1,cfg2,cfg4,prod32,col32", help="other configs summarised in the same line ('' = none)")
+    ap.add_argument("--extras", default="cfg1,cfg2,cfg4,prod32,col32,dec64", help="other configs summarised in the same line ('' = none)")
     args = ap.parse_args()
     w = workload_of(args.workload)
     if args.impl == "reference":

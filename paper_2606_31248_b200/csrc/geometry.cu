@@ -122,8 +122,23 @@ tile_stitch_rows_kernel(const float* __restrict__ tiles, const int* __restrict__
   }
   const float inv_ok = den > 0.f ? 1.f : 0.f;
   if (!overflow) {
-#pragma unroll 4
-    for (int c = c0; c < c1; ++c) {
+    constexpr int CU = 8;                           // channels per pass: their loads are independent (memory-level parallelism)
+    int c = c0;
+    for (; c + CU <= c1; c += CU) {
+      float num[CU];
+#pragma unroll
+      for (int j = 0; j < CU; ++j) num[j] = 0.f;
+#pragma unroll
+      for (int u = 0; u < kStitchLocal; ++u)
+        if (u < mine) {
+          const float* src = tiles + off[u] + c * plane;
+#pragma unroll
+          for (int j = 0; j < CU; ++j) num[j] = fmaf(w[u], __ldcs(src + j * plane), num[j]);
+        }
+#pragma unroll
+      for (int j = 0; j < CU; ++j) __stcs(out + ((long long)(c + j) * GH + gy) * GW + gx, inv_ok != 0.f ? num[j] / den : 0.f);
+    }
+    for (; c < c1; ++c) {
       float num = 0.f;
 #pragma unroll
       for (int u = 0; u < kStitchLocal; ++u)

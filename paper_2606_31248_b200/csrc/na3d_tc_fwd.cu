@@ -373,7 +373,8 @@ cudaError_t launch_cfg(int slot, const Problem& p, const void* qr, const void* k
   X(1, 128, 5, 9, 9)         \
   X(2, 64, 3, 5, 5)          \
   X(3, 64, 3, 3, 3)          \
-  X(4, 64, 9, 9, 9)
+  X(4, 64, 9, 9, 9)         \
+  X(5, 128, 9, 9, 9)
 
 bool tc_fwd_supported(const Problem& p) {
   if (p.dtype != 1) return false;

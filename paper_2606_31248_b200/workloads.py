@@ -107,8 +107,13 @@ def production(which: str) -> Workload:
     """The paper's own attention shapes (PAPER.md:325-326 Table S1, 454): 24 levels, 16 heads, head_dim 1024 / 16 =
     64, NATTEN kernel size 9 (read as 9 x 9 x 9, DESIGN.md R2), tiles of 64 x 64 or 128 x 128 cells at patch size 4;
     inputs as QK-RMSNorm leaves them.  "col*": the column-wise attention blocks that alternate with
-    them: every level of one (y, x) column.  Not BASELINE.json configs: extra bench / parity shapes."""
+    them: every level of one (y, x) column.  "dec64": the de-aliasing decoder's NA3D blocks (PAPER.md:326:
+    embedding dimension 128, NA3D kernel size 9, at full horizontal resolution: the 64 x 64 cells of a 16 x 16-patch
+    tile, 24 levels); the paper gives no head count for it -- read as ONE head of 128 channels (R26; two
+    heads of 64 would be the prod shapes' kernel).  Not BASELINE.json configs: extra bench / parity shapes."""
     s = BASE_SEED + 50
+    if which == "dec64":
+        return Workload("dec64_fwd", -1, 2, 1, 128, (24, 64, 64), (9, 9, 9), "bf16", value_scale="qknorm", seed=s)
     shapes = {"prod16": ((24, 16, 16), (9, 9, 9)), "prod32": ((24, 32, 32), (9, 9, 9)),
               "col16": ((24, 16, 16), (24, 1, 1)), "col32": ((24, 32, 32), (24, 1, 1))}
     grid, window = shapes[which]

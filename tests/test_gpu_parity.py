@@ -472,6 +472,38 @@ def test_production_window_9x9x9_on_the_tensor_cores(oracle_mod, case):
     check_full(oracle_mod, w, binding.IMPL_AUTO)
 
 
+def test_production_shape_at_the_size_the_bench_times(oracle_mod):
+    """workloads.production("prod32") as bench.py runs it: 24 x 32 x 32 tokens, 16 heads, batch 2, window 9 x 9 x 9 --
+    every element of O, LSE, dQ, dK, dV against the oracle (about a minute of oracle time)."""
+    check_full(oracle_mod, wl.production("prod32"), binding.IMPL_AUTO)
+
+
+@pytest.mark.parametrize("case", [dict(grid=(10, 17, 19), heads=1), dict(grid=(24, 16, 16), heads=2),
+                                  dict(grid=(9, 12, 9), heads=1, batch=2, rope_pairing=1)])
+def test_decoder_window_9x9x9_with_head_dim_128(oracle_mod, case):
+    """PAPER.md:326, the de-aliasing decoder's NA3D blocks: embedding 128 (one head of 128 channels, reading R26),
+    kernel 9.  Forward on the tcgen05 tile kernel (Cfg<128, 9, 9, 9>); the d = 128 backward runs on the CUDA cores."""
+    w = wl.small(name="dec999", dtype="bf16", value_scale="qknorm", window=(9, 9, 9), head_dim=128, **case)
+    assert binding.strata_na3d_impl_selected(desc_of(w)) == binding.IMPL_TCGEN05
+    assert binding.strata_na3d_impl_selected(desc_of(w), True) == binding.IMPL_SIMT
+    check_full(oracle_mod, w, binding.IMPL_AUTO)
+
+
+def test_decoder_shape_sampled_rows_at_bench_size(oracle_mod):
+    """workloads.production("dec64") (24 x 64 x 64 tokens, one head of 128, batch 2) in the launch configuration bench.py
+    times: 4096 random rows against the oracle, every output finite."""
+    w = wl.production("dec64")
+    inp = wl.make_inputs(w)
+    d, o, lse = run_fwd(w, inp)
+    assert bool(torch.isfinite(o.float()).all()) and bool(torch.isfinite(lse).all())
+    idx = np.sort(np.random.default_rng(3).choice(w.batch * w.tokens * w.heads, size=4096, replace=False))
+    o_ref, lse_ref = oracle_mod.na3d_fwd_queries(inp["q"], inp["k"], inp["v"], inp["coords"], inp["freqs"], w.window, idx)
+    assert w.heads == 1                                      # (so that LSE [B, H, N] and the row index (b N + t) H + h coincide)
+    got_o = to_f64(o).reshape(-1, w.head_dim)[idx]
+    assert_parity(got_o, np.asarray(o_ref).reshape(-1, w.head_dim), "bf16", "dec64 sampled O")
+    assert_parity(to_f64(lse).reshape(-1)[idx], np.asarray(lse_ref).reshape(-1), "bf16", "dec64 sampled LSE", rms_bound=1e-2)
+
+
 @pytest.mark.parametrize("case", [dict(grid=(24, 5, 7), heads=3), dict(grid=(8, 9, 6), heads=2, batch=2),
                                   dict(grid=(32, 3, 4), heads=1, rope_pairing=1), dict(grid=(5, 4, 4), heads=2, rope_axes=0)])
 def test_column_attention(oracle_mod, case):
@@ -524,7 +556,8 @@ def test_column_attention_with_level_dependent_coordinates(oracle_mod):
 @pytest.mark.parametrize("case", [dict(dtype="bf16", grid=(8, 18, 21), window=(3, 7, 7), heads=2, head_dim=64),          # fused fwd, tcgen05 bwd
                                   dict(dtype="bf16", grid=(6, 10, 9), window=(5, 9, 9), heads=1, head_dim=128),         # tile fwd, SIMT bwd
                                   dict(dtype="f32", grid=(3, 6, 7), window=(3, 3, 3), heads=2, head_dim=32),
-                                  dict(dtype="bf16", grid=(5, 9, 12), window=(3, 5, 5), heads=3, head_dim=64, gate=False)])
+                                  dict(dtype="bf16", grid=(5, 9, 12), window=(3, 5, 5), heads=3, head_dim=64, gate=False),
+                                  dict(dtype="bf16", grid=(8, 64, 64), window=(3, 7, 7), heads=8, head_dim=64, batch=4)])  # config 1's size
 def test_qk_rmsnorm_and_head_gate(oracle_mod, case):
     kw = dict(case)
     with_gate = kw.pop("gate", True)
