@@ -993,7 +993,10 @@ cudaError_t launch_fix_rows(const Problem& p, const void* q, const void* k, cons
   if (p.D != 64 && p.D != 128) return cudaErrorInvalidValue;
   prof_begin("na3d_fix_rows", stream);
   auto kernel = p.D == 64 ? na3d_fix_rows_kernel<64> : na3d_fix_rows_kernel<128>;
-  kernel<<<148, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, coords, freqs,
+  // One warp per listed row, grid-stride.  8 blocks of 4 warps per SM: an empty list costs the same few microseconds
+  // as a smaller grid (every block reads two words and returns), while the take-all case (list overflow, level-dependent
+  // coordinates: every row of the problem) gets 32 warps per SM instead of 4 to hide its fp64 sincos and gather latency.
+  kernel<<<148 * 8, 128, 0, stream>>>((const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, coords, freqs,
                                   (__nv_bfloat16*)o, lse, reinterpret_cast<const unsigned long long*>(fix), kFixCap, p);
   prof_end(stream);
   if (launches) ++*launches;
